@@ -1,0 +1,139 @@
+/*
+ * tm.h -- C-ABI boundary of the B200-native even-odd preconditioned Wilson twisted-mass dslash
+ * (hot path of arXiv 1311.4462; citations are PAPER.md:<line> + section / equation).
+ *
+ * Operator (Eq. 2.1; readings C1-C3), hopping-parameter normalisation:
+ *     M = 2 kappa D = R - kappa D_hop,     R = 1 + i a gamma5 tau3 + b tau1,  a = 2 kappa mu,  b = 2 kappa epsilon
+ *     (D_hop psi)(x) = sum_mu  eta+ (1 - gamma_mu) U_mu(x) psi(x+mu) + eta- (1 + gamma_mu) U_mu(x-mu)^dag psi(x-mu)
+ * periodic in space; in time the wrapped hop is multiplied by t_boundary (-1 = antiperiodic).
+ * gamma matrices: gamma_4-diagonal "non-relativistic" basis (C5):
+ *     gamma_k = [[0, i sigma_k], [-i sigma_k, 0]],  gamma_4 = diag(1,1,-1,-1),  gamma_5 = [[0,1],[1,0]].
+ *
+ * Everything runs on ONE GPU (sm_100a); there is no CPU fallback.  All functions return TM_OK (0) or a
+ * negative tm_status; they never throw, abort or print.  tm_last_error() gives a thread-local message.
+ *
+ * HOST canonical order (always double, complex = (re, im), C-contiguous; never retained after return):
+ *     spinor, full lattice : [flavor (n_flavor)][lex site (V)][spin 4][color 3][2]
+ *     spinor, one parity   : [flavor (n_flavor)][cb  site (V/2)][spin 4][color 3][2]
+ *     gauge                : [mu 0..3 = x,y,z,t][lex site (V)][row 3][col 3][2]  = U_mu(x), the link x -> x+mu,
+ *                            pure SU(3), no boundary phase folded in
+ *     lex = x1 + X (x2 + Y (x3 + Z x4)),  parity = (x1+x2+x3+x4) & 1 (0 = even),  cb = lex / 2.
+ * DEVICE layout is private to the library: checkerboarded SoA in 128-bit chunks.
+ */
+#ifndef TM_H
+#define TM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TM_OK = 0,
+    TM_ERR_ARG = -1,          /* NULL handle / pointer, bad enum value                                   */
+    TM_ERR_DIMS = -2,         /* an extent is odd or < 4 (the checkerboard needs even extents; at extent 2
+                                 the forward and backward neighbours coincide)                           */
+    TM_ERR_MISMATCH = -3,     /* operands differ in context, precision or flavor count; gauge precision
+                                 differs from the fields'; params.twist_flavor disagrees with n_flavor   */
+    TM_ERR_ALIAS = -4,        /* out aliases in (neighbour reads make in-place application impossible)   */
+    TM_ERR_PARAM = -5,        /* |1 + a^2 - b^2| < 1e-12: R has no inverse; or epsilon != 0 with a single
+                                 flavor; or t_boundary not +-1                                           */
+    TM_ERR_NOMEM = -6,
+    TM_ERR_CUDA = -7,         /* a CUDA call failed; tm_last_error() holds cudaGetErrorString            */
+    TM_ERR_UNSUPPORTED = -8   /* tm_mat_pc(TM_MATPC_SYM, dagger=1): needs the D R^-1 ordering */
+} tm_status;
+
+typedef enum { TM_DOUBLE = 8, TM_SINGLE = 4, TM_HALF = 2 } tm_precision;
+/* TM_HALF: 16-bit fixed point, one float norm per (site, flavor): q = rint(v * 32767 / max|v|)
+ * (Table 1 "half"; format per DESIGN.md reading C9); arithmetic in fp32.              */
+
+typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12 } tm_recon;
+/* TM_RECON_12: rows 0 and 1 stored, row 2 = conj(row0 x row1) rebuilt in the kernel.      */
+
+typedef enum { TM_EVEN = 0, TM_ODD = 1 } tm_parity;
+
+typedef enum {                       /* the fused kernels of PAPER.md:68 (section 2.1); p = output parity */
+    TM_TWIST_INV_DSLASH = 0,         /* A      : out_p = R^-1 D_hop in                                   */
+    TM_TWIST_INV_DSLASH_XPAY = 1,    /* A-xpay : out_p = x_p - kappa^2 R^-1 D_hop in                     */
+    TM_DSLASH_TWIST_XPAY = 2,        /* B      : out_p = R x_p - kappa^2 D_hop in                        */
+    TM_RECONSTRUCT = 3               /* REC    : out_p = R^-1 (x_p + kappa D_hop in)     (Eq. 2.4)       */
+} tm_kernel_type;
+/* dagger != 0: D_hop -> D_hop^dag (projectors swapped) and R -> R^dag (a -> -a), order kept.            */
+
+typedef enum { TM_MATPC_ASYM = 0 /* LHS of Eq. 2.2 */, TM_MATPC_SYM = 1 /* LHS of Eq. 2.3 */ } tm_matpc;
+
+typedef struct {
+    double kappa, mu, epsilon;   /* bare mu-bar, epsilon-bar                          */
+    int twist_flavor;            /* +1 / -1: one flavor, tau3 -> +-1, epsilon must be 0 (QUDA_TWIST_PLUS /
+                                    MINUS); 0: non-degenerate doublet (n_flavor = 2)     */
+    int t_boundary;              /* -1 antiperiodic in time, +1 periodic                                 */
+} tm_params;
+
+typedef struct tm_ctx tm_ctx;       /* lattice geometry + device + stream                                 */
+typedef struct tm_field tm_field;   /* ONE single-parity spinor field (V/2 sites, n_flavor flavors)       */
+typedef struct tm_gauge tm_gauge;   /* all 4V links, both parities                                        */
+
+/* ---- context ------------------------------------------------------------------------------------- */
+/* dims: host pointer to {X, Y, Z, T}. Selects cuda_device for the calling thread. */
+int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx);
+/* cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default stream.
+ * All later compute calls on this context are enqueued there. */
+int tm_set_stream(tm_ctx *ctx, void *cuda_stream);
+int tm_sync(tm_ctx *ctx);           /* cudaStreamSynchronize; surfaces asynchronous faults */
+void tm_finalize(tm_ctx *ctx);      /* does not free fields / gauges created from it */
+
+/* ---- fields (a1 of DESIGN.md: checkerboarded SoA layouts) ------------------------------------------ */
+size_t tm_field_bytes(const tm_ctx *ctx, tm_precision prec, int n_flavor);   /* 0 on bad arguments */
+/* ext_dev_ptr == NULL: the library allocates (and frees in tm_field_free).  Otherwise ext_dev_ptr is DEVICE
+ * memory of at least tm_field_bytes() bytes, 256-byte aligned, BORROWED (e.g. a torch tensor's storage). */
+int tm_field_alloc(tm_ctx *ctx, tm_precision prec, int n_flavor, void *ext_dev_ptr, size_t ext_bytes,
+                   tm_field **f);
+void tm_field_free(tm_field *f);
+void *tm_field_device_ptr(const tm_field *f);
+/* host_full: HOST pointer, full-lattice canonical spinor; only the sites of `parity` are read / written.
+ * Both calls synchronise the context stream. */
+int tm_field_upload(tm_field *f, tm_parity parity, const double *host_full);
+int tm_field_download(const tm_field *f, tm_parity parity, double *host_full);
+/* host_cb: HOST pointer, single-parity canonical spinor [n_flavor][V/2][4][3][2] in cb order of `parity`.
+ * (The cb order does not depend on the parity; the argument is kept for symmetry and validated.) */
+int tm_field_upload_cb(tm_field *f, tm_parity parity, const double *host_cb);
+int tm_field_download_cb(const tm_field *f, tm_parity parity, double *host_cb);
+
+/* ---- gauge (a1, a4) -------------------------------------------------------------------------------- */
+/* host_links: HOST pointer, canonical gauge field; copied (may be freed on return). */
+int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_recon recon, tm_gauge **g);
+void tm_gauge_free(tm_gauge *g);
+
+/* ---- the hot path ---------------------------------------------------------------------------------- */
+/* One fused kernel launch (rows a2-a9 of DESIGN.md).  out: field on `parity`; in: field on the
+ * opposite parity; x: field on `parity` (NULL allowed only for TM_TWIST_INV_DSLASH).  out must not alias in
+ * (TM_ERR_ALIAS); out may alias x.  `prec` must equal the operands' precision (TM_ERR_MISMATCH).
+ * Asynchronous: enqueues on the context stream and returns. */
+int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const tm_gauge *g,
+                    const tm_params *p, tm_parity parity, int dagger, tm_kernel_type kt, tm_precision prec);
+
+/* LHS of Eq. 2.2 (ASYM: out_e = (R_ee - kappa^2 D_eo R_oo^-1 D_oe) in_e) or Eq. 2.3 (SYM:
+ * out_e = (1 - kappa^2 R_ee^-1 D_eo R_oo^-1 D_oe) in_e): two launches, tmp_o is the odd
+ * intermediate R_oo^-1 D_oe in_e.  dagger: the same two launches with the daggered kernels -- the exact
+ * adjoint for ASYM; SYM + dagger returns TM_ERR_UNSUPPORTED.  Asynchronous. */
+int tm_mat_pc(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p,
+              tm_matpc type, int dagger);
+
+/* Eq. 2.4 (reading C4): psi_o = R_oo^-1 (b_o + kappa D_oe psi_e).  psi_o may alias b_o. */
+int tm_reconstruct_odd(tm_field *psi_o, const tm_field *psi_e, const tm_field *b_o, const tm_gauge *g,
+                       const tm_params *p);
+
+/* ---- diagnostics ----------------------------------------------------------------------------------- */
+const char *tm_last_error(void);       /* thread-local, never NULL */
+/* Number of dslash kernel launches issued through this context so far (bench.py's gpu_launches). */
+long tm_launch_count(const tm_ctx *ctx);
+/* Name of the kernel variant the last tm_dslash_apply on this context dispatched to (static string). */
+const char *tm_last_kernel_name(const tm_ctx *ctx);
+/* Force a code path: 0 = automatic (default), 1 = generic direct-load kernels only.  For tests / profiling. */
+int tm_set_path(tm_ctx *ctx, int path);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TM_H */

@@ -1,0 +1,324 @@
+// tm_api.cu -- the C-ABI boundary declared in include/tm.h: handles, validation, dispatch.
+// No arithmetic of the method lives here except forming a = 2 kappa mu, b = 2 kappa epsilon and the
+// twist coefficients in double (reading C2, C10-ii).
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "tm_internal.h"
+
+const TmKernelEntry *tm_generic_table_8_1();
+const TmKernelEntry *tm_generic_table_8_2();
+const TmKernelEntry *tm_generic_table_4_1();
+const TmKernelEntry *tm_generic_table_4_2();
+const TmKernelEntry *tm_generic_table_2_1();
+const TmKernelEntry *tm_generic_table_2_2();
+
+const TmKernelEntry *tm_generic_table(int prec, int nf)
+{
+    if (prec == 8) return nf == 1 ? tm_generic_table_8_1() : tm_generic_table_8_2();
+    if (prec == 4) return nf == 1 ? tm_generic_table_4_1() : tm_generic_table_4_2();
+    return nf == 1 ? tm_generic_table_2_1() : tm_generic_table_2_2();
+}
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+int cuda_fail(cudaError_t e, const char *what)
+{
+    return fail(TM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+bool valid_prec(int p) { return p == TM_DOUBLE || p == TM_SINGLE || p == TM_HALF; }
+
+size_t field_bytes(const TmGeom &g, int prec, int nf)
+{
+    size_t b = (size_t)nf * g.Vh * tm_spinor_site_bytes(prec);
+    if (prec == TM_HALF) b += (size_t)nf * g.Vh * sizeof(float);
+    return b;
+}
+
+bool overlap(const tm_field *a, const tm_field *b)
+{
+    const char *pa = static_cast<const char *>(a->ptr), *pb = static_cast<const char *>(b->ptr);
+    return pa < pb + b->bytes && pb < pa + a->bytes;
+}
+
+// RAII device staging buffer for upload / download (not hot)
+struct Staging {
+    void *p = nullptr;
+    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes); }
+    ~Staging() { if (p) cudaFree(p); }
+};
+
+struct Coeffs {
+    double alpha, beta, scale;
+};
+
+// a = 2 kappa mu, b = 2 kappa epsilon; R = 1 + i a g5 tau3 + b tau1; R^-1 = (1 - i a g5 tau3 - b tau1)/(1 + a^2 - b^2)
+int make_coeffs(const tm_params *p, int nf, int dagger, int kt, Coeffs *c)
+{
+    if (!(p->t_boundary == 1 || p->t_boundary == -1)) return fail(TM_ERR_PARAM, "t_boundary must be +1 or -1");
+    if (nf == 1 && !(p->twist_flavor == 1 || p->twist_flavor == -1))
+        return fail(TM_ERR_MISMATCH, "single-flavor fields need twist_flavor = +1 or -1 (got %d)", p->twist_flavor);
+    if (nf == 2 && p->twist_flavor != 0)
+        return fail(TM_ERR_MISMATCH, "doublet fields need twist_flavor = 0 (got %d)", p->twist_flavor);
+    if (nf == 1 && p->epsilon != 0.0) return fail(TM_ERR_PARAM, "epsilon must be 0 for a single flavor (PAPER.md:87)");
+    double a = 2.0 * p->kappa * p->mu, b = 2.0 * p->kappa * p->epsilon;
+    if (dagger) a = -a;
+    if (nf == 1) { a *= (double)p->twist_flavor; b = 0.0; }
+    if (kt == TM_DSLASH_TWIST_XPAY) {
+        c->alpha = a; c->beta = b; c->scale = 1.0;
+    } else {
+        const double den = 1.0 + a * a - b * b;
+        if (std::fabs(den) < 1e-12) return fail(TM_ERR_PARAM, "1 + a^2 - b^2 = %g: R is singular", den);
+        c->alpha = -a; c->beta = -b; c->scale = 1.0 / den;
+    }
+    return TM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *tm_last_error(void) { return g_err; }
+
+int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
+{
+    if (!dims || !ctx) return fail(TM_ERR_ARG, "tm_init: NULL argument");
+    *ctx = nullptr;
+    for (int d = 0; d < 4; d++)
+        if (dims[d] < 4 || (dims[d] & 1)) return fail(TM_ERR_DIMS, "extent %d = %d must be even and >= 4", d, dims[d]);
+    const long V = (long)dims[0] * dims[1] * dims[2] * dims[3];
+    if (V / 2 > 0x3fffffffL) return fail(TM_ERR_DIMS, "lattice too large for 32-bit site indices");
+    cudaError_t e = cudaSetDevice(cuda_device);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaSetDevice");
+    tm_ctx *c = new (std::nothrow) tm_ctx();
+    if (!c) return fail(TM_ERR_NOMEM, "out of host memory");
+    for (int d = 0; d < 4; d++) c->g.X[d] = dims[d];
+    c->g.Xh = dims[0] / 2;
+    c->g.V = V;
+    c->g.Vh = (int)(V / 2);
+    c->device = cuda_device;
+    c->stream = 0;
+    c->launches = 0;
+    c->last_kernel = "";
+    c->path = 0;
+    c->sm_count = 0;
+    e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
+    if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaDeviceGetAttribute"); }
+    *ctx = c;
+    return TM_OK;
+}
+
+int tm_set_stream(tm_ctx *ctx, void *cuda_stream)
+{
+    if (!ctx) return fail(TM_ERR_ARG, "tm_set_stream: NULL context");
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+    return TM_OK;
+}
+
+int tm_sync(tm_ctx *ctx)
+{
+    if (!ctx) return fail(TM_ERR_ARG, "tm_sync: NULL context");
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
+    return TM_OK;
+}
+
+void tm_finalize(tm_ctx *ctx) { delete ctx; }
+
+int tm_set_path(tm_ctx *ctx, int path)
+{
+    if (!ctx || path < 0 || path > 1) return fail(TM_ERR_ARG, "tm_set_path: bad argument");
+    ctx->path = path;
+    return TM_OK;
+}
+
+long tm_launch_count(const tm_ctx *ctx) { return ctx ? ctx->launches : 0; }
+const char *tm_last_kernel_name(const tm_ctx *ctx) { return ctx ? ctx->last_kernel : ""; }
+
+size_t tm_field_bytes(const tm_ctx *ctx, tm_precision prec, int n_flavor)
+{
+    if (!ctx || !valid_prec(prec) || n_flavor < 1 || n_flavor > 2) return 0;
+    return field_bytes(ctx->g, prec, n_flavor);
+}
+
+int tm_field_alloc(tm_ctx *ctx, tm_precision prec, int n_flavor, void *ext_dev_ptr, size_t ext_bytes, tm_field **f)
+{
+    if (!ctx || !f) return fail(TM_ERR_ARG, "tm_field_alloc: NULL argument");
+    *f = nullptr;
+    if (!valid_prec(prec)) return fail(TM_ERR_ARG, "bad precision %d", (int)prec);
+    if (n_flavor < 1 || n_flavor > 2) return fail(TM_ERR_ARG, "n_flavor must be 1 or 2");
+    const size_t bytes = field_bytes(ctx->g, prec, n_flavor);
+    tm_field *fl = new (std::nothrow) tm_field();
+    if (!fl) return fail(TM_ERR_NOMEM, "out of host memory");
+    fl->ctx = ctx; fl->prec = prec; fl->nf = n_flavor; fl->bytes = bytes;
+    if (ext_dev_ptr) {
+        if (ext_bytes < bytes) { delete fl; return fail(TM_ERR_ARG, "external buffer has %zu bytes, need %zu", ext_bytes, bytes); }
+        if (reinterpret_cast<size_t>(ext_dev_ptr) & 255) { delete fl; return fail(TM_ERR_ARG, "external buffer must be 256-byte aligned"); }
+        fl->ptr = ext_dev_ptr; fl->owns = false;
+    } else {
+        cudaError_t e = cudaMalloc(&fl->ptr, bytes);
+        if (e != cudaSuccess) { delete fl; cudaGetLastError(); return fail(TM_ERR_NOMEM, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e)); }
+        fl->owns = true;
+    }
+    *f = fl;
+    return TM_OK;
+}
+
+void tm_field_free(tm_field *f)
+{
+    if (!f) return;
+    if (f->owns && f->ptr) cudaFree(f->ptr);
+    delete f;
+}
+
+void *tm_field_device_ptr(const tm_field *f) { return f ? f->ptr : nullptr; }
+
+static int field_upload(tm_field *f, int parity, const double *host, bool cb)
+{
+    if (!f || !host) return fail(TM_ERR_ARG, "tm_field_upload: NULL argument");
+    if (parity != 0 && parity != 1) return fail(TM_ERR_ARG, "bad parity %d", parity);
+    tm_ctx *c = f->ctx;
+    const size_t n = (size_t)f->nf * (cb ? (size_t)c->g.Vh : (size_t)c->g.V) * 24 * sizeof(double);
+    Staging st;
+    cudaError_t e = st.alloc(n);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
+    e = cudaMemcpyAsync(st.p, host, n, cudaMemcpyHostToDevice, c->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync H2D");
+    e = tm_pack_spinor(f, parity, static_cast<const double *>(st.p), cb, c->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "pack_spinor launch");
+    e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "upload sync");
+    return TM_OK;
+}
+
+static int field_download(const tm_field *f, int parity, double *host, bool cb)
+{
+    if (!f || !host) return fail(TM_ERR_ARG, "tm_field_download: NULL argument");
+    if (parity != 0 && parity != 1) return fail(TM_ERR_ARG, "bad parity %d", parity);
+    tm_ctx *c = f->ctx;
+    const size_t n = (size_t)f->nf * (cb ? (size_t)c->g.Vh : (size_t)c->g.V) * 24 * sizeof(double);
+    Staging st;
+    cudaError_t e = st.alloc(n);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
+    if (!cb) {   // only this parity's sites are written: start from the caller's array
+        e = cudaMemcpyAsync(st.p, host, n, cudaMemcpyHostToDevice, c->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync H2D");
+    }
+    e = tm_unpack_spinor(f, parity, static_cast<double *>(st.p), cb, c->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "unpack_spinor launch");
+    e = cudaMemcpyAsync(host, st.p, n, cudaMemcpyDeviceToHost, c->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync D2H");
+    e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "download sync");
+    return TM_OK;
+}
+
+int tm_field_upload(tm_field *f, tm_parity parity, const double *host_full) { return field_upload(f, parity, host_full, false); }
+int tm_field_download(const tm_field *f, tm_parity parity, double *host_full) { return field_download(f, parity, host_full, false); }
+int tm_field_upload_cb(tm_field *f, tm_parity parity, const double *host_cb) { return field_upload(f, parity, host_cb, true); }
+int tm_field_download_cb(const tm_field *f, tm_parity parity, double *host_cb) { return field_download(f, parity, host_cb, true); }
+
+int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_recon recon, tm_gauge **g)
+{
+    if (!ctx || !host_links || !g) return fail(TM_ERR_ARG, "tm_gauge_load: NULL argument");
+    *g = nullptr;
+    if (!valid_prec(prec)) return fail(TM_ERR_ARG, "bad precision %d", (int)prec);
+    if (recon != TM_RECON_18 && recon != TM_RECON_12) return fail(TM_ERR_ARG, "bad recon %d", (int)recon);
+    tm_gauge *gg = new (std::nothrow) tm_gauge();
+    if (!gg) return fail(TM_ERR_NOMEM, "out of host memory");
+    gg->ctx = ctx; gg->prec = prec; gg->recon = recon;
+    gg->bytes = (size_t)8 * ctx->g.Vh * tm_link_site_bytes(prec, recon);
+    cudaError_t e = cudaMalloc(&gg->ptr, gg->bytes);
+    if (e != cudaSuccess) { delete gg; cudaGetLastError(); return fail(TM_ERR_NOMEM, "cudaMalloc(%zu): %s", gg->bytes, cudaGetErrorString(e)); }
+    const size_t n = (size_t)4 * ctx->g.V * 18 * sizeof(double);
+    Staging st;
+    e = st.alloc(n);
+    if (e != cudaSuccess) { tm_gauge_free(gg); cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
+    e = cudaMemcpyAsync(st.p, host_links, n, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = tm_pack_gauge(gg, static_cast<const double *>(st.p), ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) { tm_gauge_free(gg); return cuda_fail(e, "tm_gauge_load"); }
+    *g = gg;
+    return TM_OK;
+}
+
+void tm_gauge_free(tm_gauge *g)
+{
+    if (!g) return;
+    if (g->ptr) cudaFree(g->ptr);
+    delete g;
+}
+
+int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const tm_gauge *g, const tm_params *p,
+                    tm_parity parity, int dagger, tm_kernel_type kt, tm_precision prec)
+{
+    if (!out || !in || !g || !p) return fail(TM_ERR_ARG, "tm_dslash_apply: NULL argument");
+    if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
+    if ((int)kt < 0 || (int)kt > 3) return fail(TM_ERR_ARG, "bad kernel type %d", (int)kt);
+    if (kt != TM_TWIST_INV_DSLASH && !x) return fail(TM_ERR_ARG, "kernel type %d needs x", (int)kt);
+    tm_ctx *c = out->ctx;
+    if (in->ctx != c || g->ctx != c || (x && x->ctx != c)) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
+    if (out->prec != (int)prec || in->prec != (int)prec || g->prec != (int)prec || (x && x->prec != (int)prec))
+        return fail(TM_ERR_MISMATCH, "precision mismatch (call %d, out %d, in %d, gauge %d)", (int)prec, out->prec, in->prec, g->prec);
+    if (in->nf != out->nf || (x && x->nf != out->nf)) return fail(TM_ERR_MISMATCH, "flavor count mismatch");
+    if (overlap(out, in)) return fail(TM_ERR_ALIAS, "out aliases in");
+    Coeffs co;
+    int rc = make_coeffs(p, out->nf, dagger ? 1 : 0, (int)kt, &co);
+    if (rc) return rc;
+
+    DslashArgs a;
+    a.out = out->ptr; a.in = in->ptr; a.x = x ? x->ptr : nullptr; a.gauge = g->ptr;
+    a.X = c->g.X[0]; a.Y = c->g.X[1]; a.Z = c->g.X[2]; a.T = c->g.X[3]; a.Xh = c->g.Xh; a.Vh = c->g.Vh;
+    a.parity = (int)parity;
+    a.alpha = co.alpha; a.beta = co.beta; a.scale = co.scale;
+    a.kappa = p->kappa; a.kappa2 = p->kappa * p->kappa;
+    a.tbound = (double)p->t_boundary;
+
+    const TmKernelEntry *tab = tm_generic_table((int)prec, out->nf);
+    const TmKernelEntry &k = tab[((g->recon == 18 ? 0 : 1) * 4 + (int)kt) * 2 + (dagger ? 1 : 0)];
+    cudaError_t e = k.fn(a, c->stream);
+    if (e != cudaSuccess) return cuda_fail(e, k.name);
+    c->launches++;
+    c->last_kernel = k.name;
+    return TM_OK;
+}
+
+int tm_mat_pc(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p,
+              tm_matpc type, int dagger)
+{
+    if (!out_e || !in_e || !tmp_o || !g || !p) return fail(TM_ERR_ARG, "tm_mat_pc: NULL argument");
+    if (type != TM_MATPC_ASYM && type != TM_MATPC_SYM) return fail(TM_ERR_ARG, "bad matpc type %d", (int)type);
+    if (type == TM_MATPC_SYM && dagger)
+        return fail(TM_ERR_UNSUPPORTED, "SYM dagger needs the D R^-1 kernel ordering (DESIGN.md C7, NEXT-1)");
+    if (overlap(tmp_o, in_e) || overlap(tmp_o, out_e)) return fail(TM_ERR_ALIAS, "tmp_o aliases in_e or out_e");
+    const tm_precision prec = (tm_precision)out_e->prec;
+    // tmp_o = R_oo^-1 D_oe in_e
+    int rc = tm_dslash_apply(tmp_o, in_e, nullptr, g, p, TM_ODD, dagger, TM_TWIST_INV_DSLASH, prec);
+    if (rc) return rc;
+    // ASYM: out_e = R_ee in_e - kappa^2 D_eo tmp_o ;  SYM: out_e = in_e - kappa^2 R_ee^-1 D_eo tmp_o
+    return tm_dslash_apply(out_e, tmp_o, in_e, g, p, TM_EVEN, dagger,
+                           type == TM_MATPC_ASYM ? TM_DSLASH_TWIST_XPAY : TM_TWIST_INV_DSLASH_XPAY, prec);
+}
+
+int tm_reconstruct_odd(tm_field *psi_o, const tm_field *psi_e, const tm_field *b_o, const tm_gauge *g, const tm_params *p)
+{
+    if (!psi_o || !psi_e || !b_o || !g || !p) return fail(TM_ERR_ARG, "tm_reconstruct_odd: NULL argument");
+    return tm_dslash_apply(psi_o, psi_e, b_o, g, p, TM_ODD, 0, TM_RECONSTRUCT, (tm_precision)psi_o->prec);
+}
+
+}  // extern "C"

@@ -1,0 +1,4 @@
+// Instantiations of the generic fused dslash kernel: precision code 4 (bytes per real), 2 flavor(s).
+#include "tm_dslash.cuh"
+
+TM_GENERIC_TABLE(4, 2)

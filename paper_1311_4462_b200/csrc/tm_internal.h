@@ -1,0 +1,85 @@
+// tm_internal.h -- private structures shared by the C-ABI layer (tm_api.cu) and the kernel launchers.
+// Device layout (row a1):
+//   spinor, one parity : [flavor][chunk][cb site] in 128-bit chunks
+//        fp64: 12 chunks of double2 (one complex each, index spin*3+color)
+//        fp32:  6 chunks of float4  (two complex each)
+//        half:  3 chunks of 8 x int16, followed by float norm[flavor][cb site]
+//   gauge : [parity][mu][plane][cb site]; a link's reals r = (row*3+col)*2+reim are cut into planes
+//        fp64: recon planes of double2              (9 for 18-real, 6 for 12-real)
+//        fp32: 18 -> 4 x float4 + 1 x float2 ; 12 -> 3 x float4
+//        half: 18 -> 2 x int4(8 x int16) + 1 x int(2 x int16) ; 12 -> 1 x int4 + 1 x int2
+//   [parity][mu] block holds U_mu(x) for the sites x of that parity.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+#include "../../include/tm.h"
+
+struct TmGeom {
+    int X[4];
+    int Xh;      // X/2
+    int Vh;      // V/2
+    long V;
+};
+
+struct tm_ctx {
+    TmGeom g;
+    int device;
+    cudaStream_t stream;
+    long launches;
+    const char *last_kernel;
+    int path;    // 0 auto, 1 generic only
+    int sm_count;
+};
+
+struct tm_field {
+    tm_ctx *ctx;
+    int prec;    // 8 / 4 / 2
+    int nf;      // 1 / 2
+    void *ptr;
+    size_t bytes;
+    bool owns;
+};
+
+struct tm_gauge {
+    tm_ctx *ctx;
+    int prec;
+    int recon;
+    void *ptr;
+    size_t bytes;
+};
+
+// bytes of one flavor's chunk block per site (without norms) and of one link per site
+static inline size_t tm_spinor_site_bytes(int prec) { return (size_t)24 * (size_t)prec; }
+static inline size_t tm_link_site_bytes(int prec, int recon) { return (size_t)recon * (size_t)prec; }
+
+// Arguments of one fused dslash launch.  Coefficients are formed in double on the host (reading C10-ii)
+// and cast to the kernel's arithmetic type on the device.
+struct DslashArgs {
+    void *out;
+    const void *in;
+    const void *x;
+    const void *gauge;
+    int X, Y, Z, T, Xh, Vh;
+    int parity;          // parity of the output sites
+    double alpha;        // local twist, flavor 0:  w = scale * (v + i alpha gamma5 v + beta v_otherflavor)
+    double beta;
+    double scale;
+    double kappa;        // REC
+    double kappa2;       // A-xpay, B
+    double tbound;       // +-1, multiplies the time hop that wraps
+};
+
+// kernel launchers (one translation unit per precision x flavor count)
+typedef cudaError_t (*tm_launch_fn)(const DslashArgs &, cudaStream_t);
+struct TmKernelEntry {
+    tm_launch_fn fn;
+    const char *name;
+};
+// index: [recon18?0:1][kt 0..3][dagger 0..1]
+const TmKernelEntry *tm_generic_table(int prec, int nf);
+
+// pack / unpack (tm_pack.cu)
+cudaError_t tm_pack_spinor(const tm_field *f, int parity, const double *dev_src, bool src_is_cb, cudaStream_t s);
+cudaError_t tm_unpack_spinor(const tm_field *f, int parity, double *dev_dst, bool dst_is_cb, cudaStream_t s);
+cudaError_t tm_pack_gauge(const tm_gauge *g, const double *dev_src, cudaStream_t s);

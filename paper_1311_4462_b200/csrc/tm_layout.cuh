@@ -1,0 +1,190 @@
+// tm_layout.cuh -- register <-> device-layout moves for spinors and links (rows a1, a4, a8 of DESIGN.md).
+// A site's spinor is 24 reals v[(spin*3+color)*2+reim]; "upper" = spin 0,1 = v[0..11], "lower" = v[12..23].
+// A link is 18 reals u[(row*3+col)*2+reim].
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define TM_DEV __device__ __forceinline__
+
+template <int PREC> struct PrecTraits;
+template <> struct PrecTraits<8> { typedef double real; static constexpr int NCH = 12; };
+template <> struct PrecTraits<4> { typedef float real;  static constexpr int NCH = 6; };
+template <> struct PrecTraits<2> { typedef float real;  static constexpr int NCH = 3; };
+
+#define TM_HALF_MAX 32767.0f
+#define TM_HALF_INV (1.0f / 32767.0f)
+
+// ---- raw 128-bit global accesses ------------------------------------------------------------------
+TM_DEV double2 ldg_d2(const void *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
+TM_DEV float4 ldg_f4(const void *p) { return __ldg(reinterpret_cast<const float4 *>(p)); }
+TM_DEV float2 ldg_f2(const void *p) { return __ldg(reinterpret_cast<const float2 *>(p)); }
+TM_DEV int4 ldg_i4(const void *p) { return __ldg(reinterpret_cast<const int4 *>(p)); }
+TM_DEV int2 ldg_i2(const void *p) { return __ldg(reinterpret_cast<const int2 *>(p)); }
+TM_DEV int ldg_i1(const void *p) { return __ldg(reinterpret_cast<const int *>(p)); }
+TM_DEV float ldg_f1(const void *p) { return __ldg(reinterpret_cast<const float *>(p)); }
+
+// two int16 packed in one 32-bit word -> two floats (exact), times s
+TM_DEV void unpack2(int w, float s, float &lo, float &hi)
+{
+    lo = (float)(short)(w & 0xffff) * s;
+    hi = (float)(w >> 16) * s;
+}
+TM_DEV int pack2(float lo, float hi)
+{
+    int a = __float2int_rn(lo), b = __float2int_rn(hi);
+    return (a & 0xffff) | (b << 16);
+}
+
+// ---- spinor loads ---------------------------------------------------------------------------------
+// `base` points at the flavor's chunk block, `norm` at the flavor's norm array (half only), Vh = sites.
+// PART: 0 = all 24 reals, 1 = upper only (v[0..11] valid), 2 = lower only (v[12..23] valid).
+template <int PREC, int PART>
+TM_DEV void load_spinor(typename PrecTraits<PREC>::real *v, const char *base, const float *norm, int Vh, int idx)
+{
+    if constexpr (PREC == 8) {
+        constexpr int lo = (PART == 2) ? 6 : 0, hi = (PART == 1) ? 6 : 12;
+#pragma unroll
+        for (int k = lo; k < hi; k++) {
+            double2 c = ldg_d2(base + ((size_t)k * Vh + idx) * 16);
+            v[2 * k] = c.x;
+            v[2 * k + 1] = c.y;
+        }
+    } else if constexpr (PREC == 4) {
+        constexpr int lo = (PART == 2) ? 3 : 0, hi = (PART == 1) ? 3 : 6;
+#pragma unroll
+        for (int k = lo; k < hi; k++) {
+            float4 c = ldg_f4(base + ((size_t)k * Vh + idx) * 16);
+            v[4 * k] = c.x;
+            v[4 * k + 1] = c.y;
+            v[4 * k + 2] = c.z;
+            v[4 * k + 3] = c.w;
+        }
+    } else {
+        // 3 chunks of 8 int16: reals 0..7, 8..15, 16..23.  upper = 0..11, lower = 12..23.
+        const float s = ldg_f1(norm + idx) * TM_HALF_INV;
+        if constexpr (PART != 2) {
+            int4 c = ldg_i4(base + ((size_t)0 * Vh + idx) * 16);
+            unpack2(c.x, s, v[0], v[1]);
+            unpack2(c.y, s, v[2], v[3]);
+            unpack2(c.z, s, v[4], v[5]);
+            unpack2(c.w, s, v[6], v[7]);
+        }
+        {
+            int4 c = ldg_i4(base + ((size_t)1 * Vh + idx) * 16);
+            if constexpr (PART != 2) {
+                unpack2(c.x, s, v[8], v[9]);
+                unpack2(c.y, s, v[10], v[11]);
+            }
+            if constexpr (PART != 1) {
+                unpack2(c.z, s, v[12], v[13]);
+                unpack2(c.w, s, v[14], v[15]);
+            }
+        }
+        if constexpr (PART != 1) {
+            int4 c = ldg_i4(base + ((size_t)2 * Vh + idx) * 16);
+            unpack2(c.x, s, v[16], v[17]);
+            unpack2(c.y, s, v[18], v[19]);
+            unpack2(c.z, s, v[20], v[21]);
+            unpack2(c.w, s, v[22], v[23]);
+        }
+    }
+}
+
+// ---- spinor store (a8): one write of the output site; half: norm = max|v|, q = rint(v * 32767 / norm)
+template <int PREC>
+TM_DEV void store_spinor(const typename PrecTraits<PREC>::real *v, char *base, float *norm, int Vh, int idx)
+{
+    if constexpr (PREC == 8) {
+#pragma unroll
+        for (int k = 0; k < 12; k++)
+            *reinterpret_cast<double2 *>(base + ((size_t)k * Vh + idx) * 16) = make_double2(v[2 * k], v[2 * k + 1]);
+    } else if constexpr (PREC == 4) {
+#pragma unroll
+        for (int k = 0; k < 6; k++)
+            *reinterpret_cast<float4 *>(base + ((size_t)k * Vh + idx) * 16) =
+                make_float4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+    } else {
+        float m = 0.f;
+#pragma unroll
+        for (int i = 0; i < 24; i++) m = fmaxf(m, fabsf(v[i]));
+        const float s = (m > 0.f) ? __fdividef(TM_HALF_MAX, m) : 0.f;
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            int4 c;
+            c.x = pack2(v[8 * k + 0] * s, v[8 * k + 1] * s);
+            c.y = pack2(v[8 * k + 2] * s, v[8 * k + 3] * s);
+            c.z = pack2(v[8 * k + 4] * s, v[8 * k + 5] * s);
+            c.w = pack2(v[8 * k + 6] * s, v[8 * k + 7] * s);
+            *reinterpret_cast<int4 *>(base + ((size_t)k * Vh + idx) * 16) = c;
+        }
+        norm[idx] = m;
+    }
+}
+
+// ---- link load + SU(3) row rebuild (a4) -----------------------------------------------------------
+// `base` points at the [parity][mu] block.  12-real: rows 0,1 stored, row2 = conj(row0 x row1).
+template <typename real>
+TM_DEV void rebuild_row2(real *u)
+{
+    // u[r][c] = u[(r*3+c)*2 + ri];  row2[c] = conj(row0[c+1] row1[c+2] - row0[c+2] row1[c+1])
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        const real ar = u[2 * c1], ai = u[2 * c1 + 1];               // row0[c1]
+        const real br = u[2 * (3 + c2)], bi = u[2 * (3 + c2) + 1];   // row1[c2]
+        const real cr = u[2 * c2], ci = u[2 * c2 + 1];               // row0[c2]
+        const real dr = u[2 * (3 + c1)], di = u[2 * (3 + c1) + 1];   // row1[c1]
+        u[2 * (6 + c)] = (ar * br - ai * bi) - (cr * dr - ci * di);
+        u[2 * (6 + c) + 1] = -((ar * bi + ai * br) - (cr * di + ci * dr));
+    }
+}
+
+template <int PREC, int RECON>
+TM_DEV void load_link(typename PrecTraits<PREC>::real *u, const char *base, int Vh, int idx)
+{
+    if constexpr (PREC == 8) {
+#pragma unroll
+        for (int k = 0; k < RECON / 2; k++) {
+            double2 c = ldg_d2(base + ((size_t)k * Vh + idx) * 16);
+            u[2 * k] = c.x;
+            u[2 * k + 1] = c.y;
+        }
+    } else if constexpr (PREC == 4) {
+        constexpr int NF4 = (RECON == 18) ? 4 : 3;
+#pragma unroll
+        for (int k = 0; k < NF4; k++) {
+            float4 c = ldg_f4(base + ((size_t)k * Vh + idx) * 16);
+            u[4 * k] = c.x;
+            u[4 * k + 1] = c.y;
+            u[4 * k + 2] = c.z;
+            u[4 * k + 3] = c.w;
+        }
+        if constexpr (RECON == 18) {
+            float2 c = ldg_f2(base + (size_t)4 * Vh * 16 + (size_t)idx * 8);
+            u[16] = c.x;
+            u[17] = c.y;
+        }
+    } else {
+        const float s = TM_HALF_INV;
+        int4 c = ldg_i4(base + (size_t)idx * 16);
+        unpack2(c.x, s, u[0], u[1]);
+        unpack2(c.y, s, u[2], u[3]);
+        unpack2(c.z, s, u[4], u[5]);
+        unpack2(c.w, s, u[6], u[7]);
+        if constexpr (RECON == 18) {
+            int4 d = ldg_i4(base + ((size_t)Vh + idx) * 16);
+            unpack2(d.x, s, u[8], u[9]);
+            unpack2(d.y, s, u[10], u[11]);
+            unpack2(d.z, s, u[12], u[13]);
+            unpack2(d.w, s, u[14], u[15]);
+            int e = ldg_i1(base + (size_t)2 * Vh * 16 + (size_t)idx * 4);
+            unpack2(e, s, u[16], u[17]);
+        } else {
+            int2 d = ldg_i2(base + (size_t)Vh * 16 + (size_t)idx * 8);
+            unpack2(d.x, s, u[8], u[9]);
+            unpack2(d.y, s, u[10], u[11]);
+        }
+    }
+    if constexpr (RECON == 12) rebuild_row2(u);
+}

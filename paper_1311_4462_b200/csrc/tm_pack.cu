@@ -1,0 +1,141 @@
+// tm_pack.cu -- host canonical order (double) <-> device checkerboard SoA (row a1 of DESIGN.md).
+// Not on the hot path: runs once per upload / download.  Sources are device staging copies of the host arrays.
+#include "tm_internal.h"
+#include "tm_layout.cuh"
+
+namespace {
+
+struct PackGeom {
+    int X, Y, Z, T, Xh, Vh;
+    long V;
+};
+
+__device__ __forceinline__ long cb_to_lex(const PackGeom &g, int i, int parity)
+{
+    int r = i / g.Xh;
+    const int y = r % g.Y;
+    r /= g.Y;
+    const int z = r % g.Z;
+    const int t = r / g.Z;
+    return 2L * i + ((y + z + t + parity) & 1);      // lex / 2 == i, x1 parity fixed by the row
+}
+
+template <int PREC>
+__global__ void pack_spinor_kernel(char *dst, const double *src, PackGeom g, int parity, int nf, bool src_is_cb)
+{
+    typedef typename PrecTraits<PREC>::real real;
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= nf * g.Vh) return;
+    const int f = tid / g.Vh, i = tid % g.Vh;
+    const double *s = src_is_cb ? src + ((size_t)f * g.Vh + i) * 24 : src + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
+    real v[24];
+#pragma unroll
+    for (int k = 0; k < 24; k++) v[k] = (real)s[k];
+    const size_t fl_bytes = (size_t)PrecTraits<PREC>::NCH * g.Vh * 16;
+    store_spinor<PREC>(v, dst + f * fl_bytes, reinterpret_cast<float *>(dst + nf * fl_bytes) + (size_t)f * g.Vh, g.Vh, i);
+}
+
+template <int PREC>
+__global__ void unpack_spinor_kernel(double *dst, const char *src, PackGeom g, int parity, int nf, bool dst_is_cb)
+{
+    typedef typename PrecTraits<PREC>::real real;
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= nf * g.Vh) return;
+    const int f = tid / g.Vh, i = tid % g.Vh;
+    const size_t fl_bytes = (size_t)PrecTraits<PREC>::NCH * g.Vh * 16;
+    real v[24];
+    load_spinor<PREC, 0>(v, src + f * fl_bytes, reinterpret_cast<const float *>(src + nf * fl_bytes) + (size_t)f * g.Vh, g.Vh, i);
+    double *d = dst_is_cb ? dst + ((size_t)f * g.Vh + i) * 24 : dst + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
+#pragma unroll
+    for (int k = 0; k < 24; k++) d[k] = (double)v[k];
+}
+
+// one thread per (parity, mu, cb site): U_mu(x) for x of that parity
+template <int PREC, int RECON>
+__global__ void pack_gauge_kernel(char *dst, const double *src, PackGeom g)
+{
+    const long tid = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= 8L * g.Vh) return;
+    const int i = (int)(tid % g.Vh);
+    const int pm = (int)(tid / g.Vh);       // parity * 4 + mu
+    const int parity = pm >> 2, mu = pm & 3;
+    const double *s = src + ((size_t)mu * g.V + cb_to_lex(g, i, parity)) * 18;
+    char *blk = dst + (size_t)pm * RECON * PREC * g.Vh;
+    const int Vh = g.Vh;
+    if constexpr (PREC == 8) {
+#pragma unroll
+        for (int k = 0; k < RECON / 2; k++)
+            *reinterpret_cast<double2 *>(blk + ((size_t)k * Vh + i) * 16) = make_double2(s[2 * k], s[2 * k + 1]);
+    } else if constexpr (PREC == 4) {
+        constexpr int NF4 = (RECON == 18) ? 4 : 3;
+#pragma unroll
+        for (int k = 0; k < NF4; k++)
+            *reinterpret_cast<float4 *>(blk + ((size_t)k * Vh + i) * 16) =
+                make_float4((float)s[4 * k], (float)s[4 * k + 1], (float)s[4 * k + 2], (float)s[4 * k + 3]);
+        if constexpr (RECON == 18)
+            *reinterpret_cast<float2 *>(blk + (size_t)4 * Vh * 16 + (size_t)i * 8) = make_float2((float)s[16], (float)s[17]);
+    } else {
+        int w[9];
+#pragma unroll
+        for (int k = 0; k < RECON / 2; k++)
+            w[k] = pack2((float)s[2 * k] * TM_HALF_MAX, (float)s[2 * k + 1] * TM_HALF_MAX);
+        *reinterpret_cast<int4 *>(blk + (size_t)i * 16) = make_int4(w[0], w[1], w[2], w[3]);
+        if constexpr (RECON == 18) {
+            *reinterpret_cast<int4 *>(blk + ((size_t)Vh + i) * 16) = make_int4(w[4], w[5], w[6], w[7]);
+            *reinterpret_cast<int *>(blk + (size_t)2 * Vh * 16 + (size_t)i * 4) = w[8];
+        } else {
+            *reinterpret_cast<int2 *>(blk + (size_t)Vh * 16 + (size_t)i * 8) = make_int2(w[4], w[5]);
+        }
+    }
+}
+
+PackGeom geom_of(const tm_ctx *c)
+{
+    PackGeom g;
+    g.X = c->g.X[0];
+    g.Y = c->g.X[1];
+    g.Z = c->g.X[2];
+    g.T = c->g.X[3];
+    g.Xh = c->g.Xh;
+    g.Vh = c->g.Vh;
+    g.V = c->g.V;
+    return g;
+}
+
+}  // namespace
+
+cudaError_t tm_pack_spinor(const tm_field *f, int parity, const double *dev_src, bool src_is_cb, cudaStream_t s)
+{
+    const PackGeom g = geom_of(f->ctx);
+    const int n = f->nf * g.Vh, threads = 128, blocks = (n + threads - 1) / threads;
+    char *dst = static_cast<char *>(f->ptr);
+    if (f->prec == 8) pack_spinor_kernel<8><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb);
+    else if (f->prec == 4) pack_spinor_kernel<4><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb);
+    else pack_spinor_kernel<2><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb);
+    return cudaGetLastError();
+}
+
+cudaError_t tm_unpack_spinor(const tm_field *f, int parity, double *dev_dst, bool dst_is_cb, cudaStream_t s)
+{
+    const PackGeom g = geom_of(f->ctx);
+    const int n = f->nf * g.Vh, threads = 128, blocks = (n + threads - 1) / threads;
+    const char *src = static_cast<const char *>(f->ptr);
+    if (f->prec == 8) unpack_spinor_kernel<8><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb);
+    else if (f->prec == 4) unpack_spinor_kernel<4><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb);
+    else unpack_spinor_kernel<2><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb);
+    return cudaGetLastError();
+}
+
+cudaError_t tm_pack_gauge(const tm_gauge *gg, const double *dev_src, cudaStream_t s)
+{
+    const PackGeom g = geom_of(gg->ctx);
+    const long n = 8L * g.Vh;
+    const int threads = 128, blocks = (int)((n + threads - 1) / threads);
+    char *dst = static_cast<char *>(gg->ptr);
+#define TM_PG(P, R) pack_gauge_kernel<P, R><<<blocks, threads, 0, s>>>(dst, dev_src, g)
+    if (gg->prec == 8) { if (gg->recon == 18) TM_PG(8, 18); else TM_PG(8, 12); }
+    else if (gg->prec == 4) { if (gg->recon == 18) TM_PG(4, 18); else TM_PG(4, 12); }
+    else { if (gg->recon == 18) TM_PG(2, 18); else TM_PG(2, 12); }
+#undef TM_PG
+    return cudaGetLastError();
+}

@@ -1,0 +1,215 @@
+"""GPU parity tests: every C-ABI entry point against the CPU oracle, element by element, on seeded inputs.
+
+Tolerances are BASELINE.json's: relative L2 over the whole output parity field (both flavors together)
+<= 1e-12 (double), 1e-5 (single), 5e-3 (half).  Half inputs are quantised by the library on upload; the oracle
+always sees the unquantised double inputs (reading C9, primary comparison).
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1311_4462_b200 as tm
+import synth_inputs as si
+from gpu_util import TOL, PREC_NAME, Bench, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+KAPPA = 0.1632
+PRECS = [tm.TM_DOUBLE, tm.TM_SINGLE, tm.TM_HALF]
+RECONS = [tm.TM_RECON_18, tm.TM_RECON_12]
+FLAVORS = [
+    dict(mu=0.004, epsilon=0.0, twist_flavor=1),
+    dict(mu=0.3, epsilon=0.0, twist_flavor=-1),
+    dict(mu=0.15, epsilon=0.19, twist_flavor=0),
+]
+
+
+def nf_of(kw):
+    return 2 if kw["twist_flavor"] == 0 else 1
+
+
+_cache = {}
+
+
+def bench_for(dims, kind, seed):
+    key = (tuple(dims), kind, seed)
+    if key not in _cache:
+        _cache[key] = Bench(dims, si.gauge_field(dims, seed, kind))
+    return _cache[key]
+
+
+# ---- T1: layouts round trip -----------------------------------------------------------------------
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 8), (4, 6, 8, 10)])
+@pytest.mark.parametrize("nf", [1, 2])
+def test_t1_spinor_pack_unpack_round_trip(dims, nf):
+    lat = tm.Lattice(dims)
+    psi = si.spinor_field(dims, nf, 5)
+    for prec in PRECS:
+        for parity in (0, 1):
+            f = lat.field(prec, nf).upload(parity, psi)
+            back = f.download(parity)
+            want = si.mask_parity(psi, dims, parity)
+            assert np.abs(si.mask_parity(back, dims, 1 - parity)).max() == 0
+            if prec == tm.TM_DOUBLE:
+                assert np.array_equal(back, want)
+            elif prec == tm.TM_SINGLE:
+                assert np.array_equal(back, want.astype(np.complex64).astype(np.complex128))
+            else:
+                # <= 1/2 LSB of the site's scale: |v - deq| <= 0.5 * norm / 32767 (+ fp32 rounding)
+                idx = si.parity_sites(dims, parity)
+                w = want[:, idx].reshape(nf, len(idx), 24 // 2)
+                b = back[:, idx].reshape(nf, len(idx), 24 // 2)
+                norm = np.maximum(np.abs(w.real).max(axis=2), np.abs(w.imag).max(axis=2))[..., None]
+                err = np.maximum(np.abs((w - b).real), np.abs((w - b).imag))
+                assert (err <= (0.5 / 32767 + 1e-6) * norm).all()     # 1e-6: fp32 rounding of the scale
+            # the cb entry points see the same field
+            cb = f.download_cb(parity)
+            assert np.array_equal(cb, back[:, si.parity_sites(dims, parity)])
+            g = lat.field(prec, nf).upload_cb(parity, si.to_parity(psi, dims, parity))
+            assert np.array_equal(g.download(parity), back)
+
+
+# ---- T2: every kernel variant vs the oracle -------------------------------------------------------
+
+@pytest.mark.parametrize("dims,kind", [((4, 4, 4, 8), "haar"), ((4, 6, 8, 10), "near_identity"), ((8, 4, 6, 4), "haar")])
+@pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
+def test_t2_every_kernel_variant_matches_oracle(dims, kind, kw):
+    nf = nf_of(kw)
+    bench = bench_for(dims, kind, 1)
+    po = oracle.params(dims, KAPPA, **kw)
+    pg = tm.params(KAPPA, **kw)
+    full_in, full_x = si.spinor_field(dims, nf, 2), si.spinor_field(dims, nf, 3)
+    worst = {}
+    for parity, dagger, kt in itertools.product((0, 1), (0, 1), (0, 1, 2, 3)):
+        inp = si.mask_parity(full_in, dims, 1 - parity)
+        x = si.mask_parity(full_x, dims, parity)
+        want = oracle.kernel(inp, x, bench.U, po, parity, dagger, kt)
+        for prec, recon in itertools.product(PRECS, RECONS):
+            got = bench.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, prec, recon, nf)
+            err = rel_l2(got, want)
+            worst[prec] = max(worst.get(prec, 0.0), err)
+            assert err <= TOL[prec], (PREC_NAME[prec], recon, parity, dagger, kt, err)
+            assert np.abs(si.mask_parity(got, dims, 1 - parity)).max() == 0
+    print("worst rel L2:", {PREC_NAME[k]: v for k, v in worst.items()})
+
+
+def test_t2b_periodic_time_and_wilson_limit():
+    dims = (4, 4, 6, 8)
+    bench = bench_for(dims, "haar", 7)
+    for kw in (dict(mu=0.0, epsilon=0.0, twist_flavor=1, t_boundary=+1), dict(mu=0.0, epsilon=0.0, twist_flavor=0, t_boundary=-1),
+               dict(mu=0.15, epsilon=0.19, twist_flavor=0, t_boundary=+1)):
+        nf = nf_of(kw)
+        po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+        inp = si.mask_parity(si.spinor_field(dims, nf, 8), dims, 0)
+        x = si.mask_parity(si.spinor_field(dims, nf, 9), dims, 1)
+        for kt in (0, 1, 2, 3):
+            want = oracle.kernel(inp, x, bench.U, po, 1, 0, kt)
+            for prec in PRECS:
+                got = bench.kernel(inp, x, pg, 1, 0, kt, prec, tm.TM_RECON_12, nf)
+                assert rel_l2(got, want) <= TOL[prec]
+
+
+# ---- T3: composites; BASELINE.json config 1 -------------------------------------------------------
+
+@pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
+def test_t3_mat_pc_and_reconstruct_match_oracle(kw):
+    dims = (4, 4, 4, 8)
+    nf = nf_of(kw)
+    bench = bench_for(dims, "haar", 1)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    psi = si.spinor_field(dims, nf, 4)
+    psi_e, b_o = si.mask_parity(psi, dims, 0), si.mask_parity(si.spinor_field(dims, nf, 6), dims, 1)
+    for prec, recon in itertools.product(PRECS, RECONS):
+        for typ, dagger in ((tm.TM_MATPC_ASYM, 0), (tm.TM_MATPC_ASYM, 1), (tm.TM_MATPC_SYM, 0)):
+            want = oracle.matpc(psi_e, bench.U, po, typ, dagger)
+            got = bench.matpc(psi_e, pg, typ, dagger, prec, recon, nf)
+            assert rel_l2(got, want) <= TOL[prec], (PREC_NAME[prec], recon, typ, dagger)
+        want = oracle.reconstruct_odd(psi_e, b_o, bench.U, po)
+        assert rel_l2(bench.reconstruct_odd(psi_e, b_o, pg, prec, recon, nf), want) <= TOL[prec]
+
+
+def test_t3b_config1_solve_check():
+    """BASELINE.json configs[0]: 4^3x8, degenerate, fp64, Haar links seed 1, kappa=0.1632, mu=0.004, antiperiodic.
+    Draw a full psi, b = M psi (oracle); the GPU's LHS of Eq. 2.2 applied to psi_e must equal the prepared
+    RHS b_e + kappa D_eo R_oo^-1 b_o, and Eq. 2.4 must return psi_o."""
+    dims = (4, 4, 4, 8)
+    kw = dict(mu=0.004, epsilon=0.0, twist_flavor=1)
+    bench = bench_for(dims, "haar", 1)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    psi = si.spinor_field(dims, 1, 1)
+    b = oracle.mat(psi, bench.U, po)
+    b_e, b_o = si.mask_parity(b, dims, 0), si.mask_parity(b, dims, 1)
+    psi_e, psi_o = si.mask_parity(psi, dims, 0), si.mask_parity(psi, dims, 1)
+    rhs = b_e + KAPPA * si.mask_parity(oracle.dhop(oracle.twist(b_o, po, inverse=1), bench.U, po), dims, 0)
+    for recon in RECONS:
+        lhs = bench.matpc(psi_e, pg, tm.TM_MATPC_ASYM, 0, tm.TM_DOUBLE, recon, 1)
+        assert rel_l2(lhs, rhs) <= 1e-12
+        rec = bench.reconstruct_odd(psi_e, b_o, pg, tm.TM_DOUBLE, recon, 1)
+        assert rel_l2(rec, psi_o) <= 1e-12
+
+
+# ---- T4: GPU-side properties that need no oracle --------------------------------------------------
+
+@pytest.mark.parametrize("kw", [FLAVORS[0], FLAVORS[2]], ids=["deg", "ndeg"])
+def test_t4_asym_composite_adjointness_on_gpu(kw):
+    dims = (8, 8, 8, 8)
+    nf = nf_of(kw)
+    bench = bench_for(dims, "haar", 11)
+    pg = tm.params(KAPPA, **kw)
+    psi = si.mask_parity(si.spinor_field(dims, nf, 12), dims, 0)
+    phi = si.mask_parity(si.spinor_field(dims, nf, 13), dims, 0)
+    for prec, tol in ((tm.TM_DOUBLE, 1e-12), (tm.TM_SINGLE, 1e-5)):
+        m_psi = bench.matpc(psi, pg, tm.TM_MATPC_ASYM, 0, prec, tm.TM_RECON_12, nf)
+        md_phi = bench.matpc(phi, pg, tm.TM_MATPC_ASYM, 1, prec, tm.TM_RECON_12, nf)
+        lhs, rhs = np.vdot(phi, m_psi), np.vdot(md_phi, psi)
+        assert abs(lhs - rhs) <= tol * np.linalg.norm(phi) * np.linalg.norm(m_psi)
+
+
+# ---- T6: error paths of the boundary --------------------------------------------------------------
+
+def test_t6_error_paths():
+    dims = (4, 4, 4, 8)
+    bench = bench_for(dims, "haar", 1)
+    lat = bench.lat
+    g = bench.gauge(tm.TM_SINGLE, tm.TM_RECON_12)
+    p = tm.params(KAPPA, 0.004)
+    a, b, c = lat.field(tm.TM_SINGLE, 1), lat.field(tm.TM_SINGLE, 1), lat.field(tm.TM_SINGLE, 1)
+    d64, two = lat.field(tm.TM_DOUBLE, 1), lat.field(tm.TM_SINGLE, 2)
+
+    def status(fn):
+        with pytest.raises(tm.TmError) as e:
+            fn()
+        return e.value.status
+
+    assert status(lambda: tm.dslash_apply(a, a, None, g, p, 0, 0, 0)) == tm.TM_ERR_ALIAS
+    assert status(lambda: tm.dslash_apply(a, b, None, g, p, 0, 0, tm.TM_DSLASH_TWIST_XPAY)) == tm.TM_ERR_ARG
+    assert status(lambda: tm.dslash_apply(d64, b, None, g, p, 0, 0, 0)) == tm.TM_ERR_MISMATCH
+    assert status(lambda: tm.dslash_apply(a, two, None, g, p, 0, 0, 0)) == tm.TM_ERR_MISMATCH
+    assert status(lambda: tm.tm_dslash_apply(a.h, b.h, None, g.h, p, 0, 0, 0, tm.TM_DOUBLE)) == tm.TM_ERR_MISMATCH
+    assert status(lambda: tm.dslash_apply(a, b, None, g, tm.params(KAPPA, 0.1, twist_flavor=0), 0, 0, 0)) == tm.TM_ERR_MISMATCH
+    assert status(lambda: tm.dslash_apply(a, b, None, g, tm.params(KAPPA, 0.1, epsilon=0.1), 0, 0, 0)) == tm.TM_ERR_PARAM
+    assert status(lambda: tm.dslash_apply(a, b, None, g, tm.params(KAPPA, 0.1, t_boundary=0), 0, 0, 0)) == tm.TM_ERR_PARAM
+    sing = tm.params(KAPPA, 0.0, epsilon=1.0 / (2 * KAPPA), twist_flavor=0)     # 1 + a^2 - b^2 = 0
+    t2, t3 = lat.field(tm.TM_SINGLE, 2), lat.field(tm.TM_SINGLE, 2)
+    assert status(lambda: tm.dslash_apply(t2, t3, None, g, sing, 0, 0, 0)) == tm.TM_ERR_PARAM
+    assert status(lambda: tm.mat_pc(a, b, c, g, p, tm.TM_MATPC_SYM, 1)) == tm.TM_ERR_UNSUPPORTED
+    assert status(lambda: tm.mat_pc(a, b, b, g, p, tm.TM_MATPC_ASYM, 0)) == tm.TM_ERR_ALIAS
+    assert status(lambda: tm.tm_init((4, 4, 4, 7))) == tm.TM_ERR_DIMS
+    assert status(lambda: tm.tm_init((2, 4, 4, 8))) == tm.TM_ERR_DIMS
+    # out may alias x (B kernel reads its own site before the store)
+    x = si.mask_parity(si.spinor_field(dims, 1, 3), dims, 0)
+    inp = si.mask_parity(si.spinor_field(dims, 1, 2), dims, 1)
+    fx = lat.field(tm.TM_DOUBLE, 1).upload(0, x)
+    fi = lat.field(tm.TM_DOUBLE, 1).upload(1, inp)
+    g64 = bench.gauge(tm.TM_DOUBLE, tm.TM_RECON_18)
+    tm.dslash_apply(fx, fi, fx, g64, p, 0, 0, tm.TM_DSLASH_TWIST_XPAY)
+    lat.sync()
+    want = oracle.kernel(inp, x, bench.U, oracle.params(dims, KAPPA, 0.004), 0, 0, oracle.B)
+    assert rel_l2(fx.download(0), want) <= 1e-12
+    # the launch counter counts dslash kernels
+    n0 = lat.launches()
+    tm.mat_pc(a, b, c, g, p, tm.TM_MATPC_ASYM, 0)
+    assert lat.launches() == n0 + 2
