@@ -130,6 +130,11 @@ const char *tm_last_error(void);       /* thread-local, never NULL */
 long tm_launch_count(const tm_ctx *ctx);
 /* Name of the kernel variant the last tm_dslash_apply on this context dispatched to (static string). */
 const char *tm_last_kernel_name(const tm_ctx *ctx);
+/* Per-launch device timing (bench.py's roofline leg): while enabled, every dslash launch is bracketed by CUDA
+ * events on the context stream.  tm_timing_read synchronises, writes up to max_records (kernel name, milliseconds)
+ * pairs in launch order into the HOST arrays names / ms, stores the number written in *n, and clears the log. */
+int tm_timing_enable(tm_ctx *ctx, int on);
+int tm_timing_read(tm_ctx *ctx, int max_records, const char **names, float *ms, int *n);
 /* Force a code path: 0 = automatic (default), 1 = generic direct-load kernels only.  For tests / profiling. */
 int tm_set_path(tm_ctx *ctx, int path);
 

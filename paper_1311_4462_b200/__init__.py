@@ -31,7 +31,7 @@ EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
     "tm_field_device_ptr", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb",
     "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_last_error",
-    "tm_launch_count", "tm_last_kernel_name", "tm_set_path",
+    "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_timing_enable", "tm_timing_read",
 ]
 
 
@@ -90,6 +90,9 @@ def lib():
     L.tm_last_kernel_name.argtypes = [vp]
     L.tm_last_kernel_name.restype = ctypes.c_char_p
     L.tm_set_path.argtypes = [vp, i]
+    L.tm_timing_enable.argtypes = [vp, i]
+    L.tm_timing_read.argtypes = [vp, i, ctypes.POINTER(ctypes.c_char_p), ctypes.POINTER(ctypes.c_float),
+                                 ctypes.POINTER(i)]
     _lib = L
     return L
 
@@ -195,6 +198,19 @@ def tm_last_kernel_name(ctx):
 
 def tm_set_path(ctx, path):
     _check(lib().tm_set_path(ctx, int(path)))
+
+
+def tm_timing_enable(ctx, on):
+    _check(lib().tm_timing_enable(ctx, int(on)))
+
+
+def tm_timing_read(ctx, max_records=1 << 16):
+    """-> list of (kernel name, milliseconds) per dslash launch since the last read, in launch order."""
+    names = (ctypes.c_char_p * max_records)()
+    ms = (ctypes.c_float * max_records)()
+    n = ctypes.c_int(0)
+    _check(lib().tm_timing_read(ctx, max_records, names, ms, ctypes.byref(n)))
+    return [(names[k].decode(), float(ms[k])) for k in range(n.value)]
 
 
 # ---- handle owners: torch supplies the memory and the stream -------------------------------------------

@@ -56,11 +56,25 @@ bool overlap(const tm_field *a, const tm_field *b)
     return pa < pb + b->bytes && pb < pa + a->bytes;
 }
 
-// RAII device staging buffer for upload / download (not hot)
+// Device staging buffer for upload / download, cached on the context (grown on demand, freed in tm_finalize).
+// Safe to reuse: every upload / download synchronises the stream before it returns.
 struct Staging {
+    tm_ctx *c;
     void *p = nullptr;
-    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes); }
-    ~Staging() { if (p) cudaFree(p); }
+    explicit Staging(tm_ctx *ctx) : c(ctx) {}
+    cudaError_t alloc(size_t bytes)
+    {
+        if (c->staging_bytes < bytes) {
+            if (c->staging) cudaFree(c->staging);
+            c->staging = nullptr;
+            c->staging_bytes = 0;
+            cudaError_t e = cudaMalloc(&c->staging, bytes);
+            if (e != cudaSuccess) return e;
+            c->staging_bytes = bytes;
+        }
+        p = c->staging;
+        return cudaSuccess;
+    }
 };
 
 struct Coeffs {
@@ -117,6 +131,9 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->last_kernel = "";
     c->path = 0;
     c->sm_count = 0;
+    c->staging = nullptr;
+    c->staging_bytes = 0;
+    c->timing = false;
     e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
     if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaDeviceGetAttribute"); }
     *ctx = c;
@@ -138,7 +155,46 @@ int tm_sync(tm_ctx *ctx)
     return TM_OK;
 }
 
-void tm_finalize(tm_ctx *ctx) { delete ctx; }
+void tm_finalize(tm_ctx *ctx)
+{
+    if (!ctx) return;
+    if (ctx->staging) cudaFree(ctx->staging);
+    for (auto &t : ctx->timed) { cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
+    delete ctx;
+}
+
+static void clear_timed(tm_ctx *ctx)
+{
+    for (auto &t : ctx->timed) { cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
+    ctx->timed.clear();
+}
+
+int tm_timing_enable(tm_ctx *ctx, int on)
+{
+    if (!ctx) return fail(TM_ERR_ARG, "tm_timing_enable: NULL context");
+    ctx->timing = on != 0;
+    if (!ctx->timing) clear_timed(ctx);
+    return TM_OK;
+}
+
+int tm_timing_read(tm_ctx *ctx, int max_records, const char **names, float *ms, int *n)
+{
+    if (!ctx || !names || !ms || !n || max_records < 0) return fail(TM_ERR_ARG, "tm_timing_read: bad argument");
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
+    int k = 0;
+    for (auto &t : ctx->timed) {
+        if (k >= max_records) break;
+        float v = 0.f;
+        if ((e = cudaEventElapsedTime(&v, t.start, t.stop)) != cudaSuccess) return cuda_fail(e, "cudaEventElapsedTime");
+        names[k] = t.name;
+        ms[k] = v;
+        k++;
+    }
+    *n = k;
+    clear_timed(ctx);
+    return TM_OK;
+}
 
 int tm_set_path(tm_ctx *ctx, int path)
 {
@@ -194,7 +250,7 @@ static int field_upload(tm_field *f, int parity, const double *host, bool cb)
     if (parity != 0 && parity != 1) return fail(TM_ERR_ARG, "bad parity %d", parity);
     tm_ctx *c = f->ctx;
     const size_t n = (size_t)f->nf * (cb ? (size_t)c->g.Vh : (size_t)c->g.V) * 24 * sizeof(double);
-    Staging st;
+    Staging st(c);
     cudaError_t e = st.alloc(n);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
     e = cudaMemcpyAsync(st.p, host, n, cudaMemcpyHostToDevice, c->stream);
@@ -212,7 +268,7 @@ static int field_download(const tm_field *f, int parity, double *host, bool cb)
     if (parity != 0 && parity != 1) return fail(TM_ERR_ARG, "bad parity %d", parity);
     tm_ctx *c = f->ctx;
     const size_t n = (size_t)f->nf * (cb ? (size_t)c->g.Vh : (size_t)c->g.V) * 24 * sizeof(double);
-    Staging st;
+    Staging st(c);
     cudaError_t e = st.alloc(n);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
     if (!cb) {   // only this parity's sites are written: start from the caller's array
@@ -246,7 +302,7 @@ int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_r
     cudaError_t e = cudaMalloc(&gg->ptr, gg->bytes);
     if (e != cudaSuccess) { delete gg; cudaGetLastError(); return fail(TM_ERR_NOMEM, "cudaMalloc(%zu): %s", gg->bytes, cudaGetErrorString(e)); }
     const size_t n = (size_t)4 * ctx->g.V * 18 * sizeof(double);
-    Staging st;
+    Staging st(ctx);
     e = st.alloc(n);
     if (e != cudaSuccess) { tm_gauge_free(gg); cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
     e = cudaMemcpyAsync(st.p, host_links, n, cudaMemcpyHostToDevice, ctx->stream);
@@ -291,7 +347,19 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
 
     const TmKernelEntry *tab = tm_generic_table((int)prec, out->nf);
     const TmKernelEntry &k = tab[((g->recon == 18 ? 0 : 1) * 4 + (int)kt) * 2 + (dagger ? 1 : 0)];
-    cudaError_t e = k.fn(a, c->stream);
+    cudaError_t e;
+    if (c->timing) {
+        tm_ctx::TimedLaunch t;
+        t.name = k.name;
+        if ((e = cudaEventCreate(&t.start)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
+        if ((e = cudaEventCreate(&t.stop)) != cudaSuccess) { cudaEventDestroy(t.start); return cuda_fail(e, "cudaEventCreate"); }
+        cudaEventRecord(t.start, c->stream);
+        e = k.fn(a, c->stream);
+        cudaEventRecord(t.stop, c->stream);
+        c->timed.push_back(t);
+    } else {
+        e = k.fn(a, c->stream);
+    }
     if (e != cudaSuccess) return cuda_fail(e, k.name);
     c->launches++;
     c->last_kernel = k.name;

@@ -13,6 +13,8 @@
 #include <cuda_runtime.h>
 #include <stddef.h>
 
+#include <vector>
+
 #include "../../include/tm.h"
 
 struct TmGeom {
@@ -30,6 +32,11 @@ struct tm_ctx {
     const char *last_kernel;
     int path;    // 0 auto, 1 generic only
     int sm_count;
+    void *staging;        // device staging for upload / download
+    size_t staging_bytes;
+    bool timing;          // tm_timing_enable
+    struct TimedLaunch { cudaEvent_t start, stop; const char *name; };
+    std::vector<TimedLaunch> timed;
 };
 
 struct tm_field {
