@@ -80,10 +80,6 @@ def op_bytes(op, vh):
     return sum(bytes_per_site(nf, prec, RECON, kt) for nf, prec, kt, _ in op_kernels(op)) * vh
 
 
-def kernel_name(nf, prec, kt, dagger):
-    return "generic<%d,%d,%d,%d,%s>" % (prec, nf, RECON, kt, "dagger" if dagger else "plain")
-
-
 def measured_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -282,6 +278,7 @@ def run_ours(args, log):
     import paper_1311_4462_b200 as tm
     w = Workload(local, log)
     lat, vh = w.lat, w.vh
+    tm.tm_set_path(lat.ctx, args.path)
     ops = step_ops()
     step_flops = sum(op_flops(o, vh) for o in ops)
     step_bytes = sum(op_bytes(o, vh) for o in ops)
@@ -320,28 +317,26 @@ def run_ours(args, log):
 
     # ---- per-kernel roofline from the events recorded inside the timed region
     peak, peak_src = measured_peak()
+    step_kernels = [k for op in ops for k in op_kernels(op)]        # launch order inside one step
+    assert len(records) == args.steps * len(step_kernels), (len(records), args.steps, len(step_kernels))
     per = {}
-    for name, t in records:
-        a = per.setdefault(name, [0.0, 0])
+    for i, (name, t) in enumerate(records):
+        a = per.setdefault(step_kernels[i % len(step_kernels)], [0.0, 0, name])
         a[0] += t
         a[1] += 1
+        assert a[2] == name, (a[2], name)
+    total_ms = sum(v[0] for v in per.values())
     kernels = []
-    seen = set()
-    for op in ops:
-        for nf, prec, kt, dagger in op_kernels(op):
-            name = tm_kernel_label(w, nf, prec, kt, dagger)
-            if name in seen or name not in per:
-                continue
-            seen.add(name)
-            avg_ms = per[name][0] / per[name][1]
-            b = bytes_per_site(nf, prec, RECON, kt) * vh
-            f = flops_per_site(nf, kt) * vh
-            gbs = b / (avg_ms * 1e-3) / 1e9
-            kernels.append({"kernel": name, "flavors": nf, "prec": PREC_NAME[prec], "type": KT_NAME[kt], "dagger": dagger,
-                            "launches": per[name][1], "us": 1e3 * avg_ms, "gflops": f / (avg_ms * 1e-3) / 1e9,
-                            "alg_gbs": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_8TBs": gbs / 8000.0,
-                            "bytes_per_site": bytes_per_site(nf, prec, RECON, kt), "flops_per_site": flops_per_site(nf, kt),
-                            "share_of_step": per[name][0] / sum(v[0] for v in per.values())})
+    for (nf, prec, kt, dagger), (tot, cnt, name) in per.items():
+        avg_ms = tot / cnt
+        b = bytes_per_site(nf, prec, RECON, kt) * vh
+        f = flops_per_site(nf, kt) * vh
+        gbs = b / (avg_ms * 1e-3) / 1e9
+        kernels.append({"kernel": name, "flavors": nf, "prec": PREC_NAME[prec], "type": KT_NAME[kt], "dagger": dagger,
+                        "launches": cnt, "us": 1e3 * avg_ms, "gflops": f / (avg_ms * 1e-3) / 1e9,
+                        "alg_gbs": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_8TBs": gbs / 8000.0,
+                        "bytes_per_site": bytes_per_site(nf, prec, RECON, kt), "flops_per_site": flops_per_site(nf, kt),
+                        "share_of_step": tot / total_ms})
     dom = max(kernels, key=lambda k: k["share_of_step"]) if kernels else None
     roofline = None
     if dom:
@@ -395,10 +390,6 @@ def run_ours(args, log):
         dist.destroy_process_group()
 
 
-def tm_kernel_label(w, nf, prec, kt, dagger):
-    return kernel_name(nf, prec, kt, dagger)
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -407,6 +398,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", type=int, default=0, help="tm_set_path: 0 = default kernel selection, 1 = scalar kernels only")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
 

@@ -23,6 +23,19 @@ const TmKernelEntry *tm_generic_table(int prec, int nf)
     return nf == 1 ? tm_generic_table_2_1() : tm_generic_table_2_2();
 }
 
+const TmKernelEntry *tm_f2_table_4_1();
+const TmKernelEntry *tm_f2_table_4_2();
+const TmKernelEntry *tm_f2_table_2_1();
+const TmKernelEntry *tm_f2_table_2_2();
+
+// packed-FP32 (FFMA2) kernels: fp32 and half only (fp64 has no packed form)
+const TmKernelEntry *tm_f2_table(int prec, int nf)
+{
+    if (prec == 4) return nf == 1 ? tm_f2_table_4_1() : tm_f2_table_4_2();
+    if (prec == 2) return nf == 1 ? tm_f2_table_2_1() : tm_f2_table_2_2();
+    return nullptr;
+}
+
 namespace {
 
 thread_local char g_err[512] = "";
@@ -345,7 +358,9 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.kappa = p->kappa; a.kappa2 = p->kappa * p->kappa;
     a.tbound = (double)p->t_boundary;
 
-    const TmKernelEntry *tab = tm_generic_table((int)prec, out->nf);
+    // path 0: fp32 / half run the packed-FP32 kernels, fp64 the scalar kernel; path 1 forces the scalar kernel
+    const TmKernelEntry *tab = (c->path == 0 && (int)prec != TM_DOUBLE) ? tm_f2_table((int)prec, out->nf)
+                                                                       : tm_generic_table((int)prec, out->nf);
     const TmKernelEntry &k = tab[((g->recon == 18 ? 0 : 1) * 4 + (int)kt) * 2 + (dagger ? 1 : 0)];
     cudaError_t e;
     if (c->timing) {

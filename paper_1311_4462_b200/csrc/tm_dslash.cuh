@@ -46,19 +46,22 @@ TM_DEV void su3_mul(real *g, const real *u, const real *h)
     for (int s = 0; s < 2; s++)
 #pragma unroll
         for (int c = 0; c < 3; c++) {
-            real re = 0, im = 0;
+            real re, im;
 #pragma unroll
             for (int d = 0; d < 3; d++) {
                 const real hr = h[6 * s + 2 * d], hi = h[6 * s + 2 * d + 1];
-                if constexpr (!ADJ) {
-                    const real ur = u[2 * (3 * c + d)], ui = u[2 * (3 * c + d) + 1];
-                    re += ur * hr - ui * hi;
-                    im += ur * hi + ui * hr;
+                // explicit FMA chains (4 per complex multiply-add); ADJ: conj(U[d][c])
+                const real ur = ADJ ? u[2 * (3 * d + c)] : u[2 * (3 * c + d)];
+                const real ui = ADJ ? -u[2 * (3 * d + c) + 1] : u[2 * (3 * c + d) + 1];
+                if (d == 0) {
+                    re = ur * hr;
+                    im = ur * hi;
                 } else {
-                    const real ur = u[2 * (3 * d + c)], ui = u[2 * (3 * d + c) + 1];
-                    re += ur * hr + ui * hi;
-                    im += ur * hi - ui * hr;
+                    re = tm_fma(ur, hr, re);
+                    im = tm_fma(ur, hi, im);
                 }
+                re = tm_fma(-ui, hi, re);
+                im = tm_fma(ui, hr, im);
             }
             g[6 * s + 2 * c] = re;
             g[6 * s + 2 * c + 1] = im;

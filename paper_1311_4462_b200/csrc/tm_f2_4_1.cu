@@ -1,0 +1,4 @@
+// Instantiations of the packed-FP32 (FFMA2) fused dslash kernel: precision code 4, 1 flavor(s).
+#include "tm_dslash_f2.cuh"
+
+TM_F2_TABLE(4, 1)

@@ -5,7 +5,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#ifndef TM_DEV
 #define TM_DEV __device__ __forceinline__
+#endif
 
 template <int PREC> struct PrecTraits;
 template <> struct PrecTraits<8> { typedef double real; static constexpr int NCH = 12; };
@@ -14,6 +16,9 @@ template <> struct PrecTraits<2> { typedef float real;  static constexpr int NCH
 
 #define TM_HALF_MAX 32767.0f
 #define TM_HALF_INV (1.0f / 32767.0f)
+
+TM_DEV float tm_fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+TM_DEV double tm_fma(double a, double b, double c) { return __fma_rn(a, b, c); }
 
 // ---- raw 128-bit global accesses ------------------------------------------------------------------
 TM_DEV double2 ldg_d2(const void *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
@@ -24,21 +29,32 @@ TM_DEV int2 ldg_i2(const void *p) { return __ldg(reinterpret_cast<const int2 *>(
 TM_DEV int ldg_i1(const void *p) { return __ldg(reinterpret_cast<const int *>(p)); }
 TM_DEV float ldg_f1(const void *p) { return __ldg(reinterpret_cast<const float *>(p)); }
 
-// two int16 packed in one 32-bit word -> two floats (exact), times s
+// Stored int16 are OFFSET BINARY (u = q + 32768, see tm_f2.cuh): two per 32-bit word -> two floats (exact), times s
 TM_DEV void unpack2(int w, float s, float &lo, float &hi)
 {
-    lo = (float)(short)(w & 0xffff) * s;
-    hi = (float)(w >> 16) * s;
+    lo = (float)((int)(w & 0xffff) - 32768) * s;
+    hi = (float)((int)((unsigned)w >> 16) - 32768) * s;
 }
 TM_DEV int pack2(float lo, float hi)
 {
-    int a = __float2int_rn(lo), b = __float2int_rn(hi);
+    int a = __float2int_rn(lo) + 32768, b = __float2int_rn(hi) + 32768;
     return (a & 0xffff) | (b << 16);
+}
+
+// fp32 / half spinors keep a site's 24 reals in the order [half u/l][color][re/im][spin within the half], so that a
+// 64-bit register pair holds the same (color, re/im) of two spin components (the packed-FP32 kernels, tm_f2.cuh).
+// raw_pos(o): position in that order of the canonical real o = (spin*3+color)*2+reim.  fp64 stays canonical.
+__host__ __device__ constexpr int raw_pos(int o)
+{
+    return ((o / 6) / 2) * 12 + ((o / 2) % 3) * 4 + (o % 2) * 2 + ((o / 6) % 2);
 }
 
 // ---- spinor loads ---------------------------------------------------------------------------------
 // `base` points at the flavor's chunk block, `norm` at the flavor's norm array (half only), Vh = sites.
 // PART: 0 = all 24 reals, 1 = upper only (v[0..11] valid), 2 = lower only (v[12..23] valid).
+template <int PART>
+TM_DEV void load_spinor_half_raw(float *v, const char *base, const float *norm, int Vh, int idx);
+
 template <int PREC, int PART>
 TM_DEV void load_spinor(typename PrecTraits<PREC>::real *v, const char *base, const float *norm, int Vh, int idx)
 {
@@ -52,16 +68,30 @@ TM_DEV void load_spinor(typename PrecTraits<PREC>::real *v, const char *base, co
         }
     } else if constexpr (PREC == 4) {
         constexpr int lo = (PART == 2) ? 3 : 0, hi = (PART == 1) ? 3 : 6;
+        float r[24];
 #pragma unroll
         for (int k = lo; k < hi; k++) {
             float4 c = ldg_f4(base + ((size_t)k * Vh + idx) * 16);
-            v[4 * k] = c.x;
-            v[4 * k + 1] = c.y;
-            v[4 * k + 2] = c.z;
-            v[4 * k + 3] = c.w;
+            r[4 * k] = c.x;
+            r[4 * k + 1] = c.y;
+            r[4 * k + 2] = c.z;
+            r[4 * k + 3] = c.w;
         }
+#pragma unroll
+        for (int o = (PART == 2 ? 12 : 0); o < (PART == 1 ? 12 : 24); o++) v[o] = r[raw_pos(o)];
     } else {
-        // 3 chunks of 8 int16: reals 0..7, 8..15, 16..23.  upper = 0..11, lower = 12..23.
+        // 3 chunks of 8 int16: raw 0..7, 8..15, 16..23.  upper = raw 0..11, lower = raw 12..23.
+        float r[24];
+        load_spinor_half_raw<PART>(r, base, norm, Vh, idx);
+#pragma unroll
+        for (int o = (PART == 2 ? 12 : 0); o < (PART == 1 ? 12 : 24); o++) v[o] = r[raw_pos(o)];
+    }
+}
+
+template <int PART>
+TM_DEV void load_spinor_half_raw(float *v, const char *base, const float *norm, int Vh, int idx)
+{
+    {
         const float s = ldg_f1(norm + idx) * TM_HALF_INV;
         if constexpr (PART != 2) {
             int4 c = ldg_i4(base + ((size_t)0 * Vh + idx) * 16);
@@ -100,11 +130,18 @@ TM_DEV void store_spinor(const typename PrecTraits<PREC>::real *v, char *base, f
         for (int k = 0; k < 12; k++)
             *reinterpret_cast<double2 *>(base + ((size_t)k * Vh + idx) * 16) = make_double2(v[2 * k], v[2 * k + 1]);
     } else if constexpr (PREC == 4) {
+        float r[24];
+#pragma unroll
+        for (int o = 0; o < 24; o++) r[raw_pos(o)] = v[o];
 #pragma unroll
         for (int k = 0; k < 6; k++)
             *reinterpret_cast<float4 *>(base + ((size_t)k * Vh + idx) * 16) =
-                make_float4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+                make_float4(r[4 * k], r[4 * k + 1], r[4 * k + 2], r[4 * k + 3]);
     } else {
+        float r[24];
+#pragma unroll
+        for (int o = 0; o < 24; o++) r[raw_pos(o)] = v[o];
+        v = r;
         float m = 0.f;
 #pragma unroll
         for (int i = 0; i < 24; i++) m = fmaxf(m, fabsf(v[i]));
@@ -135,8 +172,9 @@ TM_DEV void rebuild_row2(real *u)
         const real br = u[2 * (3 + c2)], bi = u[2 * (3 + c2) + 1];   // row1[c2]
         const real cr = u[2 * c2], ci = u[2 * c2 + 1];               // row0[c2]
         const real dr = u[2 * (3 + c1)], di = u[2 * (3 + c1) + 1];   // row1[c1]
-        u[2 * (6 + c)] = (ar * br - ai * bi) - (cr * dr - ci * di);
-        u[2 * (6 + c) + 1] = -((ar * bi + ai * br) - (cr * di + ci * dr));
+        // explicit FMA chains: 4 + 4 instructions per component
+        u[2 * (6 + c)] = tm_fma(ci, di, tm_fma(-cr, dr, tm_fma(-ai, bi, ar * br)));
+        u[2 * (6 + c) + 1] = tm_fma(ci, dr, tm_fma(cr, di, tm_fma(-ai, br, -(ar * bi))));
     }
 }
 

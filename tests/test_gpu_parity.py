@@ -37,6 +37,7 @@ def bench_for(dims, kind, seed):
     key = (tuple(dims), kind, seed)
     if key not in _cache:
         _cache[key] = Bench(dims, si.gauge_field(dims, seed, kind))
+    tm.tm_set_path(_cache[key].lat.ctx, 0)         # default kernel selection unless a test asks otherwise
     return _cache[key]
 
 
@@ -76,9 +77,11 @@ def test_t1_spinor_pack_unpack_round_trip(dims, nf):
 
 @pytest.mark.parametrize("dims,kind", [((4, 4, 4, 8), "haar"), ((4, 6, 8, 10), "near_identity"), ((8, 4, 6, 4), "haar")])
 @pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
-def test_t2_every_kernel_variant_matches_oracle(dims, kind, kw):
+@pytest.mark.parametrize("path", [0, 1], ids=["default-kernels", "scalar-kernels"])
+def test_t2_every_kernel_variant_matches_oracle(dims, kind, kw, path):
     nf = nf_of(kw)
     bench = bench_for(dims, kind, 1)
+    tm.tm_set_path(bench.lat.ctx, path)
     po = oracle.params(dims, KAPPA, **kw)
     pg = tm.params(KAPPA, **kw)
     full_in, full_x = si.spinor_field(dims, nf, 2), si.spinor_field(dims, nf, 3)
