@@ -31,7 +31,7 @@ EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
     "tm_field_device_ptr", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb",
     "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_last_error",
-    "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_timing_enable", "tm_timing_read",
+    "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_set_tuning", "tm_timing_enable", "tm_timing_read",
 ]
 
 
@@ -90,6 +90,7 @@ def lib():
     L.tm_last_kernel_name.argtypes = [vp]
     L.tm_last_kernel_name.restype = ctypes.c_char_p
     L.tm_set_path.argtypes = [vp, i]
+    L.tm_set_tuning.argtypes = [vp, ctypes.c_char_p, i]
     L.tm_timing_enable.argtypes = [vp, i]
     L.tm_timing_read.argtypes = [vp, i, ctypes.POINTER(ctypes.c_char_p), ctypes.POINTER(ctypes.c_float),
                                  ctypes.POINTER(i)]
@@ -198,6 +199,10 @@ def tm_last_kernel_name(ctx):
 
 def tm_set_path(ctx, path):
     _check(lib().tm_set_path(ctx, int(path)))
+
+
+def tm_set_tuning(ctx, key, value):
+    _check(lib().tm_set_tuning(ctx, key.encode(), int(value)))
 
 
 def tm_timing_enable(ctx, on):

@@ -143,6 +143,9 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->launches = 0;
     c->last_kernel = "";
     c->path = 0;
+    c->pf_dist = 0;
+    c->stage = -1;
+    c->block_threads = 0;
     c->sm_count = 0;
     c->staging = nullptr;
     c->staging_bytes = 0;
@@ -214,6 +217,27 @@ int tm_set_path(tm_ctx *ctx, int path)
     if (!ctx || path < 0 || path > 1) return fail(TM_ERR_ARG, "tm_set_path: bad argument");
     ctx->path = path;
     return TM_OK;
+}
+
+int tm_set_tuning(tm_ctx *ctx, const char *key, int value)
+{
+    if (!ctx || !key) return fail(TM_ERR_ARG, "tm_set_tuning: NULL argument");
+    if (!strcmp(key, "prefetch_blocks")) {
+        if (value < 0) return fail(TM_ERR_ARG, "prefetch_blocks must be >= 0");
+        ctx->pf_dist = value;
+        return TM_OK;
+    }
+    if (!strcmp(key, "stage_links")) {
+        if (value < -1 || value > 1) return fail(TM_ERR_ARG, "stage_links must be -1 (default), 0 or 1");
+        ctx->stage = value;
+        return TM_OK;
+    }
+    if (!strcmp(key, "block_threads")) {
+        if (value != 0 && value != 32 && value != 64 && value != 128) return fail(TM_ERR_ARG, "block_threads must be 0 (default), 32, 64 or 128");
+        ctx->block_threads = value;
+        return TM_OK;
+    }
+    return fail(TM_ERR_ARG, "tm_set_tuning: unknown key '%s'", key);
 }
 
 long tm_launch_count(const tm_ctx *ctx) { return ctx ? ctx->launches : 0; }
@@ -357,11 +381,16 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.alpha = co.alpha; a.beta = co.beta; a.scale = co.scale;
     a.kappa = p->kappa; a.kappa2 = p->kappa * p->kappa;
     a.tbound = (double)p->t_boundary;
+    a.pf_dist = c->pf_dist;
+    // launch shape: library defaults unless overridden through tm_set_tuning
+    int stage = c->stage >= 0 ? c->stage : 0;
+    a.block_threads = c->block_threads ? c->block_threads : 128;
+    while (stage && (size_t)8 * g->recon * (int)prec * a.block_threads > 96 * 1024 && a.block_threads > 32) a.block_threads /= 2;
 
     // path 0: fp32 / half run the packed-FP32 kernels, fp64 the scalar kernel; path 1 forces the scalar kernel
     const TmKernelEntry *tab = (c->path == 0 && (int)prec != TM_DOUBLE) ? tm_f2_table((int)prec, out->nf)
                                                                        : tm_generic_table((int)prec, out->nf);
-    const TmKernelEntry &k = tab[((g->recon == 18 ? 0 : 1) * 4 + (int)kt) * 2 + (dagger ? 1 : 0)];
+    const TmKernelEntry &k = tab[(((g->recon == 18 ? 0 : 1) * 4 + (int)kt) * 2 + (dagger ? 1 : 0)) * 2 + stage];
     cudaError_t e;
     if (c->timing) {
         tm_ctx::TimedLaunch t;

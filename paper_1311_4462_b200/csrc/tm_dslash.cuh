@@ -1,5 +1,5 @@
 // tm_dslash.cuh -- the generic fused twisted-mass dslash kernel (rows a2-a9 of DESIGN.md).
-// One thread per (output site, flavor); direct 128-bit read-only loads, neighbour reuse through L1/L2.
+// One thread per output site (both flavors of a doublet); direct 128-bit read-only loads, neighbour reuse through L1/L2.
 // Works for every even lattice with extents >= 4; the tiled TMA path (tm_dslash_tma.cuh) takes over on
 // conforming lattices.
 //
@@ -10,6 +10,7 @@
 #pragma once
 #include "tm_internal.h"
 #include "tm_layout.cuh"
+#include "tm_stream.cuh"
 
 // ---- spin projection (a3): 24 -> 12 reals -----------------------------------------------------------
 template <int MU, int SGN, typename real>
@@ -103,27 +104,35 @@ TM_DEV void reconstruct_acc(real *acc, const real *g, real w)
     }
 }
 
-// one of the 8 hops.  FWD: U_mu(x) psi(x+mu) with (1 - sgn gamma_mu);  else U_mu(x-mu)^dag psi(x-mu), (1 + sgn gamma_mu)
-template <int PREC, int RECON, int MU, bool FWD, bool DAG>
-TM_DEV void hop(typename PrecTraits<PREC>::real *acc, const char *in, const float *in_norm, const char *gauge_blk,
-                int Vh, int nbr, int link_idx, typename PrecTraits<PREC>::real w)
+// one of the 8 hops.  FWD: U_mu(x) psi(x+mu) with (1 - sgn gamma_mu);  else U_mu(x-mu)^dag psi(x-mu), (1 + sgn gamma_mu).
+// a6: the link is fetched (and its third row rebuilt) once and applied to every flavor.
+// STG: the link was staged in shared memory (tm_stream.cuh): L addresses the block's [plane][thread] slots and
+// WAITN is the number of younger cp.async groups that may still be pending.
+template <int PREC, int NF, int RECON, int MU, bool FWD, bool DAG, bool STG, int WAITN>
+TM_DEV void hop(typename PrecTraits<PREC>::real *acc, const char *in, const float *in_norm, size_t fl_bytes,
+                const LinkSrc L, int Vh, int nbr, typename PrecTraits<PREC>::real w)
 {
     typedef typename PrecTraits<PREC>::real real;
     constexpr int SGN = (FWD != DAG) ? +1 : -1;     // projector sign: forward carries (1 - gamma) unless daggered
-    real h[12], g[12], u[18];
-    if constexpr (MU == 3) {
-        real v[24];
-        load_spinor<PREC, (SGN > 0) ? 2 : 1>(v, in, in_norm, Vh, nbr);
+    real u[18];
+    if constexpr (STG) cp_async_wait<WAITN>();
+    load_link<PREC, RECON, STG>(u, L.base, L.stride, L.idx);
 #pragma unroll
-        for (int i = 0; i < 12; i++) h[i] = (SGN > 0) ? v[12 + i] : v[i];
-    } else {
-        real v[24];
-        load_spinor<PREC, 0>(v, in, in_norm, Vh, nbr);
-        project<MU, SGN>(h, v);
+    for (int f = 0; f < NF; f++) {
+        real h[12], g[12];
+        if constexpr (MU == 3) {
+            real v[24];
+            load_spinor<PREC, (SGN > 0) ? 2 : 1>(v, in + f * fl_bytes, in_norm + (size_t)f * Vh, Vh, nbr);
+#pragma unroll
+            for (int i = 0; i < 12; i++) h[i] = (SGN > 0) ? v[12 + i] : v[i];
+        } else {
+            real v[24];
+            load_spinor<PREC, 0>(v, in + f * fl_bytes, in_norm + (size_t)f * Vh, Vh, nbr);
+            project<MU, SGN>(h, v);
+        }
+        su3_mul<!FWD>(g, u, h);
+        reconstruct_acc<MU, SGN>(acc + 24 * f, g, w);
     }
-    load_link<PREC, RECON>(u, gauge_blk, Vh, link_idx);
-    su3_mul<!FWD>(g, u, h);
-    reconstruct_acc<MU, SGN>(acc, g, w);
 }
 
 // ---- local twist (a7):  w = scale * (v + i alpha gamma5 v + beta o),  o = the other flavor's v -----
@@ -147,51 +156,34 @@ TM_DEV void twist(real *w, const real *v, const real *o, real alpha, real beta, 
     }
 }
 
-template <typename real>
-TM_DEV void other_flavor(real *o, const real *v)
-{
-#pragma unroll
-    for (int i = 0; i < 24; i++) o[i] = __shfl_xor_sync(0xffffffffu, v[i], 16);
-}
-
-// The fused epilogue: KT 0 = A, 1 = A-xpay, 2 = B, 3 = REC.  acc is overwritten with the output.
+// The fused epilogue: KT 0 = A, 1 = A-xpay, 2 = B, 3 = REC.  acc (NF x 24) is overwritten with the output.
+// Flavor f sees tau3 = +1 (f = 0) or -1 (f = 1) and, through beta tau1, the other flavor's vector.
 template <int NF, int KT, typename real>
 TM_DEV void epilogue(real *acc, const real *xv, real alpha, real beta, real scale, real kappa, real kappa2)
 {
-    real v[24], o[24], w[24];
+    real v[NF * 24], w[NF * 24];
 #pragma unroll
-    for (int i = 0; i < 24; i++) v[i] = (KT == 2) ? xv[i] : (KT == 3) ? xv[i] + kappa * acc[i] : acc[i];
-    if constexpr (NF == 2) other_flavor(o, v);
-    twist<NF>(w, v, o, alpha, beta, scale);
+    for (int i = 0; i < NF * 24; i++) v[i] = (KT == 2) ? xv[i] : (KT == 3) ? xv[i] + kappa * acc[i] : acc[i];
 #pragma unroll
-    for (int i = 0; i < 24; i++) {
+    for (int f = 0; f < NF; f++) twist<NF>(w + 24 * f, v + 24 * f, v + 24 * (NF - 1 - f), f == 0 ? alpha : -alpha, beta, scale);
+#pragma unroll
+    for (int i = 0; i < NF * 24; i++) {
         if constexpr (KT == 0 || KT == 3) acc[i] = w[i];
         else if constexpr (KT == 1) acc[i] = xv[i] - kappa2 * w[i];
         else acc[i] = w[i] - kappa2 * acc[i];
     }
 }
 
-template <int PREC, int NF, int RECON, int KT, bool DAG>
-__global__ void __launch_bounds__(128) tm_dslash_generic(const DslashArgs a)
+
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
+__global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? 3 : (PREC == 8 ? 2 : 1)) tm_dslash_generic(const DslashArgs a)
 {
     typedef typename PrecTraits<PREC>::real real;
     constexpr int NCH = PrecTraits<PREC>::NCH;
     const int Vh = a.Vh;
-    int site, f;
-    bool active;
-    if constexpr (NF == 2) {         // a6: lanes 0-15 carry flavor 0, lanes 16-31 flavor 1 of the same 16 sites;
-        const int lane = threadIdx.x & 31;          // both halves issue the same link addresses -> one fetch
-        const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-        f = lane >> 4;
-        site = warp * 16 + (lane & 15);
-        active = site < Vh;
-        if (!active) site = Vh - 1;  // keep the lane alive for the flavor shuffle
-    } else {
-        f = 0;
-        site = blockIdx.x * blockDim.x + threadIdx.x;
-        active = site < Vh;
-        if (!active) return;
-    }
+    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x);
+    const int site = blockIdx.x * blockDim.x + threadIdx.x;        // one thread per output site, all flavors
+    if (site >= Vh) return;
 
     // a2: site decode and neighbours
     const int Xh = a.Xh;
@@ -214,59 +206,83 @@ __global__ void __launch_bounds__(128) tm_dslash_generic(const DslashArgs a)
     const real wtp = (real)2 * ((t == a.T - 1) ? (real)a.tbound : (real)1);
     const real wtm = (real)2 * ((t == 0) ? (real)a.tbound : (real)1);
 
-    const size_t fl_bytes = (size_t)NCH * Vh * 16;
-    const char *in = static_cast<const char *>(a.in) + f * fl_bytes;
-    const float *in_norm = reinterpret_cast<const float *>(static_cast<const char *>(a.in) + NF * fl_bytes) + (size_t)f * Vh;
+    const size_t fl_bytes = (size_t)NCH * Vh * 16;                      // one flavor's chunk block
+    const char *in = static_cast<const char *>(a.in);
+    const float *in_norm = reinterpret_cast<const float *>(in + NF * fl_bytes);
     const size_t blk = (size_t)RECON * PREC * Vh;                       // one [parity][mu] block
     const char *gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * 4 * blk;        // U_mu(x)
     const char *gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * 4 * blk;  // U_mu(x - mu)
 
-    real acc[24];
+    // a4 (staged): start all 8 link copies now; hops consume them in order
+    const int nt = blockDim.x, tid = threadIdx.x;
+    constexpr int LB = RECON * PREC;                                    // bytes of one stored link
+    if constexpr (STG) {
+        stage_link<PREC, RECON>(tm_smem + 0 * LB * nt, gf + 0 * blk, Vh, site, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 1 * LB * nt, gb + 0 * blk, Vh, xm, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 2 * LB * nt, gf + 1 * blk, Vh, site, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 3 * LB * nt, gb + 1 * blk, Vh, ym, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 4 * LB * nt, gf + 2 * blk, Vh, site, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 5 * LB * nt, gb + 2 * blk, Vh, zm, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 6 * LB * nt, gf + 3 * blk, Vh, site, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 7 * LB * nt, gb + 3 * blk, Vh, tm, nt, tid);
+    }
+    real acc[NF * 24];
 #pragma unroll
-    for (int i = 0; i < 24; i++) acc[i] = 0;
+    for (int i = 0; i < NF * 24; i++) acc[i] = 0;
 
-    hop<PREC, RECON, 0, true, DAG>(acc, in, in_norm, gf + 0 * blk, Vh, xp, site, (real)1);
-    hop<PREC, RECON, 0, false, DAG>(acc, in, in_norm, gb + 0 * blk, Vh, xm, xm, (real)1);
-    hop<PREC, RECON, 1, true, DAG>(acc, in, in_norm, gf + 1 * blk, Vh, yp, site, (real)1);
-    hop<PREC, RECON, 1, false, DAG>(acc, in, in_norm, gb + 1 * blk, Vh, ym, ym, (real)1);
-    hop<PREC, RECON, 2, true, DAG>(acc, in, in_norm, gf + 2 * blk, Vh, zp, site, (real)1);
-    hop<PREC, RECON, 2, false, DAG>(acc, in, in_norm, gb + 2 * blk, Vh, zm, zm, (real)1);
-    hop<PREC, RECON, 3, true, DAG>(acc, in, in_norm, gf + 3 * blk, Vh, tp, site, wtp);
-    hop<PREC, RECON, 3, false, DAG>(acc, in, in_norm, gb + 3 * blk, Vh, tm, tm, wtm);
+    hop<PREC, NF, RECON, 0, true, DAG, STG, 7>(acc, in, in_norm, fl_bytes, link_src<STG>(0, LB, gf + 0 * blk, Vh, site), Vh, xp, (real)1);
+    hop<PREC, NF, RECON, 0, false, DAG, STG, 6>(acc, in, in_norm, fl_bytes, link_src<STG>(1, LB, gb + 0 * blk, Vh, xm), Vh, xm, (real)1);
+    hop<PREC, NF, RECON, 1, true, DAG, STG, 5>(acc, in, in_norm, fl_bytes, link_src<STG>(2, LB, gf + 1 * blk, Vh, site), Vh, yp, (real)1);
+    hop<PREC, NF, RECON, 1, false, DAG, STG, 4>(acc, in, in_norm, fl_bytes, link_src<STG>(3, LB, gb + 1 * blk, Vh, ym), Vh, ym, (real)1);
+    hop<PREC, NF, RECON, 2, true, DAG, STG, 3>(acc, in, in_norm, fl_bytes, link_src<STG>(4, LB, gf + 2 * blk, Vh, site), Vh, zp, (real)1);
+    hop<PREC, NF, RECON, 2, false, DAG, STG, 2>(acc, in, in_norm, fl_bytes, link_src<STG>(5, LB, gb + 2 * blk, Vh, zm), Vh, zm, (real)1);
+    hop<PREC, NF, RECON, 3, true, DAG, STG, 1>(acc, in, in_norm, fl_bytes, link_src<STG>(6, LB, gf + 3 * blk, Vh, site), Vh, tp, wtp);
+    hop<PREC, NF, RECON, 3, false, DAG, STG, 0>(acc, in, in_norm, fl_bytes, link_src<STG>(7, LB, gb + 3 * blk, Vh, tm), Vh, tm, wtm);
 
     // a7: fused local epilogue
-    real xv[24];
+    real xv[NF * 24];
     if constexpr (KT != 0) {
-        const char *xb = static_cast<const char *>(a.x) + f * fl_bytes;
-        const float *xn = reinterpret_cast<const float *>(static_cast<const char *>(a.x) + NF * fl_bytes) + (size_t)f * Vh;
-        load_spinor<PREC, 0>(xv, xb, xn, Vh, site);
+        const char *xb = static_cast<const char *>(a.x);
+        const float *xn = reinterpret_cast<const float *>(xb + NF * fl_bytes);
+#pragma unroll
+        for (int f = 0; f < NF; f++) load_spinor<PREC, 0>(xv + 24 * f, xb + f * fl_bytes, xn + (size_t)f * Vh, Vh, site);
     }
-    const real alpha = (NF == 2 && f == 1) ? -(real)a.alpha : (real)a.alpha;     // tau3 = diag(1, -1)
-    epilogue<NF, KT>(acc, xv, alpha, (real)a.beta, (real)a.scale, (real)a.kappa, (real)a.kappa2);
+    epilogue<NF, KT>(acc, xv, (real)a.alpha, (real)a.beta, (real)a.scale, (real)a.kappa, (real)a.kappa2);
 
     // a8: single store
-    if (active) {
-        char *ob = static_cast<char *>(a.out) + f * fl_bytes;
-        float *on = reinterpret_cast<float *>(static_cast<char *>(a.out) + NF * fl_bytes) + (size_t)f * Vh;
-        store_spinor<PREC>(acc, ob, on, Vh, site);
-    }
+    char *ob = static_cast<char *>(a.out);
+    float *on = reinterpret_cast<float *>(ob + NF * fl_bytes);
+#pragma unroll
+    for (int f = 0; f < NF; f++) store_spinor<PREC>(acc + 24 * f, ob + f * fl_bytes, on + (size_t)f * Vh, Vh, site);
 }
 
-template <int PREC, int NF, int RECON, int KT, bool DAG>
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
 cudaError_t tm_launch_generic(const DslashArgs &a, cudaStream_t s)
 {
-    const int threads = 128;
-    const long nthreads = (NF == 2) ? 2L * ((a.Vh + 15) / 16) * 16 : a.Vh;
-    const int blocks = (int)((nthreads + threads - 1) / threads);
-    tm_dslash_generic<PREC, NF, RECON, KT, DAG><<<blocks, threads, 0, s>>>(a);
+    const int threads = a.block_threads;
+    const int blocks = (a.Vh + threads - 1) / threads;
+    const size_t smem = STG ? (size_t)8 * RECON * PREC * threads : 0;
+    if (smem > 48 * 1024) {
+        static bool raised = false;      // per instantiation
+        if (!raised) {
+            cudaError_t e = cudaFuncSetAttribute(tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG>,
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+            if (e != cudaSuccess) return e;
+            raised = true;
+        }
+    }
+    tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG><<<blocks, threads, smem, s>>>(a);
     return cudaGetLastError();
 }
 
-#define TM_GENERIC_ROW(P, N, R, K)                                                                    \
-    {tm_launch_generic<P, N, R, K, false>, "generic<" #P "," #N "," #R "," #K ",plain>"},            \
-    {tm_launch_generic<P, N, R, K, true>, "generic<" #P "," #N "," #R "," #K ",dagger>"}
+// table index: [recon18?0:1][kt 0..3][dagger 0..1][staged 0..1]
+#define TM_GENERIC_ROW(P, N, R, K)                                                                          \
+    {tm_launch_generic<P, N, R, K, false, false>, "generic<" #P "," #N "," #R "," #K ",plain>"},           \
+    {tm_launch_generic<P, N, R, K, false, true>, "generic_staged<" #P "," #N "," #R "," #K ",plain>"},     \
+    {tm_launch_generic<P, N, R, K, true, false>, "generic<" #P "," #N "," #R "," #K ",dagger>"},           \
+    {tm_launch_generic<P, N, R, K, true, true>, "generic_staged<" #P "," #N "," #R "," #K ",dagger>"}
 #define TM_GENERIC_TABLE(P, N)                                                                        \
-    static const TmKernelEntry table_##P##_##N[16] = {                                               \
+    static const TmKernelEntry table_##P##_##N[32] = {                                               \
         TM_GENERIC_ROW(P, N, 18, 0), TM_GENERIC_ROW(P, N, 18, 1), TM_GENERIC_ROW(P, N, 18, 2),       \
         TM_GENERIC_ROW(P, N, 18, 3), TM_GENERIC_ROW(P, N, 12, 0), TM_GENERIC_ROW(P, N, 12, 1),       \
         TM_GENERIC_ROW(P, N, 12, 2), TM_GENERIC_ROW(P, N, 12, 3)};                                   \

@@ -18,6 +18,7 @@
 #include "tm_f2.cuh"
 #include "tm_internal.h"
 #include "tm_layout.cuh"
+#include "tm_stream.cuh"
 
 #define TM_INV15 (1.0f / 32767.0f)
 
@@ -55,31 +56,30 @@ TM_DEV void load_spinor_f2(f2 *S, const char *base, int Vh, int idx)
 
 // Link as 9 (re, im) pairs W[row*3+col]; half: RAW integers for rows 0,1 (12-real: row 2 rebuilt and rescaled to
 // the same raw scale).  a4 of DESIGN.md.
-template <int PREC, int RECON>
+template <int PREC, int RECON, bool SM>
 TM_DEV void load_link_f2(f2 *W, const char *base, int Vh, int idx)
 {
     if constexpr (PREC == 4) {
         constexpr int NF4 = (RECON == 18) ? 4 : 3;
-        const float4 *p = reinterpret_cast<const float4 *>(base) + idx;
 #pragma unroll
         for (int k = 0; k < NF4; k++) {
-            const float4 c = __ldg(p + (size_t)k * Vh);
+            const float4 c = ld_f4<SM>(base + ((size_t)k * Vh + idx) * 16);
             W[2 * k] = mk2(c.x, c.y);
             W[2 * k + 1] = mk2(c.z, c.w);
         }
         if constexpr (RECON == 18) {
-            const float2 c = __ldg(reinterpret_cast<const float2 *>(base + (size_t)4 * Vh * 16) + idx);
+            const float2 c = ld_f2<SM>(base + (size_t)4 * Vh * 16 + (size_t)idx * 8);
             W[8] = mk2(c.x, c.y);
         }
     } else {
-        const int4 c = __ldg(reinterpret_cast<const int4 *>(base) + idx);
+        const int4 c = ld_i4<SM>(base + (size_t)idx * 16);
         W[0] = cvt_pair(c.x); W[1] = cvt_pair(c.y); W[2] = cvt_pair(c.z); W[3] = cvt_pair(c.w);
         if constexpr (RECON == 18) {
-            const int4 d = __ldg(reinterpret_cast<const int4 *>(base) + (size_t)Vh + idx);
+            const int4 d = ld_i4<SM>(base + ((size_t)Vh + idx) * 16);
             W[4] = cvt_pair(d.x); W[5] = cvt_pair(d.y); W[6] = cvt_pair(d.z); W[7] = cvt_pair(d.w);
-            W[8] = cvt_pair(__ldg(reinterpret_cast<const int *>(base + (size_t)2 * Vh * 16) + idx));
+            W[8] = cvt_pair(ld_i1<SM>(base + (size_t)2 * Vh * 16 + (size_t)idx * 4));
         } else {
-            const int2 d = __ldg(reinterpret_cast<const int2 *>(base + (size_t)Vh * 16) + idx);
+            const int2 d = ld_i2<SM>(base + (size_t)Vh * 16 + (size_t)idx * 8);
             W[4] = cvt_pair(d.x); W[5] = cvt_pair(d.y);
         }
     }
@@ -181,24 +181,31 @@ TM_DEV void reconstruct_f2(f2 *A, const f2 *G, float w)
     }
 }
 
-template <int PREC, int RECON, int MU, bool FWD, bool DAG>
-TM_DEV void hop_f2(f2 *A, const char *in, const float *in_norm, const char *gauge_blk, int Vh, int nbr, int link_idx,
-                   float w)
+// a6: the link is fetched, converted and rebuilt once and applied to every flavor.
+template <int PREC, int NF, int RECON, int MU, bool FWD, bool DAG, bool STG, int WAITN>
+TM_DEV void hop_f2(f2 *A, const char *in, const float *in_norm, size_t fl_bytes, const LinkSrc L, int Vh, int nbr, float w)
 {
     constexpr int SGN = (FWD != DAG) ? +1 : -1;
-    f2 S[12], H[6], G[6], W[9];
-    if constexpr (MU == 3) {
-        load_spinor_f2<PREC, (SGN > 0) ? 2 : 1>(S, in, Vh, nbr);
+    f2 W[9];
+    if constexpr (STG) cp_async_wait<WAITN>();
+    load_link_f2<PREC, RECON, STG>(W, L.base, L.stride, L.idx);
 #pragma unroll
-        for (int i = 0; i < 6; i++) H[i] = (SGN > 0) ? S[6 + i] : S[i];
-    } else {
-        load_spinor_f2<PREC, 0>(S, in, Vh, nbr);
-        project_f2<MU, SGN>(H, S);
+    for (int f = 0; f < NF; f++) {
+        f2 S[12], H[6], G[6];
+        const char *inf = in + f * fl_bytes;
+        if constexpr (MU == 3) {
+            load_spinor_f2<PREC, (SGN > 0) ? 2 : 1>(S, inf, Vh, nbr);
+#pragma unroll
+            for (int i = 0; i < 6; i++) H[i] = (SGN > 0) ? S[6 + i] : S[i];
+        } else {
+            load_spinor_f2<PREC, 0>(S, inf, Vh, nbr);
+            project_f2<MU, SGN>(H, S);
+        }
+        float wf = w;
+        if constexpr (PREC == 2) wf *= __ldg(in_norm + (size_t)f * Vh + nbr) * (TM_INV15 * TM_INV15);   // site norm x link scale
+        su3_mul_f2<!FWD>(G, W, H);
+        reconstruct_f2<MU, SGN>(A + 12 * f, G, wf);
     }
-    if constexpr (PREC == 2) w *= __ldg(in_norm + nbr) * (TM_INV15 * TM_INV15);   // site norm x link scale
-    load_link_f2<PREC, RECON>(W, gauge_blk, Vh, link_idx);
-    su3_mul_f2<!FWD>(G, W, H);
-    reconstruct_f2<MU, SGN>(A, G, w);
 }
 
 // ---- a7: local twist, packed:  W = scale (V + i alpha gamma5 V + beta O) ------------------------------
@@ -225,20 +232,17 @@ TM_DEV void twist_f2(f2 *Wo, const f2 *V, const f2 *O, float alpha, float beta, 
     }
 }
 
+// A (NF x 12 pairs) is overwritten with the output; flavor f sees tau3 = +1 (f = 0) / -1 (f = 1) and the other flavor.
 template <int NF, int KT>
 TM_DEV void epilogue_f2(f2 *A, const f2 *X, float alpha, float beta, float scale, float kappa, float kappa2)
 {
-    f2 V[12], O[12], Wt[12];
+    f2 V[NF * 12], Wt[NF * 12];
 #pragma unroll
-    for (int i = 0; i < 12; i++) V[i] = (KT == 2) ? X[i] : (KT == 3) ? fma2(A[i], bc2(kappa), X[i]) : A[i];
-    if constexpr (NF == 2) {
+    for (int i = 0; i < NF * 12; i++) V[i] = (KT == 2) ? X[i] : (KT == 3) ? fma2(A[i], bc2(kappa), X[i]) : A[i];
 #pragma unroll
-        for (int i = 0; i < 12; i++)
-            O[i] = mk2(__shfl_xor_sync(0xffffffffu, V[i].x, 16), __shfl_xor_sync(0xffffffffu, V[i].y, 16));
-    }
-    twist_f2<NF>(Wt, V, O, alpha, beta, scale);
+    for (int f = 0; f < NF; f++) twist_f2<NF>(Wt + 12 * f, V + 12 * f, V + 12 * (NF - 1 - f), f == 0 ? alpha : -alpha, beta, scale);
 #pragma unroll
-    for (int i = 0; i < 12; i++) {
+    for (int i = 0; i < NF * 12; i++) {
         if constexpr (KT == 0 || KT == 3) A[i] = Wt[i];
         else if constexpr (KT == 1) A[i] = fma2(Wt[i], bc2(-kappa2), X[i]);
         else A[i] = fma2(A[i], bc2(-kappa2), Wt[i]);
@@ -272,26 +276,14 @@ TM_DEV void store_spinor_f2(const f2 *A, char *base, float *norm, int Vh, int id
     }
 }
 
-template <int PREC, int NF, int RECON, int KT, bool DAG>
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
 __global__ void __launch_bounds__(128) tm_dslash_f2(const DslashArgs a)
 {
     constexpr int NCH = PrecTraits<PREC>::NCH;
     const int Vh = a.Vh;
-    int site, f;
-    bool active;
-    if constexpr (NF == 2) {         // a6: lanes 0-15 flavor 0, lanes 16-31 flavor 1 of the same 16 sites
-        const int lane = threadIdx.x & 31;
-        const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-        f = lane >> 4;
-        site = warp * 16 + (lane & 15);
-        active = site < Vh;
-        if (!active) site = Vh - 1;
-    } else {
-        f = 0;
-        site = blockIdx.x * blockDim.x + threadIdx.x;
-        active = site < Vh;
-        if (!active) return;
-    }
+    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x);
+    const int site = blockIdx.x * blockDim.x + threadIdx.x;        // one thread per output site, all flavors
+    if (site >= Vh) return;
 
     // a2: site decode and neighbours
     const int Xh = a.Xh;
@@ -315,61 +307,87 @@ __global__ void __launch_bounds__(128) tm_dslash_f2(const DslashArgs a)
     const float wtm = 2.f * ((t == 0) ? (float)a.tbound : 1.f);
 
     const size_t fl_bytes = (size_t)NCH * Vh * 16;
-    const char *in = static_cast<const char *>(a.in) + f * fl_bytes;
-    const float *in_norm = reinterpret_cast<const float *>(static_cast<const char *>(a.in) + NF * fl_bytes) + (size_t)f * Vh;
+    const char *in = static_cast<const char *>(a.in);
+    const float *in_norm = reinterpret_cast<const float *>(in + NF * fl_bytes);
     const size_t blk = (size_t)RECON * PREC * Vh;
     const char *gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * 4 * blk;
     const char *gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * 4 * blk;
 
-    f2 A[12];
+    const int nt = blockDim.x, tid = threadIdx.x;
+    constexpr int LB = RECON * PREC;
+    if constexpr (STG) {
+        stage_link<PREC, RECON>(tm_smem + 0 * LB * nt, gf + 0 * blk, Vh, site, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 1 * LB * nt, gb + 0 * blk, Vh, xm, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 2 * LB * nt, gf + 1 * blk, Vh, site, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 3 * LB * nt, gb + 1 * blk, Vh, ym, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 4 * LB * nt, gf + 2 * blk, Vh, site, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 5 * LB * nt, gb + 2 * blk, Vh, zm, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 6 * LB * nt, gf + 3 * blk, Vh, site, nt, tid);
+        stage_link<PREC, RECON>(tm_smem + 7 * LB * nt, gb + 3 * blk, Vh, tm, nt, tid);
+    }
+
+    f2 A[NF * 12];
 #pragma unroll
-    for (int i = 0; i < 12; i++) A[i] = mk2(0.f, 0.f);
+    for (int i = 0; i < NF * 12; i++) A[i] = mk2(0.f, 0.f);
 
-    hop_f2<PREC, RECON, 0, true, DAG>(A, in, in_norm, gf + 0 * blk, Vh, xp, site, 1.f);
-    hop_f2<PREC, RECON, 0, false, DAG>(A, in, in_norm, gb + 0 * blk, Vh, xm, xm, 1.f);
-    hop_f2<PREC, RECON, 1, true, DAG>(A, in, in_norm, gf + 1 * blk, Vh, yp, site, 1.f);
-    hop_f2<PREC, RECON, 1, false, DAG>(A, in, in_norm, gb + 1 * blk, Vh, ym, ym, 1.f);
-    hop_f2<PREC, RECON, 2, true, DAG>(A, in, in_norm, gf + 2 * blk, Vh, zp, site, 1.f);
-    hop_f2<PREC, RECON, 2, false, DAG>(A, in, in_norm, gb + 2 * blk, Vh, zm, zm, 1.f);
-    hop_f2<PREC, RECON, 3, true, DAG>(A, in, in_norm, gf + 3 * blk, Vh, tp, site, wtp);
-    hop_f2<PREC, RECON, 3, false, DAG>(A, in, in_norm, gb + 3 * blk, Vh, tm, tm, wtm);
+    hop_f2<PREC, NF, RECON, 0, true, DAG, STG, 7>(A, in, in_norm, fl_bytes, link_src<STG>(0, LB, gf + 0 * blk, Vh, site), Vh, xp, 1.f);
+    hop_f2<PREC, NF, RECON, 0, false, DAG, STG, 6>(A, in, in_norm, fl_bytes, link_src<STG>(1, LB, gb + 0 * blk, Vh, xm), Vh, xm, 1.f);
+    hop_f2<PREC, NF, RECON, 1, true, DAG, STG, 5>(A, in, in_norm, fl_bytes, link_src<STG>(2, LB, gf + 1 * blk, Vh, site), Vh, yp, 1.f);
+    hop_f2<PREC, NF, RECON, 1, false, DAG, STG, 4>(A, in, in_norm, fl_bytes, link_src<STG>(3, LB, gb + 1 * blk, Vh, ym), Vh, ym, 1.f);
+    hop_f2<PREC, NF, RECON, 2, true, DAG, STG, 3>(A, in, in_norm, fl_bytes, link_src<STG>(4, LB, gf + 2 * blk, Vh, site), Vh, zp, 1.f);
+    hop_f2<PREC, NF, RECON, 2, false, DAG, STG, 2>(A, in, in_norm, fl_bytes, link_src<STG>(5, LB, gb + 2 * blk, Vh, zm), Vh, zm, 1.f);
+    hop_f2<PREC, NF, RECON, 3, true, DAG, STG, 1>(A, in, in_norm, fl_bytes, link_src<STG>(6, LB, gf + 3 * blk, Vh, site), Vh, tp, wtp);
+    hop_f2<PREC, NF, RECON, 3, false, DAG, STG, 0>(A, in, in_norm, fl_bytes, link_src<STG>(7, LB, gb + 3 * blk, Vh, tm), Vh, tm, wtm);
 
-    f2 X[12];
+    f2 X[NF * 12];
     if constexpr (KT != 0) {
-        const char *xb = static_cast<const char *>(a.x) + f * fl_bytes;
-        load_spinor_f2<PREC, 0>(X, xb, Vh, site);
-        if constexpr (PREC == 2) {
-            const float *xn = reinterpret_cast<const float *>(static_cast<const char *>(a.x) + NF * fl_bytes) + (size_t)f * Vh;
-            const float s = __ldg(xn + site) * TM_INV15;
+        const char *xb = static_cast<const char *>(a.x);
+        const float *xn = reinterpret_cast<const float *>(xb + NF * fl_bytes);
 #pragma unroll
-            for (int i = 0; i < 12; i++) X[i] = mul2(X[i], bc2(s));
+        for (int f = 0; f < NF; f++) {
+            load_spinor_f2<PREC, 0>(X + 12 * f, xb + f * fl_bytes, Vh, site);
+            if constexpr (PREC == 2) {
+                const float s = __ldg(xn + (size_t)f * Vh + site) * TM_INV15;
+#pragma unroll
+                for (int i = 0; i < 12; i++) X[12 * f + i] = mul2(X[12 * f + i], bc2(s));
+            }
         }
     }
-    const float alpha = (NF == 2 && f == 1) ? -(float)a.alpha : (float)a.alpha;
-    epilogue_f2<NF, KT>(A, X, alpha, (float)a.beta, (float)a.scale, (float)a.kappa, (float)a.kappa2);
+    epilogue_f2<NF, KT>(A, X, (float)a.alpha, (float)a.beta, (float)a.scale, (float)a.kappa, (float)a.kappa2);
 
-    if (active) {
-        char *ob = static_cast<char *>(a.out) + f * fl_bytes;
-        float *on = reinterpret_cast<float *>(static_cast<char *>(a.out) + NF * fl_bytes) + (size_t)f * Vh;
-        store_spinor_f2<PREC>(A, ob, on, Vh, site);
-    }
+    char *ob = static_cast<char *>(a.out);
+    float *on = reinterpret_cast<float *>(ob + NF * fl_bytes);
+#pragma unroll
+    for (int f = 0; f < NF; f++) store_spinor_f2<PREC>(A + 12 * f, ob + f * fl_bytes, on + (size_t)f * Vh, Vh, site);
 }
 
-template <int PREC, int NF, int RECON, int KT, bool DAG>
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
 cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
 {
-    const int threads = 128;
-    const long nthreads = (NF == 2) ? 2L * ((a.Vh + 15) / 16) * 16 : a.Vh;
-    const int blocks = (int)((nthreads + threads - 1) / threads);
-    tm_dslash_f2<PREC, NF, RECON, KT, DAG><<<blocks, threads, 0, s>>>(a);
+    const int threads = a.block_threads;
+    const int blocks = (a.Vh + threads - 1) / threads;
+    const size_t smem = STG ? (size_t)8 * RECON * PREC * threads : 0;
+    if (smem > 48 * 1024) {
+        static bool raised = false;      // per instantiation
+        if (!raised) {
+            cudaError_t e = cudaFuncSetAttribute(tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG>,
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+            if (e != cudaSuccess) return e;
+            raised = true;
+        }
+    }
+    tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG><<<blocks, threads, smem, s>>>(a);
     return cudaGetLastError();
 }
 
-#define TM_F2_ROW(P, N, R, K)                                                                \
-    {tm_launch_f2<P, N, R, K, false>, "f2<" #P "," #N "," #R "," #K ",plain>"},             \
-    {tm_launch_f2<P, N, R, K, true>, "f2<" #P "," #N "," #R "," #K ",dagger>"}
+// table index: [recon18?0:1][kt 0..3][dagger 0..1][staged 0..1]
+#define TM_F2_ROW(P, N, R, K)                                                                       \
+    {tm_launch_f2<P, N, R, K, false, false>, "f2<" #P "," #N "," #R "," #K ",plain>"},             \
+    {tm_launch_f2<P, N, R, K, false, true>, "f2_staged<" #P "," #N "," #R "," #K ",plain>"},       \
+    {tm_launch_f2<P, N, R, K, true, false>, "f2<" #P "," #N "," #R "," #K ",dagger>"},             \
+    {tm_launch_f2<P, N, R, K, true, true>, "f2_staged<" #P "," #N "," #R "," #K ",dagger>"}
 #define TM_F2_TABLE(P, N)                                                                    \
-    static const TmKernelEntry f2table_##P##_##N[16] = {                                    \
+    static const TmKernelEntry f2table_##P##_##N[32] = {                                    \
         TM_F2_ROW(P, N, 18, 0), TM_F2_ROW(P, N, 18, 1), TM_F2_ROW(P, N, 18, 2),             \
         TM_F2_ROW(P, N, 18, 3), TM_F2_ROW(P, N, 12, 0), TM_F2_ROW(P, N, 12, 1),             \
         TM_F2_ROW(P, N, 12, 2), TM_F2_ROW(P, N, 12, 3)};                                    \

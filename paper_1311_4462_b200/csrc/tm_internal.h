@@ -31,6 +31,9 @@ struct tm_ctx {
     long launches;
     const char *last_kernel;
     int path;    // 0 auto, 1 generic only
+    int pf_dist; // tm_set_tuning("prefetch_blocks")
+    int stage;   // tm_set_tuning("stage_links"): -1 library default, 0 direct loads, 1 links staged through shared memory
+    int block_threads;   // tm_set_tuning("block_threads"): 0 library default, else 32 / 64 / 128
     int sm_count;
     void *staging;        // device staging for upload / download
     size_t staging_bytes;
@@ -75,6 +78,8 @@ struct DslashArgs {
     double kappa;        // REC
     double kappa2;       // A-xpay, B
     double tbound;       // +-1, multiplies the time hop that wraps
+    int block_threads;   // threads per block (= sites per block)
+    int pf_dist;         // L2 prefetch distance in thread blocks (0 = off): block b prefetches the tile of block b + pf_dist
 };
 
 // kernel launchers (one translation unit per precision x flavor count)
@@ -83,7 +88,7 @@ struct TmKernelEntry {
     tm_launch_fn fn;
     const char *name;
 };
-// index: [recon18?0:1][kt 0..3][dagger 0..1]
+// index: [recon18?0:1][kt 0..3][dagger 0..1][staged 0..1]
 const TmKernelEntry *tm_generic_table(int prec, int nf);
 
 // pack / unpack (tm_pack.cu)

@@ -28,6 +28,13 @@ TM_DEV int4 ldg_i4(const void *p) { return __ldg(reinterpret_cast<const int4 *>(
 TM_DEV int2 ldg_i2(const void *p) { return __ldg(reinterpret_cast<const int2 *>(p)); }
 TM_DEV int ldg_i1(const void *p) { return __ldg(reinterpret_cast<const int *>(p)); }
 TM_DEV float ldg_f1(const void *p) { return __ldg(reinterpret_cast<const float *>(p)); }
+// SM = true: the pointer is shared memory (staged links, tm_stream.cuh) -> plain loads
+template <bool SM> TM_DEV double2 ld_d2(const void *p) { if constexpr (SM) return *reinterpret_cast<const double2 *>(p); else return ldg_d2(p); }
+template <bool SM> TM_DEV float4 ld_f4(const void *p) { if constexpr (SM) return *reinterpret_cast<const float4 *>(p); else return ldg_f4(p); }
+template <bool SM> TM_DEV float2 ld_f2(const void *p) { if constexpr (SM) return *reinterpret_cast<const float2 *>(p); else return ldg_f2(p); }
+template <bool SM> TM_DEV int4 ld_i4(const void *p) { if constexpr (SM) return *reinterpret_cast<const int4 *>(p); else return ldg_i4(p); }
+template <bool SM> TM_DEV int2 ld_i2(const void *p) { if constexpr (SM) return *reinterpret_cast<const int2 *>(p); else return ldg_i2(p); }
+template <bool SM> TM_DEV int ld_i1(const void *p) { if constexpr (SM) return *reinterpret_cast<const int *>(p); else return ldg_i1(p); }
 
 // Stored int16 are OFFSET BINARY (u = q + 32768, see tm_f2.cuh): two per 32-bit word -> two floats (exact), times s
 TM_DEV void unpack2(int w, float s, float &lo, float &hi)
@@ -178,13 +185,13 @@ TM_DEV void rebuild_row2(real *u)
     }
 }
 
-template <int PREC, int RECON>
+template <int PREC, int RECON, bool SM = false>
 TM_DEV void load_link(typename PrecTraits<PREC>::real *u, const char *base, int Vh, int idx)
 {
     if constexpr (PREC == 8) {
 #pragma unroll
         for (int k = 0; k < RECON / 2; k++) {
-            double2 c = ldg_d2(base + ((size_t)k * Vh + idx) * 16);
+            double2 c = ld_d2<SM>(base + ((size_t)k * Vh + idx) * 16);
             u[2 * k] = c.x;
             u[2 * k + 1] = c.y;
         }
@@ -192,37 +199,59 @@ TM_DEV void load_link(typename PrecTraits<PREC>::real *u, const char *base, int 
         constexpr int NF4 = (RECON == 18) ? 4 : 3;
 #pragma unroll
         for (int k = 0; k < NF4; k++) {
-            float4 c = ldg_f4(base + ((size_t)k * Vh + idx) * 16);
+            float4 c = ld_f4<SM>(base + ((size_t)k * Vh + idx) * 16);
             u[4 * k] = c.x;
             u[4 * k + 1] = c.y;
             u[4 * k + 2] = c.z;
             u[4 * k + 3] = c.w;
         }
         if constexpr (RECON == 18) {
-            float2 c = ldg_f2(base + (size_t)4 * Vh * 16 + (size_t)idx * 8);
+            float2 c = ld_f2<SM>(base + (size_t)4 * Vh * 16 + (size_t)idx * 8);
             u[16] = c.x;
             u[17] = c.y;
         }
     } else {
         const float s = TM_HALF_INV;
-        int4 c = ldg_i4(base + (size_t)idx * 16);
+        int4 c = ld_i4<SM>(base + (size_t)idx * 16);
         unpack2(c.x, s, u[0], u[1]);
         unpack2(c.y, s, u[2], u[3]);
         unpack2(c.z, s, u[4], u[5]);
         unpack2(c.w, s, u[6], u[7]);
         if constexpr (RECON == 18) {
-            int4 d = ldg_i4(base + ((size_t)Vh + idx) * 16);
+            int4 d = ld_i4<SM>(base + ((size_t)Vh + idx) * 16);
             unpack2(d.x, s, u[8], u[9]);
             unpack2(d.y, s, u[10], u[11]);
             unpack2(d.z, s, u[12], u[13]);
             unpack2(d.w, s, u[14], u[15]);
-            int e = ldg_i1(base + (size_t)2 * Vh * 16 + (size_t)idx * 4);
+            int e = ld_i1<SM>(base + (size_t)2 * Vh * 16 + (size_t)idx * 4);
             unpack2(e, s, u[16], u[17]);
         } else {
-            int2 d = ldg_i2(base + (size_t)Vh * 16 + (size_t)idx * 8);
+            int2 d = ld_i2<SM>(base + (size_t)Vh * 16 + (size_t)idx * 8);
             unpack2(d.x, s, u[8], u[9]);
             unpack2(d.y, s, u[10], u[11]);
         }
     }
     if constexpr (RECON == 12) rebuild_row2(u);
+}
+
+// ---- L2 prefetch of a later tile ("streaming") ---------------------------------------
+// A link block [parity][mu] is a sequence of planes, plane p = Vh elements of link_plane_width(p) bytes.
+template <int PREC, int RECON> __host__ __device__ constexpr int link_planes()
+{
+    return PREC == 8 ? RECON / 2 : PREC == 4 ? (RECON == 18 ? 5 : 3) : (RECON == 18 ? 3 : 2);
+}
+template <int PREC, int RECON> __host__ __device__ constexpr int link_plane_width(int p)
+{
+    return PREC == 8 ? 16 : PREC == 4 ? (p < 4 ? 16 : 8) : (RECON == 18 ? (p < 2 ? 16 : 4) : (p < 1 ? 16 : 8));
+}
+template <int PREC, int RECON> __host__ __device__ constexpr int link_plane_offset(int p)     // bytes per site before plane p
+{
+    int o = 0;
+    for (int q = 0; q < p; q++) o += link_plane_width<PREC, RECON>(q);
+    return o;
+}
+
+TM_DEV void prefetch_l2(const void *p, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }

@@ -26,6 +26,16 @@ FLAVORS = [
 ]
 
 
+# code paths of the library: (id, tm_set_path, tm_set_tuning overrides); results must not depend on them
+VARIANTS = [
+    ("default", 0, {}),
+    ("scalar", 1, {}),
+    ("packed-direct", 0, {"stage_links": 0, "block_threads": 128}),
+    ("packed-staged", 0, {"stage_links": 1, "block_threads": 64, "prefetch_blocks": 3}),
+    ("scalar-staged", 1, {"stage_links": 1, "block_threads": 32}),
+]
+
+
 def nf_of(kw):
     return 2 if kw["twist_flavor"] == 0 else 1
 
@@ -37,7 +47,11 @@ def bench_for(dims, kind, seed):
     key = (tuple(dims), kind, seed)
     if key not in _cache:
         _cache[key] = Bench(dims, si.gauge_field(dims, seed, kind))
-    tm.tm_set_path(_cache[key].lat.ctx, 0)         # default kernel selection unless a test asks otherwise
+    ctx = _cache[key].lat.ctx                       # default kernel selection unless a test asks otherwise
+    tm.tm_set_path(ctx, 0)
+    tm.tm_set_tuning(ctx, "stage_links", -1)
+    tm.tm_set_tuning(ctx, "block_threads", 0)
+    tm.tm_set_tuning(ctx, "prefetch_blocks", 0)
     return _cache[key]
 
 
@@ -77,11 +91,13 @@ def test_t1_spinor_pack_unpack_round_trip(dims, nf):
 
 @pytest.mark.parametrize("dims,kind", [((4, 4, 4, 8), "haar"), ((4, 6, 8, 10), "near_identity"), ((8, 4, 6, 4), "haar")])
 @pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
-@pytest.mark.parametrize("path", [0, 1], ids=["default-kernels", "scalar-kernels"])
-def test_t2_every_kernel_variant_matches_oracle(dims, kind, kw, path):
+@pytest.mark.parametrize("variant", VARIANTS, ids=[v[0] for v in VARIANTS])
+def test_t2_every_kernel_variant_matches_oracle(dims, kind, kw, variant):
     nf = nf_of(kw)
     bench = bench_for(dims, kind, 1)
-    tm.tm_set_path(bench.lat.ctx, path)
+    tm.tm_set_path(bench.lat.ctx, variant[1])
+    for key, val in variant[2].items():
+        tm.tm_set_tuning(bench.lat.ctx, key, val)
     po = oracle.params(dims, KAPPA, **kw)
     pg = tm.params(KAPPA, **kw)
     full_in, full_x = si.spinor_field(dims, nf, 2), si.spinor_field(dims, nf, 3)
