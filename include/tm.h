@@ -138,8 +138,8 @@ int tm_timing_read(tm_ctx *ctx, int max_records, const char **names, float *ms, 
 /* Force a code path: 0 = automatic (default), 1 = generic direct-load kernels only.  For tests / profiling. */
 int tm_set_path(tm_ctx *ctx, int path);
 /* Performance knobs (never change results).  key is a HOST C string:
- *   "prefetch_blocks": L2 prefetch distance of the dslash kernels in thread blocks, 0 = off (default: chosen by
- *   the library per lattice);
+ *   "prefetch_blocks": L2 prefetch distance of the dslash kernels in thread blocks, 0 = off, -1 = library
+ *   default (chosen per precision and flavor count);
  *   "stage_links": 1 = the 8 links of a site are copied to shared memory with cp.async before the hops, 0 = direct
  *   loads, -1 = library default;   "block_threads": 32 / 64 / 128 sites per thread block, 0 = library default.
  *   Unknown key or bad value -> TM_ERR_ARG. */

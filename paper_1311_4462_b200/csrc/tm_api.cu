@@ -143,7 +143,7 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->launches = 0;
     c->last_kernel = "";
     c->path = 0;
-    c->pf_dist = 0;
+    c->pf_dist = -1;
     c->stage = -1;
     c->block_threads = 0;
     c->sm_count = 0;
@@ -223,7 +223,7 @@ int tm_set_tuning(tm_ctx *ctx, const char *key, int value)
 {
     if (!ctx || !key) return fail(TM_ERR_ARG, "tm_set_tuning: NULL argument");
     if (!strcmp(key, "prefetch_blocks")) {
-        if (value < 0) return fail(TM_ERR_ARG, "prefetch_blocks must be >= 0");
+        if (value < -1) return fail(TM_ERR_ARG, "prefetch_blocks must be -1 (default) or >= 0");
         ctx->pf_dist = value;
         return TM_OK;
     }
@@ -381,9 +381,11 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.alpha = co.alpha; a.beta = co.beta; a.scale = co.scale;
     a.kappa = p->kappa; a.kappa2 = p->kappa * p->kappa;
     a.tbound = (double)p->t_boundary;
-    a.pf_dist = c->pf_dist;
+    // measured defaults (profiles/): the fp32 doublet kernels gain from an L2 prefetch 8 tiles ahead, the half
+    // doublet kernels from staging the link stream through shared memory; everything else runs plain
+    a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_SINGLE && out->nf == 2 ? 8 : 0);
     // launch shape: library defaults unless overridden through tm_set_tuning
-    int stage = c->stage >= 0 ? c->stage : 0;
+    int stage = c->stage >= 0 ? c->stage : ((int)prec == TM_HALF && out->nf == 2 ? 1 : 0);
     a.block_threads = c->block_threads ? c->block_threads : 128;
     while (stage && (size_t)8 * g->recon * (int)prec * a.block_threads > 96 * 1024 && a.block_threads > 32) a.block_threads /= 2;
 

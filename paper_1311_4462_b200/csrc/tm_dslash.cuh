@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? 3 : (PRE
     typedef typename PrecTraits<PREC>::real real;
     constexpr int NCH = PrecTraits<PREC>::NCH;
     const int Vh = a.Vh;
-    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x);
+    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, blockIdx.x);
     const int site = blockIdx.x * blockDim.x + threadIdx.x;        // one thread per output site, all flavors
     if (site >= Vh) return;
 

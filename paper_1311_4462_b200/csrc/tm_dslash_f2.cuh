@@ -22,65 +22,163 @@
 
 #define TM_INV15 (1.0f / 32767.0f)
 
-// ---- loads ------------------------------------------------------------------------------------------
-// PART: 0 all, 1 upper only (S[0..5]), 2 lower only (S[6..11]).  fp32: values; half: RAW integers (scale deferred).
-template <int PREC, int PART>
-TM_DEV void load_spinor_f2(f2 *S, const char *base, int Vh, int idx)
+// Software-pipeline depth (hops of loads in flight ahead of the arithmetic) per (precision, flavors); chosen by
+// measurement on B200 (profiles/), overridable at compile time for sweeps.
+#ifndef TM_PD_4_1
+#define TM_PD_4_1 1
+#endif
+#ifndef TM_PD_4_2
+#define TM_PD_4_2 1
+#endif
+#ifndef TM_PD_2_1
+#define TM_PD_2_1 0
+#endif
+#ifndef TM_PD_2_2
+#define TM_PD_2_2 2
+#endif
+// Resident blocks of 128 threads per SM the register allocation aims at (second __launch_bounds__ argument).  It is
+// what makes ptxas keep the pipelined loads early: without it the loads are sunk back next to their first use.
+#ifndef TM_MINB_4_1
+#define TM_MINB_4_1 4
+#endif
+#ifndef TM_MINB_4_2
+#define TM_MINB_4_2 3
+#endif
+#ifndef TM_MINB_2_1
+#define TM_MINB_2_1 5
+#endif
+#ifndef TM_MINB_2_2
+#define TM_MINB_2_2 4
+#endif
+template <int PREC, int NF> __host__ __device__ constexpr int f2_min_blocks()
+{
+    return PREC == 4 ? (NF == 1 ? TM_MINB_4_1 : TM_MINB_4_2) : (NF == 1 ? TM_MINB_2_1 : TM_MINB_2_2);
+}
+template <int PREC, int NF> __host__ __device__ constexpr int f2_pipeline_depth()
+{
+    return PREC == 4 ? (NF == 1 ? TM_PD_4_1 : TM_PD_4_2) : (NF == 1 ? TM_PD_2_1 : TM_PD_2_2);
+}
+
+// ---- loads: issue and use are separate (software pipelining) ------------------------------
+// The raw 128-bit words of one hop (link + the neighbour spinor of every flavor + norms) are loaded into a HopRaw
+// by issue_*; the arithmetic of that hop reads them PD hops later (consume_hop), so PD + 1 hops of loads are in
+// flight per thread while the previous hops are being computed.  Nothing is converted at issue time: in half a hop
+// in flight costs 19 registers per flavor-site, in fp32 36 + 24 NF.
+template <int PREC, int NF, int RECON>
+struct HopRaw {
+    static constexpr int NL = (PREC == 4) ? (RECON == 18 ? 4 : 3) : (RECON == 18 ? 2 : 1);   // 128-bit link words
+    static constexpr int NS = (PREC == 4) ? 6 : 3;                                          // 128-bit spinor words
+    uint4 l[NL];
+    uint2 lt;            // link tail: fp32/18 float2, half/12 int2, half/18 int (.x)
+    uint4 s[NF][NS];
+    float n[NF];         // half: site norms
+};
+
+// Global loads are volatile asm so that the compiler keeps them where the pipeline puts them (it otherwise sinks
+// them back next to their first use to save registers, which serialises load latency and arithmetic hop by hop).
+TM_DEV uint4 ldg_nc_u4(const void *p)
+{
+    uint4 v;
+    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
+TM_DEV uint2 ldg_nc_u2(const void *p)
+{
+    uint2 v;
+    asm volatile("ld.global.nc.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+    return v;
+}
+TM_DEV unsigned ldg_nc_u1(const void *p)
+{
+    unsigned v;
+    asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+template <bool SM> TM_DEV uint4 ld_u4(const void *p) { if constexpr (SM) return *reinterpret_cast<const uint4 *>(p); else return ldg_nc_u4(p); }
+template <bool SM> TM_DEV uint2 ld_u2(const void *p) { if constexpr (SM) return *reinterpret_cast<const uint2 *>(p); else return ldg_nc_u2(p); }
+template <bool SM> TM_DEV unsigned ld_u1(const void *p) { if constexpr (SM) return *reinterpret_cast<const unsigned *>(p); else return ldg_nc_u1(p); }
+
+// a4 (fetch): the stored words of one link, from its [parity][mu] block or from the staged shared-memory slots
+template <int PREC, int NF, int RECON, bool SM>
+TM_DEV void issue_link(HopRaw<PREC, NF, RECON> &r, const char *base, int Vh, int idx)
 {
     if constexpr (PREC == 4) {
-        constexpr int lo = (PART == 2) ? 3 : 0, hi = (PART == 1) ? 3 : 6;
-        const float4 *p = reinterpret_cast<const float4 *>(base) + idx;
 #pragma unroll
-        for (int k = lo; k < hi; k++) {
-            const float4 c = __ldg(p + (size_t)k * Vh);
-            S[2 * k] = mk2(c.x, c.y);
-            S[2 * k + 1] = mk2(c.z, c.w);
-        }
+        for (int k = 0; k < HopRaw<PREC, NF, RECON>::NL; k++) r.l[k] = ld_u4<SM>(base + ((size_t)k * Vh + idx) * 16);
+        if constexpr (RECON == 18) r.lt = ld_u2<SM>(base + (size_t)4 * Vh * 16 + (size_t)idx * 8);
     } else {
-        const int4 *p = reinterpret_cast<const int4 *>(base) + idx;
-        if constexpr (PART != 2) {
-            const int4 c = __ldg(p);
-            S[0] = cvt_pair(c.x); S[1] = cvt_pair(c.y); S[2] = cvt_pair(c.z); S[3] = cvt_pair(c.w);
-        }
-        {
-            const int4 c = __ldg(p + (size_t)Vh);
-            if constexpr (PART != 2) { S[4] = cvt_pair(c.x); S[5] = cvt_pair(c.y); }
-            if constexpr (PART != 1) { S[6] = cvt_pair(c.z); S[7] = cvt_pair(c.w); }
-        }
-        if constexpr (PART != 1) {
-            const int4 c = __ldg(p + (size_t)2 * Vh);
-            S[8] = cvt_pair(c.x); S[9] = cvt_pair(c.y); S[10] = cvt_pair(c.z); S[11] = cvt_pair(c.w);
+        r.l[0] = ld_u4<SM>(base + (size_t)idx * 16);
+        if constexpr (RECON == 18) {
+            r.l[1] = ld_u4<SM>(base + ((size_t)Vh + idx) * 16);
+            r.lt.x = ld_u1<SM>(base + (size_t)2 * Vh * 16 + (size_t)idx * 4);
+        } else {
+            r.lt = ld_u2<SM>(base + (size_t)Vh * 16 + (size_t)idx * 8);
         }
     }
 }
 
-// Link as 9 (re, im) pairs W[row*3+col]; half: RAW integers for rows 0,1 (12-real: row 2 rebuilt and rescaled to
-// the same raw scale).  a4 of DESIGN.md.
-template <int PREC, int RECON, bool SM>
-TM_DEV void load_link_f2(f2 *W, const char *base, int Vh, int idx)
+// PART: 0 all, 1 upper half only, 2 lower half only (time hops, a3).  `base` = chunk block of flavor 0.
+template <int PREC, int NF, int RECON, int PART>
+TM_DEV void issue_spinor(HopRaw<PREC, NF, RECON> &r, const char *base, const float *norm, size_t fl_bytes, int Vh, int idx)
+{
+#pragma unroll
+    for (int f = 0; f < NF; f++) {
+        const char *p = base + f * fl_bytes + (size_t)idx * 16;
+        if constexpr (PREC == 4) {
+            constexpr int lo = (PART == 2) ? 3 : 0, hi = (PART == 1) ? 3 : 6;
+#pragma unroll
+            for (int k = lo; k < hi; k++) r.s[f][k] = ld_u4<false>(p + (size_t)k * Vh * 16);
+        } else {
+            if constexpr (PART != 2) r.s[f][0] = ld_u4<false>(p);
+            r.s[f][1] = ld_u4<false>(p + (size_t)Vh * 16);
+            if constexpr (PART != 1) r.s[f][2] = ld_u4<false>(p + (size_t)2 * Vh * 16);
+            r.n[f] = __uint_as_float(ldg_nc_u1(norm + (size_t)f * Vh + idx));
+        }
+    }
+}
+
+// raw words -> pairs.  fp32: values; half: RAW integers as floats (scale deferred).  Only the PART's pairs are valid.
+template <int PREC, int PART>
+TM_DEV void raw_to_spinor(f2 *S, const uint4 *s)
 {
     if constexpr (PREC == 4) {
-        constexpr int NF4 = (RECON == 18) ? 4 : 3;
+        constexpr int lo = (PART == 2) ? 3 : 0, hi = (PART == 1) ? 3 : 6;
 #pragma unroll
-        for (int k = 0; k < NF4; k++) {
-            const float4 c = ld_f4<SM>(base + ((size_t)k * Vh + idx) * 16);
-            W[2 * k] = mk2(c.x, c.y);
-            W[2 * k + 1] = mk2(c.z, c.w);
-        }
-        if constexpr (RECON == 18) {
-            const float2 c = ld_f2<SM>(base + (size_t)4 * Vh * 16 + (size_t)idx * 8);
-            W[8] = mk2(c.x, c.y);
+        for (int k = lo; k < hi; k++) {
+            S[2 * k] = mk2(__uint_as_float(s[k].x), __uint_as_float(s[k].y));
+            S[2 * k + 1] = mk2(__uint_as_float(s[k].z), __uint_as_float(s[k].w));
         }
     } else {
-        const int4 c = ld_i4<SM>(base + (size_t)idx * 16);
-        W[0] = cvt_pair(c.x); W[1] = cvt_pair(c.y); W[2] = cvt_pair(c.z); W[3] = cvt_pair(c.w);
+        if constexpr (PART != 2) {
+            S[0] = cvt_pair(s[0].x); S[1] = cvt_pair(s[0].y); S[2] = cvt_pair(s[0].z); S[3] = cvt_pair(s[0].w);
+            S[4] = cvt_pair(s[1].x); S[5] = cvt_pair(s[1].y);
+        }
+        if constexpr (PART != 1) {
+            S[6] = cvt_pair(s[1].z); S[7] = cvt_pair(s[1].w);
+            S[8] = cvt_pair(s[2].x); S[9] = cvt_pair(s[2].y); S[10] = cvt_pair(s[2].z); S[11] = cvt_pair(s[2].w);
+        }
+    }
+}
+
+// a4 (rebuild): link as 9 (re, im) pairs W[row*3+col]; half: RAW integers for rows 0,1 (12-real: row 2 rebuilt and
+// rescaled to the same raw scale).
+template <int PREC, int NF, int RECON>
+TM_DEV void raw_to_link(f2 *W, const HopRaw<PREC, NF, RECON> &r)
+{
+    if constexpr (PREC == 4) {
+#pragma unroll
+        for (int k = 0; k < HopRaw<PREC, NF, RECON>::NL; k++) {
+            W[2 * k] = mk2(__uint_as_float(r.l[k].x), __uint_as_float(r.l[k].y));
+            W[2 * k + 1] = mk2(__uint_as_float(r.l[k].z), __uint_as_float(r.l[k].w));
+        }
+        if constexpr (RECON == 18) W[8] = mk2(__uint_as_float(r.lt.x), __uint_as_float(r.lt.y));
+    } else {
+        W[0] = cvt_pair(r.l[0].x); W[1] = cvt_pair(r.l[0].y); W[2] = cvt_pair(r.l[0].z); W[3] = cvt_pair(r.l[0].w);
         if constexpr (RECON == 18) {
-            const int4 d = ld_i4<SM>(base + ((size_t)Vh + idx) * 16);
-            W[4] = cvt_pair(d.x); W[5] = cvt_pair(d.y); W[6] = cvt_pair(d.z); W[7] = cvt_pair(d.w);
-            W[8] = cvt_pair(ld_i1<SM>(base + (size_t)2 * Vh * 16 + (size_t)idx * 4));
+            W[4] = cvt_pair(r.l[1].x); W[5] = cvt_pair(r.l[1].y); W[6] = cvt_pair(r.l[1].z); W[7] = cvt_pair(r.l[1].w);
+            W[8] = cvt_pair(r.lt.x);
         } else {
-            const int2 d = ld_i2<SM>(base + (size_t)Vh * 16 + (size_t)idx * 8);
-            W[4] = cvt_pair(d.x); W[5] = cvt_pair(d.y);
+            W[4] = cvt_pair(r.lt.x); W[5] = cvt_pair(r.lt.y);
         }
     }
     if constexpr (RECON == 12) {
@@ -181,29 +279,91 @@ TM_DEV void reconstruct_f2(f2 *A, const f2 *G, float w)
     }
 }
 
-// a6: the link is fetched, converted and rebuilt once and applied to every flavor.
-template <int PREC, int NF, int RECON, int MU, bool FWD, bool DAG, bool STG, int WAITN>
-TM_DEV void hop_f2(f2 *A, const char *in, const float *in_norm, size_t fl_bytes, const LinkSrc L, int Vh, int nbr, float w)
+// Where the fields are: the same for every site of a launch (kept in uniform registers).
+struct HopPtrs {
+    const char *in;          // input spinor, flavor 0 chunk block
+    const float *in_norm;
+    const char *x;           // xpay input (own parity)
+    const float *x_norm;
+    const char *gf, *gb;     // gauge blocks of the output parity (forward links) / the other parity (backward links)
+    size_t fl_bytes, blk;
+    int Vh;
+};
+// a2: one output site: its checkerboard index, the 8 neighbour indices (periodic wrap) and the time-hop weights.
+struct HopCtx {
+    int site;
+    int nbr[8];              // +x -x +y -y +z -z +t -t
+    float wt[2];             // weight of the +t / -t hop (2 x boundary sign)
+};
+
+TM_DEV void site_ctx(HopCtx &c, const DslashArgs &a, int site)
 {
+    const int Xh = a.Xh;
+    const int xh = site % Xh;
+    int r = site / Xh;
+    const int y = r % a.Y;
+    r /= a.Y;
+    const int z = r % a.Z;
+    const int t = r / a.Z;
+    const int q = (y + z + t + a.parity) & 1;       // x1 = 2 xh + q
+    const int sy = Xh, sz = Xh * a.Y, st = Xh * a.Y * a.Z;
+    c.site = site;
+    c.nbr[0] = q ? ((xh + 1 == Xh) ? site - (Xh - 1) : site + 1) : site;
+    c.nbr[1] = q ? site : ((xh == 0) ? site + (Xh - 1) : site - 1);
+    c.nbr[2] = (y == a.Y - 1) ? site - (a.Y - 1) * sy : site + sy;
+    c.nbr[3] = (y == 0) ? site + (a.Y - 1) * sy : site - sy;
+    c.nbr[4] = (z == a.Z - 1) ? site - (a.Z - 1) * sz : site + sz;
+    c.nbr[5] = (z == 0) ? site + (a.Z - 1) * sz : site - sz;
+    c.nbr[6] = (t == a.T - 1) ? site - (a.T - 1) * st : site + st;
+    c.nbr[7] = (t == 0) ? site + (a.T - 1) * st : site - st;
+    c.wt[0] = 2.f * ((t == a.T - 1) ? (float)a.tbound : 1.f);
+    c.wt[1] = 2.f * ((t == 0) ? (float)a.tbound : 1.f);
+}
+
+// Pipeline slot H of a site: 0..7 = the hops in the order of HopCtx::nbr, 8 = the xpay input of the site, > 8 nothing.
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, int H>
+TM_DEV void issue_slot(HopRaw<PREC, NF, RECON> &r, const HopPtrs &p, const HopCtx &c)
+{
+    if constexpr (H < 8) {
+        constexpr int MU = H / 2;
+        constexpr bool FWD = (H % 2) == 0;
+        constexpr int SGN = (FWD != DAG) ? +1 : -1;
+        constexpr int PART = (MU == 3) ? ((SGN > 0) ? 2 : 1) : 0;
+        if constexpr (!STG) issue_link<PREC, NF, RECON, false>(r, (FWD ? p.gf : p.gb) + MU * p.blk, p.Vh, FWD ? c.site : c.nbr[H]);
+        issue_spinor<PREC, NF, RECON, PART>(r, p.in, p.in_norm, p.fl_bytes, p.Vh, c.nbr[H]);
+    } else if constexpr (H == 8 && KT != 0) {
+        issue_spinor<PREC, NF, RECON, 0>(r, p.x, p.x_norm, p.fl_bytes, p.Vh, c.site);
+    }
+}
+
+// a6: the link is converted and rebuilt once and applied to every flavor.
+template <int PREC, int NF, int RECON, bool DAG, bool STG, int H>
+TM_DEV void consume_hop(f2 *A, HopRaw<PREC, NF, RECON> &r, const HopCtx &c)
+{
+    constexpr int MU = H / 2;
+    constexpr bool FWD = (H % 2) == 0;
     constexpr int SGN = (FWD != DAG) ? +1 : -1;
+    constexpr int PART = (MU == 3) ? ((SGN > 0) ? 2 : 1) : 0;
+    if constexpr (STG) {
+        cp_async_wait<7 - H>();
+        issue_link<PREC, NF, RECON, true>(r, tm_smem + (size_t)H * (RECON * PREC) * blockDim.x, blockDim.x, threadIdx.x);
+    }
     f2 W[9];
-    if constexpr (STG) cp_async_wait<WAITN>();
-    load_link_f2<PREC, RECON, STG>(W, L.base, L.stride, L.idx);
+    raw_to_link<PREC, NF, RECON>(W, r);
+    const float w = (MU == 3) ? c.wt[H & 1] : 1.f;
 #pragma unroll
     for (int f = 0; f < NF; f++) {
-        f2 S[12], H[6], G[6];
-        const char *inf = in + f * fl_bytes;
+        f2 S[12], H6[6], G[6];
+        raw_to_spinor<PREC, PART>(S, r.s[f]);
         if constexpr (MU == 3) {
-            load_spinor_f2<PREC, (SGN > 0) ? 2 : 1>(S, inf, Vh, nbr);
 #pragma unroll
-            for (int i = 0; i < 6; i++) H[i] = (SGN > 0) ? S[6 + i] : S[i];
+            for (int i = 0; i < 6; i++) H6[i] = (SGN > 0) ? S[6 + i] : S[i];
         } else {
-            load_spinor_f2<PREC, 0>(S, inf, Vh, nbr);
-            project_f2<MU, SGN>(H, S);
+            project_f2<MU, SGN>(H6, S);
         }
         float wf = w;
-        if constexpr (PREC == 2) wf *= __ldg(in_norm + (size_t)f * Vh + nbr) * (TM_INV15 * TM_INV15);   // site norm x link scale
-        su3_mul_f2<!FWD>(G, W, H);
+        if constexpr (PREC == 2) wf *= r.n[f] * (TM_INV15 * TM_INV15);   // site norm x link scale
+        su3_mul_f2<!FWD>(G, W, H6);
         reconstruct_f2<MU, SGN>(A + 12 * f, G, wf);
     }
 }
@@ -276,89 +436,80 @@ TM_DEV void store_spinor_f2(const f2 *A, char *base, float *norm, int Vh, int id
     }
 }
 
+// slot 8: the xpay input of the site, from raw words to values
+template <int PREC, int NF, int RECON>
+TM_DEV void load_x(f2 *X, const HopRaw<PREC, NF, RECON> &rx)
+{
+#pragma unroll
+    for (int f = 0; f < NF; f++) {
+        raw_to_spinor<PREC, 0>(X + 12 * f, rx.s[f]);
+        if constexpr (PREC == 2) {
+            const float s = rx.n[f] * TM_INV15;
+#pragma unroll
+            for (int i = 0; i < 12; i++) X[12 * f + i] = mul2(X[12 * f + i], bc2(s));
+        }
+    }
+}
+
+// One thread per output site, all flavors.  The 8 hops and the xpay input are 9 pipeline slots; slot h + PD is
+// issued before hop h is computed (PD = f2_pipeline_depth, PD + 1 rotating raw buffers).
 template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
-__global__ void __launch_bounds__(128) tm_dslash_f2(const DslashArgs a)
+__global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(const DslashArgs a)
 {
     constexpr int NCH = PrecTraits<PREC>::NCH;
+    constexpr int PD = f2_pipeline_depth<PREC, NF>();
     const int Vh = a.Vh;
-    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x);
-    const int site = blockIdx.x * blockDim.x + threadIdx.x;        // one thread per output site, all flavors
+    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, blockIdx.x);
+    const int site = blockIdx.x * blockDim.x + threadIdx.x;
     if (site >= Vh) return;
 
-    // a2: site decode and neighbours
-    const int Xh = a.Xh;
-    const int xh = site % Xh;
-    int r = site / Xh;
-    const int y = r % a.Y;
-    r /= a.Y;
-    const int z = r % a.Z;
-    const int t = r / a.Z;
-    const int q = (y + z + t + a.parity) & 1;
-    const int sy = Xh, sz = Xh * a.Y, st = Xh * a.Y * a.Z;
-    const int xp = q ? ((xh + 1 == Xh) ? site - (Xh - 1) : site + 1) : site;
-    const int xm = q ? site : ((xh == 0) ? site + (Xh - 1) : site - 1);
-    const int yp = (y == a.Y - 1) ? site - (a.Y - 1) * sy : site + sy;
-    const int ym = (y == 0) ? site + (a.Y - 1) * sy : site - sy;
-    const int zp = (z == a.Z - 1) ? site - (a.Z - 1) * sz : site + sz;
-    const int zm = (z == 0) ? site + (a.Z - 1) * sz : site - sz;
-    const int tp = (t == a.T - 1) ? site - (a.T - 1) * st : site + st;
-    const int tm = (t == 0) ? site + (a.T - 1) * st : site - st;
-    const float wtp = 2.f * ((t == a.T - 1) ? (float)a.tbound : 1.f);
-    const float wtm = 2.f * ((t == 0) ? (float)a.tbound : 1.f);
+    HopPtrs p;
+    p.fl_bytes = (size_t)NCH * Vh * 16;
+    p.in = static_cast<const char *>(a.in);
+    p.in_norm = reinterpret_cast<const float *>(p.in + NF * p.fl_bytes);
+    p.x = static_cast<const char *>(a.x);
+    p.x_norm = reinterpret_cast<const float *>(p.x + NF * p.fl_bytes);
+    p.blk = (size_t)RECON * PREC * Vh;
+    p.gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * 4 * p.blk;
+    p.gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * 4 * p.blk;
+    p.Vh = Vh;
 
-    const size_t fl_bytes = (size_t)NCH * Vh * 16;
-    const char *in = static_cast<const char *>(a.in);
-    const float *in_norm = reinterpret_cast<const float *>(in + NF * fl_bytes);
-    const size_t blk = (size_t)RECON * PREC * Vh;
-    const char *gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * 4 * blk;
-    const char *gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * 4 * blk;
-
-    const int nt = blockDim.x, tid = threadIdx.x;
-    constexpr int LB = RECON * PREC;
+    HopCtx c;
+    site_ctx(c, a, site);
     if constexpr (STG) {
-        stage_link<PREC, RECON>(tm_smem + 0 * LB * nt, gf + 0 * blk, Vh, site, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 1 * LB * nt, gb + 0 * blk, Vh, xm, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 2 * LB * nt, gf + 1 * blk, Vh, site, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 3 * LB * nt, gb + 1 * blk, Vh, ym, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 4 * LB * nt, gf + 2 * blk, Vh, site, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 5 * LB * nt, gb + 2 * blk, Vh, zm, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 6 * LB * nt, gf + 3 * blk, Vh, site, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 7 * LB * nt, gb + 3 * blk, Vh, tm, nt, tid);
+        constexpr int LB = RECON * PREC;
+#pragma unroll
+        for (int h = 0; h < 8; h++)
+            stage_link<PREC, RECON>(tm_smem + h * LB * blockDim.x, ((h & 1) ? p.gb : p.gf) + (h >> 1) * p.blk, Vh,
+                                    (h & 1) ? c.nbr[h] : site, blockDim.x, threadIdx.x);
     }
 
-    f2 A[NF * 12];
+    f2 A[NF * 12], X[NF * 12];
 #pragma unroll
     for (int i = 0; i < NF * 12; i++) A[i] = mk2(0.f, 0.f);
 
-    hop_f2<PREC, NF, RECON, 0, true, DAG, STG, 7>(A, in, in_norm, fl_bytes, link_src<STG>(0, LB, gf + 0 * blk, Vh, site), Vh, xp, 1.f);
-    hop_f2<PREC, NF, RECON, 0, false, DAG, STG, 6>(A, in, in_norm, fl_bytes, link_src<STG>(1, LB, gb + 0 * blk, Vh, xm), Vh, xm, 1.f);
-    hop_f2<PREC, NF, RECON, 1, true, DAG, STG, 5>(A, in, in_norm, fl_bytes, link_src<STG>(2, LB, gf + 1 * blk, Vh, site), Vh, yp, 1.f);
-    hop_f2<PREC, NF, RECON, 1, false, DAG, STG, 4>(A, in, in_norm, fl_bytes, link_src<STG>(3, LB, gb + 1 * blk, Vh, ym), Vh, ym, 1.f);
-    hop_f2<PREC, NF, RECON, 2, true, DAG, STG, 3>(A, in, in_norm, fl_bytes, link_src<STG>(4, LB, gf + 2 * blk, Vh, site), Vh, zp, 1.f);
-    hop_f2<PREC, NF, RECON, 2, false, DAG, STG, 2>(A, in, in_norm, fl_bytes, link_src<STG>(5, LB, gb + 2 * blk, Vh, zm), Vh, zm, 1.f);
-    hop_f2<PREC, NF, RECON, 3, true, DAG, STG, 1>(A, in, in_norm, fl_bytes, link_src<STG>(6, LB, gf + 3 * blk, Vh, site), Vh, tp, wtp);
-    hop_f2<PREC, NF, RECON, 3, false, DAG, STG, 0>(A, in, in_norm, fl_bytes, link_src<STG>(7, LB, gb + 3 * blk, Vh, tm), Vh, tm, wtm);
+    HopRaw<PREC, NF, RECON> buf[PD + 1];
+#define TM_ISSUE(S) issue_slot<PREC, NF, RECON, KT, DAG, STG, (S)>(buf[(S) % (PD + 1)], p, c)
+#define TM_STEP(H)                                                                  \
+    do {                                                                            \
+        TM_ISSUE((H) + PD);                                                         \
+        consume_hop<PREC, NF, RECON, DAG, STG, (H)>(A, buf[(H) % (PD + 1)], c);     \
+    } while (0)
+    if constexpr (PD >= 1) TM_ISSUE(0);
+    if constexpr (PD >= 2) TM_ISSUE(1);
+    if constexpr (PD >= 3) TM_ISSUE(2);
+    TM_STEP(0); TM_STEP(1); TM_STEP(2); TM_STEP(3); TM_STEP(4); TM_STEP(5); TM_STEP(6); TM_STEP(7);
+    if constexpr (PD == 0) TM_ISSUE(8);
+#undef TM_STEP
+#undef TM_ISSUE
+    if constexpr (KT != 0) load_x<PREC, NF, RECON>(X, buf[8 % (PD + 1)]);
 
-    f2 X[NF * 12];
-    if constexpr (KT != 0) {
-        const char *xb = static_cast<const char *>(a.x);
-        const float *xn = reinterpret_cast<const float *>(xb + NF * fl_bytes);
-#pragma unroll
-        for (int f = 0; f < NF; f++) {
-            load_spinor_f2<PREC, 0>(X + 12 * f, xb + f * fl_bytes, Vh, site);
-            if constexpr (PREC == 2) {
-                const float s = __ldg(xn + (size_t)f * Vh + site) * TM_INV15;
-#pragma unroll
-                for (int i = 0; i < 12; i++) X[12 * f + i] = mul2(X[12 * f + i], bc2(s));
-            }
-        }
-    }
     epilogue_f2<NF, KT>(A, X, (float)a.alpha, (float)a.beta, (float)a.scale, (float)a.kappa, (float)a.kappa2);
 
     char *ob = static_cast<char *>(a.out);
-    float *on = reinterpret_cast<float *>(ob + NF * fl_bytes);
+    float *on = reinterpret_cast<float *>(ob + NF * p.fl_bytes);
 #pragma unroll
-    for (int f = 0; f < NF; f++) store_spinor_f2<PREC>(A + 12 * f, ob + f * fl_bytes, on + (size_t)f * Vh, Vh, site);
+    for (int f = 0; f < NF; f++) store_spinor_f2<PREC>(A + 12 * f, ob + f * p.fl_bytes, on + (size_t)f * Vh, Vh, site);
 }
 
 template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
@@ -386,9 +537,19 @@ cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
     {tm_launch_f2<P, N, R, K, false, true>, "f2_staged<" #P "," #N "," #R "," #K ",plain>"},       \
     {tm_launch_f2<P, N, R, K, true, false>, "f2<" #P "," #N "," #R "," #K ",dagger>"},             \
     {tm_launch_f2<P, N, R, K, true, true>, "f2_staged<" #P "," #N "," #R "," #K ",dagger>"}
+#ifdef TM_F2_SWEEP   /* working builds: only recon 12, kernel types A and B, plain */
+#define TM_F2_NONE {nullptr, "absent"}
+#define TM_F2_ROW0 TM_F2_NONE, TM_F2_NONE, TM_F2_NONE, TM_F2_NONE
+#define TM_F2_ROWS(P, N, R, K) {tm_launch_f2<P, N, R, K, false, false>, "f2<" #P "," #N "," #R "," #K ",plain>"}, {tm_launch_f2<P, N, R, K, false, true>, "f2_staged<" #P "," #N "," #R "," #K ",plain>"}, TM_F2_NONE, TM_F2_NONE
+#define TM_F2_TABLE(P, N)                                                                    \
+    static const TmKernelEntry f2table_##P##_##N[32] = {                                    \
+        TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROWS(P, N, 12, 0), TM_F2_ROW0, TM_F2_ROWS(P, N, 12, 2), TM_F2_ROW0}; \
+    const TmKernelEntry *tm_f2_table_##P##_##N() { return f2table_##P##_##N; }
+#else
 #define TM_F2_TABLE(P, N)                                                                    \
     static const TmKernelEntry f2table_##P##_##N[32] = {                                    \
         TM_F2_ROW(P, N, 18, 0), TM_F2_ROW(P, N, 18, 1), TM_F2_ROW(P, N, 18, 2),             \
         TM_F2_ROW(P, N, 18, 3), TM_F2_ROW(P, N, 12, 0), TM_F2_ROW(P, N, 12, 1),             \
         TM_F2_ROW(P, N, 12, 2), TM_F2_ROW(P, N, 12, 3)};                                    \
     const TmKernelEntry *tm_f2_table_##P##_##N() { return f2table_##P##_##N; }
+#endif

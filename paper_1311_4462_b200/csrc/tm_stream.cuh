@@ -12,11 +12,11 @@
 #include "tm_layout.cuh"
 
 template <int PREC, int NF, int RECON, bool HAS_X>
-TM_DEV void prefetch_tile(const DslashArgs &a, int sites_per_block)
+TM_DEV void prefetch_tile(const DslashArgs &a, int sites_per_block, int vblock)
 {
     if (a.pf_dist <= 0) return;
     const int Vh = a.Vh;
-    const long first_l = (long)(blockIdx.x + a.pf_dist) * sites_per_block;
+    const long first_l = (long)(vblock + a.pf_dist) * sites_per_block;
     if (first_l >= Vh) return;
     const int first = (int)first_l;
     const int n = min(sites_per_block, Vh - first);
@@ -76,7 +76,7 @@ TM_DEV void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memor
 template <int N> TM_DEV void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <int PREC, int RECON>
-TM_DEV void stage_link(char *sm_hop, const char *gauge_blk, int Vh, int idx, int nt, int tid)
+TM_DEV void stage_link_nc(char *sm_hop, const char *gauge_blk, int Vh, int idx, int nt, int tid)     // no commit
 {
     constexpr int NP = link_planes<PREC, RECON>();
 #pragma unroll
@@ -88,6 +88,11 @@ TM_DEV void stage_link(char *sm_hop, const char *gauge_blk, int Vh, int idx, int
         else if (w == 8) cp_async<8>(dst, src);
         else cp_async<4>(dst, src);
     }
+}
+template <int PREC, int RECON>
+TM_DEV void stage_link(char *sm_hop, const char *gauge_blk, int Vh, int idx, int nt, int tid)
+{
+    stage_link_nc<PREC, RECON>(sm_hop, gauge_blk, Vh, idx, nt, tid);
     cp_async_commit();
 }
 

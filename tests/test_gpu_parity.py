@@ -51,7 +51,7 @@ def bench_for(dims, kind, seed):
     tm.tm_set_path(ctx, 0)
     tm.tm_set_tuning(ctx, "stage_links", -1)
     tm.tm_set_tuning(ctx, "block_threads", 0)
-    tm.tm_set_tuning(ctx, "prefetch_blocks", 0)
+    tm.tm_set_tuning(ctx, "prefetch_blocks", -1)
     return _cache[key]
 
 
