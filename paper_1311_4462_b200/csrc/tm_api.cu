@@ -8,6 +8,7 @@
 #include <new>
 
 #include "tm_internal.h"
+#include "tm_layout.cuh"
 
 const TmKernelEntry *tm_generic_table_8_1();
 const TmKernelEntry *tm_generic_table_8_2();
@@ -58,9 +59,7 @@ bool valid_prec(int p) { return p == TM_DOUBLE || p == TM_SINGLE || p == TM_HALF
 
 size_t field_bytes(const TmGeom &g, int prec, int nf)
 {
-    size_t b = (size_t)nf * g.Vh * tm_spinor_site_bytes(prec);
-    if (prec == TM_HALF) b += (size_t)nf * g.Vh * sizeof(float);
-    return b;
+    return (size_t)nf * tm_tiles(g.Vh) * spinor_tile_bytes(prec);      // tiled SoA, the last tile padded (tm_layout.cuh)
 }
 
 bool overlap(const tm_field *a, const tm_field *b)
@@ -335,7 +334,7 @@ int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_r
     tm_gauge *gg = new (std::nothrow) tm_gauge();
     if (!gg) return fail(TM_ERR_NOMEM, "out of host memory");
     gg->ctx = ctx; gg->prec = prec; gg->recon = recon;
-    gg->bytes = (size_t)8 * ctx->g.Vh * tm_link_site_bytes(prec, recon);
+    gg->bytes = (size_t)2 * tm_tiles(ctx->g.Vh) * 4 * link_tile_bytes(prec, recon);
     cudaError_t e = cudaMalloc(&gg->ptr, gg->bytes);
     if (e != cudaSuccess) { delete gg; cudaGetLastError(); return fail(TM_ERR_NOMEM, "cudaMalloc(%zu): %s", gg->bytes, cudaGetErrorString(e)); }
     const size_t n = (size_t)4 * ctx->g.V * 18 * sizeof(double);
@@ -377,15 +376,15 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     DslashArgs a;
     a.out = out->ptr; a.in = in->ptr; a.x = x ? x->ptr : nullptr; a.gauge = g->ptr;
     a.X = c->g.X[0]; a.Y = c->g.X[1]; a.Z = c->g.X[2]; a.T = c->g.X[3]; a.Xh = c->g.Xh; a.Vh = c->g.Vh;
+    a.dXh = tm_fastdiv(a.Xh); a.dY = tm_fastdiv(a.Y); a.dZ = tm_fastdiv(a.Z);
     a.parity = (int)parity;
     a.alpha = co.alpha; a.beta = co.beta; a.scale = co.scale;
     a.kappa = p->kappa; a.kappa2 = p->kappa * p->kappa;
     a.tbound = (double)p->t_boundary;
-    // measured defaults (profiles/): the fp32 doublet kernels gain from an L2 prefetch 8 tiles ahead, the half
-    // doublet kernels from staging the link stream through shared memory; everything else runs plain
-    a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_SINGLE && out->nf == 2 ? 8 : 0);
-    // launch shape: library defaults unless overridden through tm_set_tuning
-    int stage = c->stage >= 0 ? c->stage : ((int)prec == TM_HALF && out->nf == 2 ? 1 : 0);
+    // measured defaults (profiles/): the fp64 doublet kernels gain from an L2 prefetch 8 tiles ahead, the half
+    // kernels from staging the link stream through shared memory; everything else runs plain
+    a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_DOUBLE && out->nf == 2 ? 8 : 0);
+    int stage = c->stage >= 0 ? c->stage : ((int)prec == TM_HALF ? 1 : 0);
     a.block_threads = c->block_threads ? c->block_threads : 128;
     while (stage && (size_t)8 * g->recon * (int)prec * a.block_threads > 96 * 1024 && a.block_threads > 32) a.block_threads /= 2;
 

@@ -106,28 +106,35 @@ TM_DEV void reconstruct_acc(real *acc, const real *g, real w)
 
 // one of the 8 hops.  FWD: U_mu(x) psi(x+mu) with (1 - sgn gamma_mu);  else U_mu(x-mu)^dag psi(x-mu), (1 + sgn gamma_mu).
 // a6: the link is fetched (and its third row rebuilt) once and applied to every flavor.
-// STG: the link was staged in shared memory (tm_stream.cuh): L addresses the block's [plane][thread] slots and
-// WAITN is the number of younger cp.async groups that may still be pending.
-template <int PREC, int NF, int RECON, int MU, bool FWD, bool DAG, bool STG, int WAITN>
-TM_DEV void hop(typename PrecTraits<PREC>::real *acc, const char *in, const float *in_norm, size_t fl_bytes,
-                const LinkSrc L, int Vh, int nbr, typename PrecTraits<PREC>::real w)
+// H = hop number (+x -x +y -y +z -z +t -t).  `lp` = site pointer of the link in global memory, `sp` = site pointer
+// of flavor 0 of the neighbour spinor, `lane` = neighbour index & 31.  STG: the link was staged in shared memory
+// (tm_stream.cuh) and 7 - H younger cp.async groups may still be pending.
+template <int PREC, int NF, int RECON, int H, bool DAG, bool STG>
+TM_DEV void hop(typename PrecTraits<PREC>::real *acc, const char *sp, int lane, const char *lp, int llane,
+                typename PrecTraits<PREC>::real w)
 {
     typedef typename PrecTraits<PREC>::real real;
+    constexpr int MU = H / 2;
+    constexpr bool FWD = (H % 2) == 0;
     constexpr int SGN = (FWD != DAG) ? +1 : -1;     // projector sign: forward carries (1 - gamma) unless daggered
     real u[18];
-    if constexpr (STG) cp_async_wait<WAITN>();
-    load_link<PREC, RECON, STG>(u, L.base, L.stride, L.idx);
+    if constexpr (STG) {
+        cp_async_wait<7 - H>();
+        load_link<PREC, RECON, true>(u, stage_slot<PREC, RECON>(H), threadIdx.x & 31);
+    } else {
+        load_link<PREC, RECON, false>(u, lp, llane);
+    }
 #pragma unroll
     for (int f = 0; f < NF; f++) {
         real h[12], g[12];
         if constexpr (MU == 3) {
             real v[24];
-            load_spinor<PREC, (SGN > 0) ? 2 : 1>(v, in + f * fl_bytes, in_norm + (size_t)f * Vh, Vh, nbr);
+            load_spinor<PREC, (SGN > 0) ? 2 : 1>(v, sp + f * spinor_tile_bytes(PREC), lane);
 #pragma unroll
             for (int i = 0; i < 12; i++) h[i] = (SGN > 0) ? v[12 + i] : v[i];
         } else {
             real v[24];
-            load_spinor<PREC, 0>(v, in + f * fl_bytes, in_norm + (size_t)f * Vh, Vh, nbr);
+            load_spinor<PREC, 0>(v, sp + f * spinor_tile_bytes(PREC), lane);
             project<MU, SGN>(h, v);
         }
         su3_mul<!FWD>(g, u, h);
@@ -179,7 +186,6 @@ template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
 __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? 3 : (PREC == 8 ? 2 : 1)) tm_dslash_generic(const DslashArgs a)
 {
     typedef typename PrecTraits<PREC>::real real;
-    constexpr int NCH = PrecTraits<PREC>::NCH;
     const int Vh = a.Vh;
     prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, blockIdx.x);
     const int site = blockIdx.x * blockDim.x + threadIdx.x;        // one thread per output site, all flavors
@@ -187,12 +193,12 @@ __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? 3 : (PRE
 
     // a2: site decode and neighbours
     const int Xh = a.Xh;
-    const int xh = site % Xh;
-    int r = site / Xh;
-    const int y = r % a.Y;
-    r /= a.Y;
-    const int z = r % a.Z;
-    const int t = r / a.Z;
+    int r = tm_div(site, a.dXh);
+    const int xh = site - r * Xh;
+    int r2 = tm_div(r, a.dY);
+    const int y = r - r2 * a.Y;
+    const int t = tm_div(r2, a.dZ);
+    const int z = r2 - t * a.Z;
     const int q = (y + z + t + a.parity) & 1;       // x1 = 2 xh + q
     const int sy = Xh, sz = Xh * a.Y, st = Xh * a.Y * a.Z;
     const int xp = q ? ((xh + 1 == Xh) ? site - (Xh - 1) : site + 1) : site;
@@ -206,54 +212,47 @@ __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? 3 : (PRE
     const real wtp = (real)2 * ((t == a.T - 1) ? (real)a.tbound : (real)1);
     const real wtm = (real)2 * ((t == 0) ? (real)a.tbound : (real)1);
 
-    const size_t fl_bytes = (size_t)NCH * Vh * 16;                      // one flavor's chunk block
+    const int nbr[8] = {xp, xm, yp, ym, zp, zm, tp, tm};
     const char *in = static_cast<const char *>(a.in);
-    const float *in_norm = reinterpret_cast<const float *>(in + NF * fl_bytes);
-    const size_t blk = (size_t)RECON * PREC * Vh;                       // one [parity][mu] block
-    const char *gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * 4 * blk;        // U_mu(x)
-    const char *gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * 4 * blk;  // U_mu(x - mu)
+    const size_t PB = (size_t)tm_tiles(Vh) * 4 * link_tile_bytes(PREC, RECON);              // one parity's gauge block
+    const char *gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * PB;            // U_mu(x)
+    const char *gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * PB;      // U_mu(x - mu)
+    const int lane = site & (TM_TILE - 1);
+    const char *lf = gf + link_site_off(PREC, RECON, site, 0);                              // + mu * link_tile_bytes
 
     // a4 (staged): start all 8 link copies now; hops consume them in order
-    const int nt = blockDim.x, tid = threadIdx.x;
-    constexpr int LB = RECON * PREC;                                    // bytes of one stored link
     if constexpr (STG) {
-        stage_link<PREC, RECON>(tm_smem + 0 * LB * nt, gf + 0 * blk, Vh, site, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 1 * LB * nt, gb + 0 * blk, Vh, xm, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 2 * LB * nt, gf + 1 * blk, Vh, site, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 3 * LB * nt, gb + 1 * blk, Vh, ym, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 4 * LB * nt, gf + 2 * blk, Vh, site, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 5 * LB * nt, gb + 2 * blk, Vh, zm, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 6 * LB * nt, gf + 3 * blk, Vh, site, nt, tid);
-        stage_link<PREC, RECON>(tm_smem + 7 * LB * nt, gb + 3 * blk, Vh, tm, nt, tid);
+#pragma unroll
+        for (int h = 0; h < 8; h++)
+            stage_link<PREC, RECON>(h, (h & 1) ? gb + link_site_off(PREC, RECON, nbr[h], h >> 1) : lf + (h >> 1) * link_tile_bytes(PREC, RECON),
+                                    ((h & 1) ? nbr[h] : site) & (TM_TILE - 1));
     }
     real acc[NF * 24];
 #pragma unroll
     for (int i = 0; i < NF * 24; i++) acc[i] = 0;
 
-    hop<PREC, NF, RECON, 0, true, DAG, STG, 7>(acc, in, in_norm, fl_bytes, link_src<STG>(0, LB, gf + 0 * blk, Vh, site), Vh, xp, (real)1);
-    hop<PREC, NF, RECON, 0, false, DAG, STG, 6>(acc, in, in_norm, fl_bytes, link_src<STG>(1, LB, gb + 0 * blk, Vh, xm), Vh, xm, (real)1);
-    hop<PREC, NF, RECON, 1, true, DAG, STG, 5>(acc, in, in_norm, fl_bytes, link_src<STG>(2, LB, gf + 1 * blk, Vh, site), Vh, yp, (real)1);
-    hop<PREC, NF, RECON, 1, false, DAG, STG, 4>(acc, in, in_norm, fl_bytes, link_src<STG>(3, LB, gb + 1 * blk, Vh, ym), Vh, ym, (real)1);
-    hop<PREC, NF, RECON, 2, true, DAG, STG, 3>(acc, in, in_norm, fl_bytes, link_src<STG>(4, LB, gf + 2 * blk, Vh, site), Vh, zp, (real)1);
-    hop<PREC, NF, RECON, 2, false, DAG, STG, 2>(acc, in, in_norm, fl_bytes, link_src<STG>(5, LB, gb + 2 * blk, Vh, zm), Vh, zm, (real)1);
-    hop<PREC, NF, RECON, 3, true, DAG, STG, 1>(acc, in, in_norm, fl_bytes, link_src<STG>(6, LB, gf + 3 * blk, Vh, site), Vh, tp, wtp);
-    hop<PREC, NF, RECON, 3, false, DAG, STG, 0>(acc, in, in_norm, fl_bytes, link_src<STG>(7, LB, gb + 3 * blk, Vh, tm), Vh, tm, wtm);
+#define TM_HOP(H, W)                                                                                              \
+    hop<PREC, NF, RECON, (H), DAG, STG>(acc, in + spinor_site_off(PREC, NF, nbr[(H)], 0), nbr[(H)] & (TM_TILE - 1),  \
+                                        ((H) & 1) ? gb + link_site_off(PREC, RECON, nbr[(H)], (H) >> 1)             \
+                                                  : lf + ((H) >> 1) * link_tile_bytes(PREC, RECON),                 \
+                                        ((H) & 1) ? (nbr[(H)] & (TM_TILE - 1)) : lane, (W))
+    TM_HOP(0, (real)1); TM_HOP(1, (real)1); TM_HOP(2, (real)1); TM_HOP(3, (real)1);
+    TM_HOP(4, (real)1); TM_HOP(5, (real)1); TM_HOP(6, wtp); TM_HOP(7, wtm);
+#undef TM_HOP
 
     // a7: fused local epilogue
     real xv[NF * 24];
     if constexpr (KT != 0) {
-        const char *xb = static_cast<const char *>(a.x);
-        const float *xn = reinterpret_cast<const float *>(xb + NF * fl_bytes);
+        const char *xs = static_cast<const char *>(a.x) + spinor_site_off(PREC, NF, site, 0);
 #pragma unroll
-        for (int f = 0; f < NF; f++) load_spinor<PREC, 0>(xv + 24 * f, xb + f * fl_bytes, xn + (size_t)f * Vh, Vh, site);
+        for (int f = 0; f < NF; f++) load_spinor<PREC, 0>(xv + 24 * f, xs + f * spinor_tile_bytes(PREC), lane);
     }
     epilogue<NF, KT>(acc, xv, (real)a.alpha, (real)a.beta, (real)a.scale, (real)a.kappa, (real)a.kappa2);
 
     // a8: single store
-    char *ob = static_cast<char *>(a.out);
-    float *on = reinterpret_cast<float *>(ob + NF * fl_bytes);
+    char *os = static_cast<char *>(a.out) + spinor_site_off(PREC, NF, site, 0);
 #pragma unroll
-    for (int f = 0; f < NF; f++) store_spinor<PREC>(acc + 24 * f, ob + f * fl_bytes, on + (size_t)f * Vh, Vh, site);
+    for (int f = 0; f < NF; f++) store_spinor<PREC>(acc + 24 * f, os + f * spinor_tile_bytes(PREC), lane);
 }
 
 template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>

@@ -34,7 +34,7 @@
 #define TM_PD_2_1 0
 #endif
 #ifndef TM_PD_2_2
-#define TM_PD_2_2 2
+#define TM_PD_2_2 1
 #endif
 // Resident blocks of 128 threads per SM the register allocation aims at (second __launch_bounds__ argument).  It is
 // what makes ptxas keep the pipelined loads early: without it the loads are sunk back next to their first use.
@@ -45,7 +45,7 @@
 #define TM_MINB_4_2 3
 #endif
 #ifndef TM_MINB_2_1
-#define TM_MINB_2_1 5
+#define TM_MINB_2_1 3
 #endif
 #ifndef TM_MINB_2_2
 #define TM_MINB_2_2 4
@@ -98,47 +98,41 @@ template <bool SM> TM_DEV uint4 ld_u4(const void *p) { if constexpr (SM) return 
 template <bool SM> TM_DEV uint2 ld_u2(const void *p) { if constexpr (SM) return *reinterpret_cast<const uint2 *>(p); else return ldg_nc_u2(p); }
 template <bool SM> TM_DEV unsigned ld_u1(const void *p) { if constexpr (SM) return *reinterpret_cast<const unsigned *>(p); else return ldg_nc_u1(p); }
 
-// a4 (fetch): the stored words of one link, from its [parity][mu] block or from the staged shared-memory slots
+// a4 (fetch): the stored words of one link; `lp` = the link's site pointer in global memory or in the staged copy
 template <int PREC, int NF, int RECON, bool SM>
-TM_DEV void issue_link(HopRaw<PREC, NF, RECON> &r, const char *base, int Vh, int idx)
+TM_DEV void issue_link(HopRaw<PREC, NF, RECON> &r, const char *lp, int lane)
 {
-    if constexpr (PREC == 4) {
+    constexpr int N16 = link_n16<PREC, RECON>();
 #pragma unroll
-        for (int k = 0; k < HopRaw<PREC, NF, RECON>::NL; k++) r.l[k] = ld_u4<SM>(base + ((size_t)k * Vh + idx) * 16);
-        if constexpr (RECON == 18) r.lt = ld_u2<SM>(base + (size_t)4 * Vh * 16 + (size_t)idx * 8);
-    } else {
-        r.l[0] = ld_u4<SM>(base + (size_t)idx * 16);
-        if constexpr (RECON == 18) {
-            r.l[1] = ld_u4<SM>(base + ((size_t)Vh + idx) * 16);
-            r.lt.x = ld_u1<SM>(base + (size_t)2 * Vh * 16 + (size_t)idx * 4);
-        } else {
-            r.lt = ld_u2<SM>(base + (size_t)Vh * 16 + (size_t)idx * 8);
-        }
-    }
+    for (int k = 0; k < N16; k++) r.l[k] = ld_u4<SM>(lp + k * TM_PLANE);
+    if constexpr (PREC == 4 && RECON == 18) r.lt = ld_u2<SM>(lp + tail_off(4, 8, lane));
+    if constexpr (PREC == 2 && RECON == 18) r.lt.x = ld_u1<SM>(lp + tail_off(2, 4, lane));
+    if constexpr (PREC == 2 && RECON == 12) r.lt = ld_u2<SM>(lp + tail_off(1, 8, lane));
 }
 
-// PART: 0 all, 1 upper half only, 2 lower half only (time hops, a3).  `base` = chunk block of flavor 0.
+// PART: 0 all, 1 upper half only, 2 lower half only (time hops, a3).  `sp` = site pointer of flavor 0.
 template <int PREC, int NF, int RECON, int PART>
-TM_DEV void issue_spinor(HopRaw<PREC, NF, RECON> &r, const char *base, const float *norm, size_t fl_bytes, int Vh, int idx)
+TM_DEV void issue_spinor(HopRaw<PREC, NF, RECON> &r, const char *sp, int lane)
 {
 #pragma unroll
     for (int f = 0; f < NF; f++) {
-        const char *p = base + f * fl_bytes + (size_t)idx * 16;
+        const char *p = sp + f * spinor_tile_bytes(PREC);
         if constexpr (PREC == 4) {
             constexpr int lo = (PART == 2) ? 3 : 0, hi = (PART == 1) ? 3 : 6;
 #pragma unroll
-            for (int k = lo; k < hi; k++) r.s[f][k] = ld_u4<false>(p + (size_t)k * Vh * 16);
+            for (int k = lo; k < hi; k++) r.s[f][k] = ld_u4<false>(p + k * TM_PLANE);
         } else {
             if constexpr (PART != 2) r.s[f][0] = ld_u4<false>(p);
-            r.s[f][1] = ld_u4<false>(p + (size_t)Vh * 16);
-            if constexpr (PART != 1) r.s[f][2] = ld_u4<false>(p + (size_t)2 * Vh * 16);
-            r.n[f] = __uint_as_float(ldg_nc_u1(norm + (size_t)f * Vh + idx));
+            r.s[f][1] = ld_u4<false>(p + TM_PLANE);
+            if constexpr (PART != 1) r.s[f][2] = ld_u4<false>(p + 2 * TM_PLANE);
+            r.n[f] = __uint_as_float(ldg_nc_u1(p + tail_off(3, 4, lane)));
         }
     }
 }
 
-// raw words -> pairs.  fp32: values; half: RAW integers as floats (scale deferred).  Only the PART's pairs are valid.
-template <int PREC, int PART>
+// raw words -> pairs.  fp32: values; half: RAW integers as floats (scale deferred), or BIASED: raw + TM_CVT_MAGIC
+// (the bias is removed for free by the projection).  Only the PART's pairs are valid.
+template <int PREC, int PART, bool BIASED = false>
 TM_DEV void raw_to_spinor(f2 *S, const uint4 *s)
 {
     if constexpr (PREC == 4) {
@@ -149,19 +143,20 @@ TM_DEV void raw_to_spinor(f2 *S, const uint4 *s)
             S[2 * k + 1] = mk2(__uint_as_float(s[k].z), __uint_as_float(s[k].w));
         }
     } else {
+        auto cv = [](uint32_t w) { if constexpr (BIASED) return cvt_pair_biased(w); else return cvt_pair(w); };
         if constexpr (PART != 2) {
-            S[0] = cvt_pair(s[0].x); S[1] = cvt_pair(s[0].y); S[2] = cvt_pair(s[0].z); S[3] = cvt_pair(s[0].w);
-            S[4] = cvt_pair(s[1].x); S[5] = cvt_pair(s[1].y);
+            S[0] = cv(s[0].x); S[1] = cv(s[0].y); S[2] = cv(s[0].z); S[3] = cv(s[0].w);
+            S[4] = cv(s[1].x); S[5] = cv(s[1].y);
         }
         if constexpr (PART != 1) {
-            S[6] = cvt_pair(s[1].z); S[7] = cvt_pair(s[1].w);
-            S[8] = cvt_pair(s[2].x); S[9] = cvt_pair(s[2].y); S[10] = cvt_pair(s[2].z); S[11] = cvt_pair(s[2].w);
+            S[6] = cv(s[1].z); S[7] = cv(s[1].w);
+            S[8] = cv(s[2].x); S[9] = cv(s[2].y); S[10] = cv(s[2].z); S[11] = cv(s[2].w);
         }
     }
 }
 
-// a4 (rebuild): link as 9 (re, im) pairs W[row*3+col]; half: RAW integers for rows 0,1 (12-real: row 2 rebuilt and
-// rescaled to the same raw scale).
+// a4 (rebuild): link as 9 (re, im) pairs W[row*3+col]; half: RAW integers for rows 0,1; 12-real: row 2 is rebuilt and,
+// in half, left at raw x raw scale: the factor 1/32767 is applied where it is cheapest (consume_hop).
 template <int PREC, int NF, int RECON>
 TM_DEV void raw_to_link(f2 *W, const HopRaw<PREC, NF, RECON> &r)
 {
@@ -190,15 +185,26 @@ TM_DEV void raw_to_link(f2 *W, const HopRaw<PREC, NF, RECON> &r)
             const f2 A = W[c1], B = W[3 + c2], C = W[c2], D = W[3 + c1];
             const f2 S = fma2(bc2(-C.x), D, mul2(bc2(A.x), B));
             const f2 T = fma2(bc2(-C.y), sw2(D), mul2(bc2(A.y), sw2(B)));
-            float re = S.x - T.x, im = -S.y - T.y;
-            if constexpr (PREC == 2) { re *= TM_INV15; im *= TM_INV15; }     // raw * raw / 32767 -> raw scale
-            W[6 + c] = mk2(re, im);
+            // half: row 2 stays at raw * raw scale (32767 x the raw scale of rows 0, 1); consume_hop compensates
+            W[6 + c] = mk2(S.x - T.x, -S.y - T.y);
         }
     }
 }
 
 // ---- a3: spin projection, packed ----------------------------------------------------------------------
-template <int MU, int SGN>
+// Every output pair is  U + c * L'  with c = +-1 per lane (L' = L, maybe lane-swapped).  BIASED (half): U and L carry
+// the conversion bias M; a lane with c = -1 cancels it exactly, a lane with c = +1 needs U - 2M first (exact: all
+// values are integers below 2^24), so the conversion costs one FADD2 per pair with a +1 lane instead of one per
+// input pair, and the result is bit-identical to projecting the unbiased integers.
+template <bool BIASED>
+TM_DEV f2 proj_fma(f2 L, f2 c, f2 U)
+{
+    if constexpr (BIASED) {
+        if (c.x > 0.f || c.y > 0.f) U = add2(U, mk2(c.x > 0.f ? -2.f * TM_CVT_MAGIC : 0.f, c.y > 0.f ? -2.f * TM_CVT_MAGIC : 0.f));
+    }
+    return fma2(L, c, U);
+}
+template <int MU, int SGN, bool BIASED = false>
 TM_DEV void project_f2(f2 *H, const f2 *S)
 {
     const f2 *U = S, *L = S + 6;
@@ -207,14 +213,14 @@ TM_DEV void project_f2(f2 *H, const f2 *S)
     for (int c = 0; c < 3; c++) {
         const f2 Ur = U[2 * c], Ui = U[2 * c + 1], Lr = L[2 * c], Li = L[2 * c + 1];
         if constexpr (MU == 0) {
-            H[2 * c] = fma2(sw2(Li), bc2((float)SGN), Ur);
-            H[2 * c + 1] = fma2(sw2(Lr), bc2((float)-SGN), Ui);
+            H[2 * c] = proj_fma<BIASED>(sw2(Li), bc2((float)SGN), Ur);
+            H[2 * c + 1] = proj_fma<BIASED>(sw2(Lr), bc2((float)-SGN), Ui);
         } else if constexpr (MU == 1) {
-            H[2 * c] = fma2(sw2(Lr), mp, Ur);
-            H[2 * c + 1] = fma2(sw2(Li), mp, Ui);
+            H[2 * c] = proj_fma<BIASED>(sw2(Lr), mp, Ur);
+            H[2 * c + 1] = proj_fma<BIASED>(sw2(Li), mp, Ui);
         } else {
-            H[2 * c] = fma2(Li, pm, Ur);
-            H[2 * c + 1] = fma2(Lr, mp, Ui);
+            H[2 * c] = proj_fma<BIASED>(Li, pm, Ur);
+            H[2 * c + 1] = proj_fma<BIASED>(Lr, mp, Ui);
         }
     }
 }
@@ -249,21 +255,22 @@ TM_DEV void su3_mul_f2(f2 *G, const f2 *W, const f2 *H)
 //   x: (i s1 g) = (i g1, i g0)  -> Alr += -sgn sw(Gi), Ali += +sgn sw(Gr)
 //   y: (i s2 g) = (g1, -g0)     -> Alr += (sgn,-sgn) sw(Gr), Ali += (sgn,-sgn) sw(Gi)
 //   z: (i s3 g) = (i g0, -i g1) -> Alr += (-sgn,sgn) Gi,     Ali += (sgn,-sgn) Gr
+// w2 = the weight of color 2 (differs from w only when row 2 of a half-precision link was left unscaled).
 template <int MU, int SGN>
-TM_DEV void reconstruct_f2(f2 *A, const f2 *G, float w)
+TM_DEV void reconstruct_f2(f2 *A, const f2 *G, float w, float w2)
 {
     f2 *Au = A, *Al = A + 6;
     if constexpr (MU == 3) {
         f2 *dst = (SGN > 0) ? Al : Au;
 #pragma unroll
-        for (int i = 0; i < 6; i++) dst[i] = fma2(G[i], bc2(w), dst[i]);
+        for (int i = 0; i < 6; i++) dst[i] = fma2(G[i], bc2(i < 4 ? w : w2), dst[i]);
     } else {
-        const float sw_ = (float)SGN * w;
-        const f2 pm = mk2(sw_, -sw_), mp = mk2(-sw_, sw_);
 #pragma unroll
-        for (int i = 0; i < 6; i++) Au[i] = fma2(G[i], bc2(w), Au[i]);
+        for (int i = 0; i < 6; i++) Au[i] = fma2(G[i], bc2(i < 4 ? w : w2), Au[i]);
 #pragma unroll
         for (int c = 0; c < 3; c++) {
+            const float sw_ = (float)SGN * (c < 2 ? w : w2);
+            const f2 pm = mk2(sw_, -sw_), mp = mk2(-sw_, sw_);
             const f2 Gr = G[2 * c], Gi = G[2 * c + 1];
             if constexpr (MU == 0) {
                 Al[2 * c] = fma2(sw2(Gi), bc2(-sw_), Al[2 * c]);
@@ -281,13 +288,9 @@ TM_DEV void reconstruct_f2(f2 *A, const f2 *G, float w)
 
 // Where the fields are: the same for every site of a launch (kept in uniform registers).
 struct HopPtrs {
-    const char *in;          // input spinor, flavor 0 chunk block
-    const float *in_norm;
+    const char *in;          // input spinor field
     const char *x;           // xpay input (own parity)
-    const float *x_norm;
     const char *gf, *gb;     // gauge blocks of the output parity (forward links) / the other parity (backward links)
-    size_t fl_bytes, blk;
-    int Vh;
 };
 // a2: one output site: its checkerboard index, the 8 neighbour indices (periodic wrap) and the time-hop weights.
 struct HopCtx {
@@ -299,12 +302,12 @@ struct HopCtx {
 TM_DEV void site_ctx(HopCtx &c, const DslashArgs &a, int site)
 {
     const int Xh = a.Xh;
-    const int xh = site % Xh;
-    int r = site / Xh;
-    const int y = r % a.Y;
-    r /= a.Y;
-    const int z = r % a.Z;
-    const int t = r / a.Z;
+    int r = tm_div(site, a.dXh);
+    const int xh = site - r * Xh;
+    int r2 = tm_div(r, a.dY);
+    const int y = r - r2 * a.Y;
+    const int t = tm_div(r2, a.dZ);
+    const int z = r2 - t * a.Z;
     const int q = (y + z + t + a.parity) & 1;       // x1 = 2 xh + q
     const int sy = Xh, sz = Xh * a.Y, st = Xh * a.Y * a.Z;
     c.site = site;
@@ -321,6 +324,7 @@ TM_DEV void site_ctx(HopCtx &c, const DslashArgs &a, int site)
 }
 
 // Pipeline slot H of a site: 0..7 = the hops in the order of HopCtx::nbr, 8 = the xpay input of the site, > 8 nothing.
+// One address computation per neighbour (spinor_site_off / link_site_off); every load then uses an immediate offset.
 template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, int H>
 TM_DEV void issue_slot(HopRaw<PREC, NF, RECON> &r, const HopPtrs &p, const HopCtx &c)
 {
@@ -329,10 +333,14 @@ TM_DEV void issue_slot(HopRaw<PREC, NF, RECON> &r, const HopPtrs &p, const HopCt
         constexpr bool FWD = (H % 2) == 0;
         constexpr int SGN = (FWD != DAG) ? +1 : -1;
         constexpr int PART = (MU == 3) ? ((SGN > 0) ? 2 : 1) : 0;
-        if constexpr (!STG) issue_link<PREC, NF, RECON, false>(r, (FWD ? p.gf : p.gb) + MU * p.blk, p.Vh, FWD ? c.site : c.nbr[H]);
-        issue_spinor<PREC, NF, RECON, PART>(r, p.in, p.in_norm, p.fl_bytes, p.Vh, c.nbr[H]);
+        const int n = c.nbr[H];
+        if constexpr (!STG) {
+            if constexpr (FWD) issue_link<PREC, NF, RECON, false>(r, p.gf + link_site_off(PREC, RECON, c.site, MU), c.site & (TM_TILE - 1));
+            else issue_link<PREC, NF, RECON, false>(r, p.gb + link_site_off(PREC, RECON, n, MU), n & (TM_TILE - 1));
+        }
+        issue_spinor<PREC, NF, RECON, PART>(r, p.in + spinor_site_off(PREC, NF, n, 0), n & (TM_TILE - 1));
     } else if constexpr (H == 8 && KT != 0) {
-        issue_spinor<PREC, NF, RECON, 0>(r, p.x, p.x_norm, p.fl_bytes, p.Vh, c.site);
+        issue_spinor<PREC, NF, RECON, 0>(r, p.x + spinor_site_off(PREC, NF, c.site, 0), c.site & (TM_TILE - 1));
     }
 }
 
@@ -346,7 +354,7 @@ TM_DEV void consume_hop(f2 *A, HopRaw<PREC, NF, RECON> &r, const HopCtx &c)
     constexpr int PART = (MU == 3) ? ((SGN > 0) ? 2 : 1) : 0;
     if constexpr (STG) {
         cp_async_wait<7 - H>();
-        issue_link<PREC, NF, RECON, true>(r, tm_smem + (size_t)H * (RECON * PREC) * blockDim.x, blockDim.x, threadIdx.x);
+        issue_link<PREC, NF, RECON, true>(r, stage_slot<PREC, RECON>(H), threadIdx.x & 31);
     }
     f2 W[9];
     raw_to_link<PREC, NF, RECON>(W, r);
@@ -354,17 +362,25 @@ TM_DEV void consume_hop(f2 *A, HopRaw<PREC, NF, RECON> &r, const HopCtx &c)
 #pragma unroll
     for (int f = 0; f < NF; f++) {
         f2 S[12], H6[6], G[6];
-        raw_to_spinor<PREC, PART>(S, r.s[f]);
         if constexpr (MU == 3) {
+            raw_to_spinor<PREC, PART>(S, r.s[f]);
 #pragma unroll
             for (int i = 0; i < 6; i++) H6[i] = (SGN > 0) ? S[6 + i] : S[i];
         } else {
-            project_f2<MU, SGN>(H6, S);
+            raw_to_spinor<PREC, PART, PREC == 2>(S, r.s[f]);
+            project_f2<MU, SGN, PREC == 2>(H6, S);
         }
-        float wf = w;
-        if constexpr (PREC == 2) wf *= r.n[f] * (TM_INV15 * TM_INV15);   // site norm x link scale
+        float wf = w, wf2 = w;
+        if constexpr (PREC == 2) {
+            wf *= r.n[f] * (TM_INV15 * TM_INV15);                        // site norm x link scale
+            wf2 = wf;
+            if constexpr (RECON == 12) {                                 // row 2 of the link carries an extra 32767
+                if constexpr (FWD) wf2 = wf * TM_INV15;                  // U h: row 2 -> output color 2
+                else { H6[4] = mul2(H6[4], bc2(TM_INV15)); H6[5] = mul2(H6[5], bc2(TM_INV15)); }   // U^+ h: row 2 meets h color 2
+            }
+        }
         su3_mul_f2<!FWD>(G, W, H6);
-        reconstruct_f2<MU, SGN>(A + 12 * f, G, wf);
+        reconstruct_f2<MU, SGN>(A + 12 * f, G, wf, wf2);
     }
 }
 
@@ -411,18 +427,17 @@ TM_DEV void epilogue_f2(f2 *A, const f2 *X, float alpha, float beta, float scale
 
 // ---- a8: single store -----------------------------------------------------------------------------------
 template <int PREC>
-TM_DEV void store_spinor_f2(const f2 *A, char *base, float *norm, int Vh, int idx)
+TM_DEV void store_spinor_f2(const f2 *A, char *sp, int lane)
 {
     if constexpr (PREC == 4) {
-        float4 *p = reinterpret_cast<float4 *>(base) + idx;
 #pragma unroll
-        for (int k = 0; k < 6; k++) p[(size_t)k * Vh] = make_float4(A[2 * k].x, A[2 * k].y, A[2 * k + 1].x, A[2 * k + 1].y);
+        for (int k = 0; k < 6; k++)
+            *reinterpret_cast<float4 *>(sp + k * TM_PLANE) = make_float4(A[2 * k].x, A[2 * k].y, A[2 * k + 1].x, A[2 * k + 1].y);
     } else {
         float m = 0.f;
 #pragma unroll
         for (int i = 0; i < 12; i++) m = fmaxf(m, fmaxf(fabsf(A[i].x), fabsf(A[i].y)));
         const float s = (m > 0.f) ? __fdividef(32767.0f, m) : 0.f;
-        int4 *p = reinterpret_cast<int4 *>(base) + idx;
 #pragma unroll
         for (int k = 0; k < 3; k++) {
             int4 c;
@@ -430,9 +445,9 @@ TM_DEV void store_spinor_f2(const f2 *A, char *base, float *norm, int Vh, int id
             c.y = quant_pair(A[4 * k + 1], s);
             c.z = quant_pair(A[4 * k + 2], s);
             c.w = quant_pair(A[4 * k + 3], s);
-            p[(size_t)k * Vh] = c;
+            *reinterpret_cast<int4 *>(sp + k * TM_PLANE) = c;
         }
-        norm[idx] = m;
+        *reinterpret_cast<float *>(sp + tail_off(3, 4, lane)) = m;
     }
 }
 
@@ -456,7 +471,6 @@ TM_DEV void load_x(f2 *X, const HopRaw<PREC, NF, RECON> &rx)
 template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
 __global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(const DslashArgs a)
 {
-    constexpr int NCH = PrecTraits<PREC>::NCH;
     constexpr int PD = f2_pipeline_depth<PREC, NF>();
     const int Vh = a.Vh;
     prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, blockIdx.x);
@@ -464,24 +478,19 @@ __global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(c
     if (site >= Vh) return;
 
     HopPtrs p;
-    p.fl_bytes = (size_t)NCH * Vh * 16;
+    const size_t PB = (size_t)tm_tiles(Vh) * 4 * link_tile_bytes(PREC, RECON);     // one parity's gauge block
     p.in = static_cast<const char *>(a.in);
-    p.in_norm = reinterpret_cast<const float *>(p.in + NF * p.fl_bytes);
     p.x = static_cast<const char *>(a.x);
-    p.x_norm = reinterpret_cast<const float *>(p.x + NF * p.fl_bytes);
-    p.blk = (size_t)RECON * PREC * Vh;
-    p.gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * 4 * p.blk;
-    p.gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * 4 * p.blk;
-    p.Vh = Vh;
+    p.gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * PB;
+    p.gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * PB;
 
     HopCtx c;
     site_ctx(c, a, site);
     if constexpr (STG) {
-        constexpr int LB = RECON * PREC;
 #pragma unroll
         for (int h = 0; h < 8; h++)
-            stage_link<PREC, RECON>(tm_smem + h * LB * blockDim.x, ((h & 1) ? p.gb : p.gf) + (h >> 1) * p.blk, Vh,
-                                    (h & 1) ? c.nbr[h] : site, blockDim.x, threadIdx.x);
+            stage_link<PREC, RECON>(h, (h & 1) ? p.gb + link_site_off(PREC, RECON, c.nbr[h], h >> 1) : p.gf + link_site_off(PREC, RECON, site, h >> 1),
+                                    ((h & 1) ? c.nbr[h] : site) & (TM_TILE - 1));
     }
 
     f2 A[NF * 12], X[NF * 12];
@@ -506,10 +515,9 @@ __global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(c
 
     epilogue_f2<NF, KT>(A, X, (float)a.alpha, (float)a.beta, (float)a.scale, (float)a.kappa, (float)a.kappa2);
 
-    char *ob = static_cast<char *>(a.out);
-    float *on = reinterpret_cast<float *>(ob + NF * p.fl_bytes);
+    char *os = static_cast<char *>(a.out) + spinor_site_off(PREC, NF, site, 0);
 #pragma unroll
-    for (int f = 0; f < NF; f++) store_spinor_f2<PREC>(A + 12 * f, ob + f * p.fl_bytes, on + (size_t)f * Vh, Vh, site);
+    for (int f = 0; f < NF; f++) store_spinor_f2<PREC>(A + 12 * f, os + f * spinor_tile_bytes(PREC), site & (TM_TILE - 1));
 }
 
 template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>

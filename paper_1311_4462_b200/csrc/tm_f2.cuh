@@ -66,6 +66,12 @@ TM_DEV f2 sub2(f2 a, f2 b) { return add2(a, neg2(b)); }
 // Stored int16 are OFFSET BINARY: u = q + 32768.  A 32-bit word holds the pair's two lanes.
 //   float bits 0x4B000000 | u  =  2^23 + u   ->   q = that - (2^23 + 32768), exact.
 #define TM_CVT_MAGIC 8421376.0f            /* 2^23 + 2^15 */
+// The biased pair (2^23 + u_lo, 2^23 + u_hi) = (M + q_lo, M + q_hi), M = TM_CVT_MAGIC: 2 PRMT, no arithmetic.
+// Sums and differences of biased values in which the M cancel are exact (project_f2 uses this).
+TM_DEV f2 cvt_pair_biased(uint32_t w)
+{
+    return mk2(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)), __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)));
+}
 TM_DEV f2 cvt_pair(uint32_t w)             // -> (q_lo, q_hi) as integer-valued floats: 2 PRMT + 1 FADD2
 {
     const float lo = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610));

@@ -1,14 +1,15 @@
 // tm_internal.h -- private structures shared by the C-ABI layer (tm_api.cu) and the kernel launchers.
-// Device layout (row a1):
-//   spinor, one parity : [flavor][chunk][cb site] in 128-bit chunks
-//        fp64: 12 chunks of double2 (one complex each, index spin*3+color)
-//        fp32:  6 chunks of float4  (two complex each)
-//        half:  3 chunks of 8 x int16, followed by float norm[flavor][cb site]
-//   gauge : [parity][mu][plane][cb site]; a link's reals r = (row*3+col)*2+reim are cut into planes
-//        fp64: recon planes of double2              (9 for 18-real, 6 for 12-real)
+// Device layout (row a1; addressing helpers in tm_layout.cuh): tiles of 32 consecutive
+// checkerboard sites, inside a tile one 512-byte plane per 128-bit chunk
+//   spinor, one parity : [tile][flavor][plane][32]
+//        fp64: 12 planes of double2 (one complex each, index spin*3+color)
+//        fp32:  6 planes of float4  (two complex each)
+//        half:  3 planes of 8 x int16 + one 128-byte plane of float norms
+//   gauge : [parity][tile][mu][plane][32]; a link's reals r = (row*3+col)*2+reim are cut into planes
+//        fp64: recon/2 planes of double2
 //        fp32: 18 -> 4 x float4 + 1 x float2 ; 12 -> 3 x float4
 //        half: 18 -> 2 x int4(8 x int16) + 1 x int(2 x int16) ; 12 -> 1 x int4 + 1 x int2
-//   [parity][mu] block holds U_mu(x) for the sites x of that parity.
+//   the [parity] block holds U_mu(x) for the sites x of that parity.
 #pragma once
 #include <cuda_runtime.h>
 #include <stddef.h>
@@ -59,9 +60,27 @@ struct tm_gauge {
     size_t bytes;
 };
 
-// bytes of one flavor's chunk block per site (without norms) and of one link per site
-static inline size_t tm_spinor_site_bytes(int prec) { return (size_t)24 * (size_t)prec; }
-static inline size_t tm_link_site_bytes(int prec, int recon) { return (size_t)recon * (size_t)prec; }
+
+// Division of a site index (< 2^31) by a lattice extent d >= 2 without the integer-division sequence:
+// q = umulhi(n, m) >> sh with m = floor(2^(31+l) / d) + 1, l = ceil(log2 d), sh = l - 1 (exact for every n < 2^31).
+struct TmFastDiv {
+    unsigned m;
+    int sh;
+    int d;
+};
+static inline TmFastDiv tm_fastdiv(int d)
+{
+    TmFastDiv f;
+    int l = 0;
+    while ((1LL << l) < d) l++;
+    f.m = (unsigned)(((1ULL << (31 + l)) / (unsigned long long)d) + 1ULL);
+    f.sh = l - 1;
+    f.d = d;
+    return f;
+}
+#ifdef __CUDACC__
+__device__ __forceinline__ int tm_div(int n, const TmFastDiv &f) { return (int)(__umulhi((unsigned)n, f.m) >> f.sh); }
+#endif
 
 // Arguments of one fused dslash launch.  Coefficients are formed in double on the host (reading C10-ii)
 // and cast to the kernel's arithmetic type on the device.
@@ -71,6 +90,7 @@ struct DslashArgs {
     const void *x;
     const void *gauge;
     int X, Y, Z, T, Xh, Vh;
+    TmFastDiv dXh, dY, dZ;   // site decode
     int parity;          // parity of the output sites
     double alpha;        // local twist, flavor 0:  w = scale * (v + i alpha gamma5 v + beta v_otherflavor)
     double beta;

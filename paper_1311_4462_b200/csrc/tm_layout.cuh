@@ -17,6 +17,32 @@ template <> struct PrecTraits<2> { typedef float real;  static constexpr int NCH
 #define TM_HALF_MAX 32767.0f
 #define TM_HALF_INV (1.0f / 32767.0f)
 
+// ---- tiled SoA addressing ----------------------------------------------------------
+// Fields are cut into TILES of 32 consecutive checkerboard sites (one warp).  Inside a tile every 128-bit chunk is
+// a PLANE of 32 x 16 = 512 contiguous bytes, so a warp's access to a plane is one 512-byte segment and the planes
+// of a site are at COMPILE-TIME offsets from the site's pointer (one address computation per neighbour, immediate
+// offsets for every further load).
+//   spinor, one parity : [tile][flavor][plane][32]   planes: 12 (fp64) / 6 (fp32) / 3 + a 128-byte norm plane (half)
+//   gauge              : [parity][tile][mu][plane][32]  planes of 16 bytes per site, then one narrower tail plane
+#define TM_TILE 32
+#define TM_TILE_LOG 5
+#define TM_PLANE 512
+__host__ __device__ constexpr int spinor_tile_bytes(int prec) { return prec == 8 ? 12 * 512 : prec == 4 ? 6 * 512 : 3 * 512 + 128; }
+__host__ __device__ constexpr int link_tile_bytes(int prec, int recon) { return recon * prec * TM_TILE; }
+__host__ __device__ inline int tm_tiles(int Vh) { return (Vh + TM_TILE - 1) / TM_TILE; }
+// byte offset of (site idx, flavor f) in a spinor field of nf flavors: points at the site's 16 bytes of plane 0
+__host__ __device__ inline size_t spinor_site_off(int prec, int nf, int idx, int f)
+{
+    return ((size_t)(idx >> TM_TILE_LOG) * nf + f) * spinor_tile_bytes(prec) + (size_t)(idx & (TM_TILE - 1)) * 16;
+}
+// byte offset of U_mu at site idx inside one parity's gauge block (block size = tiles * 4 * link_tile_bytes)
+__host__ __device__ inline size_t link_site_off(int prec, int recon, int idx, int mu)
+{
+    return ((size_t)(idx >> TM_TILE_LOG) * 4 + mu) * link_tile_bytes(prec, recon) + (size_t)(idx & (TM_TILE - 1)) * 16;
+}
+// A narrower plane (w bytes per site) that follows n16 full planes: its element for `lane` relative to the site pointer
+__host__ __device__ constexpr int tail_off(int n16, int w, int lane) { return n16 * TM_PLANE - lane * (16 - w); }
+
 TM_DEV float tm_fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 TM_DEV double tm_fma(double a, double b, double c) { return __fma_rn(a, b, c); }
 
@@ -57,19 +83,19 @@ __host__ __device__ constexpr int raw_pos(int o)
 }
 
 // ---- spinor loads ---------------------------------------------------------------------------------
-// `base` points at the flavor's chunk block, `norm` at the flavor's norm array (half only), Vh = sites.
+// `sp` = the site's pointer (field + spinor_site_off), `lane` = idx & 31 (needed for the half norm plane).
 // PART: 0 = all 24 reals, 1 = upper only (v[0..11] valid), 2 = lower only (v[12..23] valid).
 template <int PART>
-TM_DEV void load_spinor_half_raw(float *v, const char *base, const float *norm, int Vh, int idx);
+TM_DEV void load_spinor_half_raw(float *v, const char *sp, int lane);
 
 template <int PREC, int PART>
-TM_DEV void load_spinor(typename PrecTraits<PREC>::real *v, const char *base, const float *norm, int Vh, int idx)
+TM_DEV void load_spinor(typename PrecTraits<PREC>::real *v, const char *sp, int lane)
 {
     if constexpr (PREC == 8) {
         constexpr int lo = (PART == 2) ? 6 : 0, hi = (PART == 1) ? 6 : 12;
 #pragma unroll
         for (int k = lo; k < hi; k++) {
-            double2 c = ldg_d2(base + ((size_t)k * Vh + idx) * 16);
+            double2 c = ldg_d2(sp + k * TM_PLANE);
             v[2 * k] = c.x;
             v[2 * k + 1] = c.y;
         }
@@ -78,7 +104,7 @@ TM_DEV void load_spinor(typename PrecTraits<PREC>::real *v, const char *base, co
         float r[24];
 #pragma unroll
         for (int k = lo; k < hi; k++) {
-            float4 c = ldg_f4(base + ((size_t)k * Vh + idx) * 16);
+            float4 c = ldg_f4(sp + k * TM_PLANE);
             r[4 * k] = c.x;
             r[4 * k + 1] = c.y;
             r[4 * k + 2] = c.z;
@@ -89,61 +115,57 @@ TM_DEV void load_spinor(typename PrecTraits<PREC>::real *v, const char *base, co
     } else {
         // 3 chunks of 8 int16: raw 0..7, 8..15, 16..23.  upper = raw 0..11, lower = raw 12..23.
         float r[24];
-        load_spinor_half_raw<PART>(r, base, norm, Vh, idx);
+        load_spinor_half_raw<PART>(r, sp, lane);
 #pragma unroll
         for (int o = (PART == 2 ? 12 : 0); o < (PART == 1 ? 12 : 24); o++) v[o] = r[raw_pos(o)];
     }
 }
 
 template <int PART>
-TM_DEV void load_spinor_half_raw(float *v, const char *base, const float *norm, int Vh, int idx)
+TM_DEV void load_spinor_half_raw(float *v, const char *sp, int lane)
 {
+    const float s = ldg_f1(sp + tail_off(3, 4, lane)) * TM_HALF_INV;
+    if constexpr (PART != 2) {
+        int4 c = ldg_i4(sp);
+        unpack2(c.x, s, v[0], v[1]);
+        unpack2(c.y, s, v[2], v[3]);
+        unpack2(c.z, s, v[4], v[5]);
+        unpack2(c.w, s, v[6], v[7]);
+    }
     {
-        const float s = ldg_f1(norm + idx) * TM_HALF_INV;
+        int4 c = ldg_i4(sp + TM_PLANE);
         if constexpr (PART != 2) {
-            int4 c = ldg_i4(base + ((size_t)0 * Vh + idx) * 16);
-            unpack2(c.x, s, v[0], v[1]);
-            unpack2(c.y, s, v[2], v[3]);
-            unpack2(c.z, s, v[4], v[5]);
-            unpack2(c.w, s, v[6], v[7]);
-        }
-        {
-            int4 c = ldg_i4(base + ((size_t)1 * Vh + idx) * 16);
-            if constexpr (PART != 2) {
-                unpack2(c.x, s, v[8], v[9]);
-                unpack2(c.y, s, v[10], v[11]);
-            }
-            if constexpr (PART != 1) {
-                unpack2(c.z, s, v[12], v[13]);
-                unpack2(c.w, s, v[14], v[15]);
-            }
+            unpack2(c.x, s, v[8], v[9]);
+            unpack2(c.y, s, v[10], v[11]);
         }
         if constexpr (PART != 1) {
-            int4 c = ldg_i4(base + ((size_t)2 * Vh + idx) * 16);
-            unpack2(c.x, s, v[16], v[17]);
-            unpack2(c.y, s, v[18], v[19]);
-            unpack2(c.z, s, v[20], v[21]);
-            unpack2(c.w, s, v[22], v[23]);
+            unpack2(c.z, s, v[12], v[13]);
+            unpack2(c.w, s, v[14], v[15]);
         }
+    }
+    if constexpr (PART != 1) {
+        int4 c = ldg_i4(sp + 2 * TM_PLANE);
+        unpack2(c.x, s, v[16], v[17]);
+        unpack2(c.y, s, v[18], v[19]);
+        unpack2(c.z, s, v[20], v[21]);
+        unpack2(c.w, s, v[22], v[23]);
     }
 }
 
 // ---- spinor store (a8): one write of the output site; half: norm = max|v|, q = rint(v * 32767 / norm)
 template <int PREC>
-TM_DEV void store_spinor(const typename PrecTraits<PREC>::real *v, char *base, float *norm, int Vh, int idx)
+TM_DEV void store_spinor(const typename PrecTraits<PREC>::real *v, char *sp, int lane)
 {
     if constexpr (PREC == 8) {
 #pragma unroll
-        for (int k = 0; k < 12; k++)
-            *reinterpret_cast<double2 *>(base + ((size_t)k * Vh + idx) * 16) = make_double2(v[2 * k], v[2 * k + 1]);
+        for (int k = 0; k < 12; k++) *reinterpret_cast<double2 *>(sp + k * TM_PLANE) = make_double2(v[2 * k], v[2 * k + 1]);
     } else if constexpr (PREC == 4) {
         float r[24];
 #pragma unroll
         for (int o = 0; o < 24; o++) r[raw_pos(o)] = v[o];
 #pragma unroll
         for (int k = 0; k < 6; k++)
-            *reinterpret_cast<float4 *>(base + ((size_t)k * Vh + idx) * 16) =
-                make_float4(r[4 * k], r[4 * k + 1], r[4 * k + 2], r[4 * k + 3]);
+            *reinterpret_cast<float4 *>(sp + k * TM_PLANE) = make_float4(r[4 * k], r[4 * k + 1], r[4 * k + 2], r[4 * k + 3]);
     } else {
         float r[24];
 #pragma unroll
@@ -160,14 +182,14 @@ TM_DEV void store_spinor(const typename PrecTraits<PREC>::real *v, char *base, f
             c.y = pack2(v[8 * k + 2] * s, v[8 * k + 3] * s);
             c.z = pack2(v[8 * k + 4] * s, v[8 * k + 5] * s);
             c.w = pack2(v[8 * k + 6] * s, v[8 * k + 7] * s);
-            *reinterpret_cast<int4 *>(base + ((size_t)k * Vh + idx) * 16) = c;
+            *reinterpret_cast<int4 *>(sp + k * TM_PLANE) = c;
         }
-        norm[idx] = m;
+        *reinterpret_cast<float *>(sp + tail_off(3, 4, lane)) = m;
     }
 }
 
 // ---- link load + SU(3) row rebuild (a4) -----------------------------------------------------------
-// `base` points at the [parity][mu] block.  12-real: rows 0,1 stored, row2 = conj(row0 x row1).
+// 12-real: rows 0,1 stored, row2 = conj(row0 x row1).
 template <typename real>
 TM_DEV void rebuild_row2(real *u)
 {
@@ -185,70 +207,65 @@ TM_DEV void rebuild_row2(real *u)
     }
 }
 
-template <int PREC, int RECON, bool SM = false>
-TM_DEV void load_link(typename PrecTraits<PREC>::real *u, const char *base, int Vh, int idx)
+// Planes of a stored link: n16 planes of 16 bytes per site, then (maybe) one tail plane of `tailw` bytes per site.
+template <int PREC, int RECON> __host__ __device__ constexpr int link_n16()
 {
+    return PREC == 8 ? RECON / 2 : PREC == 4 ? (RECON == 18 ? 4 : 3) : (RECON == 18 ? 2 : 1);
+}
+template <int PREC, int RECON> __host__ __device__ constexpr int link_tailw()
+{
+    return PREC == 8 ? 0 : PREC == 4 ? (RECON == 18 ? 8 : 0) : (RECON == 18 ? 4 : 8);
+}
+
+// `lp` = the link's site pointer (gauge parity block + link_site_off) or, SM = true, the thread's slot in the staged
+// shared-memory copy, which keeps the same [plane][32 sites] shape per warp.
+template <int PREC, int RECON, bool SM = false>
+TM_DEV void load_link(typename PrecTraits<PREC>::real *u, const char *lp, int lane)
+{
+    constexpr int N16 = link_n16<PREC, RECON>();
     if constexpr (PREC == 8) {
 #pragma unroll
-        for (int k = 0; k < RECON / 2; k++) {
-            double2 c = ld_d2<SM>(base + ((size_t)k * Vh + idx) * 16);
+        for (int k = 0; k < N16; k++) {
+            double2 c = ld_d2<SM>(lp + k * TM_PLANE);
             u[2 * k] = c.x;
             u[2 * k + 1] = c.y;
         }
     } else if constexpr (PREC == 4) {
-        constexpr int NF4 = (RECON == 18) ? 4 : 3;
 #pragma unroll
-        for (int k = 0; k < NF4; k++) {
-            float4 c = ld_f4<SM>(base + ((size_t)k * Vh + idx) * 16);
+        for (int k = 0; k < N16; k++) {
+            float4 c = ld_f4<SM>(lp + k * TM_PLANE);
             u[4 * k] = c.x;
             u[4 * k + 1] = c.y;
             u[4 * k + 2] = c.z;
             u[4 * k + 3] = c.w;
         }
         if constexpr (RECON == 18) {
-            float2 c = ld_f2<SM>(base + (size_t)4 * Vh * 16 + (size_t)idx * 8);
+            float2 c = ld_f2<SM>(lp + tail_off(4, 8, lane));
             u[16] = c.x;
             u[17] = c.y;
         }
     } else {
         const float s = TM_HALF_INV;
-        int4 c = ld_i4<SM>(base + (size_t)idx * 16);
+        int4 c = ld_i4<SM>(lp);
         unpack2(c.x, s, u[0], u[1]);
         unpack2(c.y, s, u[2], u[3]);
         unpack2(c.z, s, u[4], u[5]);
         unpack2(c.w, s, u[6], u[7]);
         if constexpr (RECON == 18) {
-            int4 d = ld_i4<SM>(base + ((size_t)Vh + idx) * 16);
+            int4 d = ld_i4<SM>(lp + TM_PLANE);
             unpack2(d.x, s, u[8], u[9]);
             unpack2(d.y, s, u[10], u[11]);
             unpack2(d.z, s, u[12], u[13]);
             unpack2(d.w, s, u[14], u[15]);
-            int e = ld_i1<SM>(base + (size_t)2 * Vh * 16 + (size_t)idx * 4);
+            int e = ld_i1<SM>(lp + tail_off(2, 4, lane));
             unpack2(e, s, u[16], u[17]);
         } else {
-            int2 d = ld_i2<SM>(base + (size_t)Vh * 16 + (size_t)idx * 8);
+            int2 d = ld_i2<SM>(lp + tail_off(1, 8, lane));
             unpack2(d.x, s, u[8], u[9]);
             unpack2(d.y, s, u[10], u[11]);
         }
     }
     if constexpr (RECON == 12) rebuild_row2(u);
-}
-
-// ---- L2 prefetch of a later tile ("streaming") ---------------------------------------
-// A link block [parity][mu] is a sequence of planes, plane p = Vh elements of link_plane_width(p) bytes.
-template <int PREC, int RECON> __host__ __device__ constexpr int link_planes()
-{
-    return PREC == 8 ? RECON / 2 : PREC == 4 ? (RECON == 18 ? 5 : 3) : (RECON == 18 ? 3 : 2);
-}
-template <int PREC, int RECON> __host__ __device__ constexpr int link_plane_width(int p)
-{
-    return PREC == 8 ? 16 : PREC == 4 ? (p < 4 ? 16 : 8) : (RECON == 18 ? (p < 2 ? 16 : 4) : (p < 1 ? 16 : 8));
-}
-template <int PREC, int RECON> __host__ __device__ constexpr int link_plane_offset(int p)     // bytes per site before plane p
-{
-    int o = 0;
-    for (int q = 0; q < p; q++) o += link_plane_width<PREC, RECON>(q);
-    return o;
 }
 
 TM_DEV void prefetch_l2(const void *p, unsigned bytes)

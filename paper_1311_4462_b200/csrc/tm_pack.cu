@@ -31,8 +31,7 @@ __global__ void pack_spinor_kernel(char *dst, const double *src, PackGeom g, int
     real v[24];
 #pragma unroll
     for (int k = 0; k < 24; k++) v[k] = (real)s[k];
-    const size_t fl_bytes = (size_t)PrecTraits<PREC>::NCH * g.Vh * 16;
-    store_spinor<PREC>(v, dst + f * fl_bytes, reinterpret_cast<float *>(dst + nf * fl_bytes) + (size_t)f * g.Vh, g.Vh, i);
+    store_spinor<PREC>(v, dst + spinor_site_off(PREC, nf, i, f), i & (TM_TILE - 1));
 }
 
 template <int PREC>
@@ -42,9 +41,8 @@ __global__ void unpack_spinor_kernel(double *dst, const char *src, PackGeom g, i
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= nf * g.Vh) return;
     const int f = tid / g.Vh, i = tid % g.Vh;
-    const size_t fl_bytes = (size_t)PrecTraits<PREC>::NCH * g.Vh * 16;
     real v[24];
-    load_spinor<PREC, 0>(v, src + f * fl_bytes, reinterpret_cast<const float *>(src + nf * fl_bytes) + (size_t)f * g.Vh, g.Vh, i);
+    load_spinor<PREC, 0>(v, src + spinor_site_off(PREC, nf, i, f), i & (TM_TILE - 1));
     double *d = dst_is_cb ? dst + ((size_t)f * g.Vh + i) * 24 : dst + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
 #pragma unroll
     for (int k = 0; k < 24; k++) d[k] = (double)v[k];
@@ -60,31 +58,31 @@ __global__ void pack_gauge_kernel(char *dst, const double *src, PackGeom g)
     const int pm = (int)(tid / g.Vh);       // parity * 4 + mu
     const int parity = pm >> 2, mu = pm & 3;
     const double *s = src + ((size_t)mu * g.V + cb_to_lex(g, i, parity)) * 18;
-    char *blk = dst + (size_t)pm * RECON * PREC * g.Vh;
-    const int Vh = g.Vh;
+    char *lp = dst + (size_t)parity * tm_tiles(g.Vh) * 4 * link_tile_bytes(PREC, RECON) + link_site_off(PREC, RECON, i, mu);
+    const int lane = i & (TM_TILE - 1);
     if constexpr (PREC == 8) {
 #pragma unroll
         for (int k = 0; k < RECON / 2; k++)
-            *reinterpret_cast<double2 *>(blk + ((size_t)k * Vh + i) * 16) = make_double2(s[2 * k], s[2 * k + 1]);
+            *reinterpret_cast<double2 *>(lp + k * TM_PLANE) = make_double2(s[2 * k], s[2 * k + 1]);
     } else if constexpr (PREC == 4) {
         constexpr int NF4 = (RECON == 18) ? 4 : 3;
 #pragma unroll
         for (int k = 0; k < NF4; k++)
-            *reinterpret_cast<float4 *>(blk + ((size_t)k * Vh + i) * 16) =
+            *reinterpret_cast<float4 *>(lp + k * TM_PLANE) =
                 make_float4((float)s[4 * k], (float)s[4 * k + 1], (float)s[4 * k + 2], (float)s[4 * k + 3]);
         if constexpr (RECON == 18)
-            *reinterpret_cast<float2 *>(blk + (size_t)4 * Vh * 16 + (size_t)i * 8) = make_float2((float)s[16], (float)s[17]);
+            *reinterpret_cast<float2 *>(lp + tail_off(4, 8, lane)) = make_float2((float)s[16], (float)s[17]);
     } else {
         int w[9];
 #pragma unroll
         for (int k = 0; k < RECON / 2; k++)
             w[k] = pack2((float)s[2 * k] * TM_HALF_MAX, (float)s[2 * k + 1] * TM_HALF_MAX);
-        *reinterpret_cast<int4 *>(blk + (size_t)i * 16) = make_int4(w[0], w[1], w[2], w[3]);
+        *reinterpret_cast<int4 *>(lp) = make_int4(w[0], w[1], w[2], w[3]);
         if constexpr (RECON == 18) {
-            *reinterpret_cast<int4 *>(blk + ((size_t)Vh + i) * 16) = make_int4(w[4], w[5], w[6], w[7]);
-            *reinterpret_cast<int *>(blk + (size_t)2 * Vh * 16 + (size_t)i * 4) = w[8];
+            *reinterpret_cast<int4 *>(lp + TM_PLANE) = make_int4(w[4], w[5], w[6], w[7]);
+            *reinterpret_cast<int *>(lp + tail_off(2, 4, lane)) = w[8];
         } else {
-            *reinterpret_cast<int2 *>(blk + (size_t)Vh * 16 + (size_t)i * 8) = make_int2(w[4], w[5]);
+            *reinterpret_cast<int2 *>(lp + tail_off(1, 8, lane)) = make_int2(w[4], w[5]);
         }
     }
 }

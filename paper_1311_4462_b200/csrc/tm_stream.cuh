@@ -16,53 +16,42 @@ TM_DEV void prefetch_tile(const DslashArgs &a, int sites_per_block, int vblock)
 {
     if (a.pf_dist <= 0) return;
     const int Vh = a.Vh;
-    const long first_l = (long)(vblock + a.pf_dist) * sites_per_block;
+    const long first_l = (long)(vblock + a.pf_dist) * sites_per_block;      // a multiple of TM_TILE
     if (first_l >= Vh) return;
     const int first = (int)first_l;
-    const int n = min(sites_per_block, Vh - first);
-    constexpr int NP = link_planes<PREC, RECON>();
-    constexpr int NCH = PrecTraits<PREC>::NCH;
-    constexpr int NSP = NF * (NCH + (PREC == 2 ? 1 : 0));          // spinor planes (+ norm plane in half)
-    constexpr int NSEG = 8 * NP + NSP * (HAS_X ? 2 : 1);
-    const size_t blk = (size_t)RECON * PREC * Vh;
+    const int tiles = tm_tiles(Vh);
+    const int t0 = first >> TM_TILE_LOG;
+    const int nt = min((sites_per_block + TM_TILE - 1) >> TM_TILE_LOG, tiles - t0);
+    constexpr int STB = NF * spinor_tile_bytes(PREC);
+    constexpr int LTB = link_tile_bytes(PREC, RECON);
+    const size_t PB = (size_t)tiles * 4 * LTB;                               // one parity's gauge block
     const int st = a.Xh * a.Y * a.Z;
-    const size_t fl_bytes = (size_t)NCH * Vh * 16;
-    for (int s = threadIdx.x; s < NSEG; s += blockDim.x) {
-        if (s < 8 * NP) {
-            const int dir = s / NP, plane = s - dir * NP, mu = dir & 3;
-            const bool fwd = dir < 4;
-            const int w = link_plane_width<PREC, RECON>(plane);
-            int idx = first, cnt = n;
-            if (!fwd) {                                              // U_mu(x - mu) lives at the neighbour's index
-                idx = first - (mu == 0 ? 0 : mu == 1 ? a.Xh : mu == 2 ? a.Xh * a.Y : st);
-                if (idx < 0) idx += Vh;
-                idx &= ~3;
-                cnt = min(n, Vh - idx);
-            }
-            const char *base = static_cast<const char *>(a.gauge) + (size_t)(fwd ? a.parity : 1 - a.parity) * 4 * blk +
-                               (size_t)mu * blk + (size_t)link_plane_offset<PREC, RECON>(plane) * Vh;
-            prefetch_l2(base + (size_t)idx * w, (unsigned)(cnt * w));
-        } else {
-            int r = s - 8 * NP;
-            const bool isx = r >= NSP;
-            if (isx) r -= NSP;
-            const char *fb = static_cast<const char *>(isx ? a.x : a.in);
-            int idx = first;
-            if (!isx) {                                              // first touch: the forward time hop
-                idx = first + st;
-                if (idx >= Vh) idx -= Vh;
-            }
-            const int cnt = min(n, Vh - idx);
-            const int f = r / (NSP / NF), k = r % (NSP / NF);
-            if (k < NCH) prefetch_l2(fb + f * fl_bytes + ((size_t)k * Vh + idx) * 16, (unsigned)(cnt * 16));
-            else prefetch_l2(fb + NF * fl_bytes + ((size_t)f * Vh + idx) * 4, (unsigned)(cnt * 4));
+    const int nseg = 3 + 4 * (nt + 1);
+    for (int s = threadIdx.x; s < nseg; s += blockDim.x) {
+        if (s == 0) {                                    // forward links: the block's own tiles, all four mu
+            prefetch_l2(static_cast<const char *>(a.gauge) + (size_t)a.parity * PB + (size_t)t0 * 4 * LTB, (unsigned)(nt * 4 * LTB));
+        } else if (s == 1) {                             // input spinor: first touched by the forward time hop
+            int idx = first + st;
+            if (idx >= Vh) idx -= Vh;
+            const int ti = idx >> TM_TILE_LOG;
+            prefetch_l2(static_cast<const char *>(a.in) + (size_t)ti * STB, (unsigned)(min(nt + 1, tiles - ti) * STB));
+        } else if (s == 2) {
+            if (HAS_X) prefetch_l2(static_cast<const char *>(a.x) + (size_t)t0 * STB, (unsigned)(nt * STB));
+        } else {                                         // backward links U_mu(x - mu): the neighbour's tiles, one mu each
+            const int r = s - 3, mu = r & 3, j = r >> 2;
+            int idx = first - (mu == 0 ? 0 : mu == 1 ? a.Xh : mu == 2 ? a.Xh * a.Y : st);
+            if (idx < 0) idx += Vh;
+            const int tb = (idx >> TM_TILE_LOG) + j;
+            if (tb < tiles)
+                prefetch_l2(static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * PB + ((size_t)tb * 4 + mu) * LTB, (unsigned)LTB);
         }
     }
 }
 
 // ---- staging the link stream through shared memory with cp.async (LDGSTS) ------------------------------------
 // Every thread starts the copy of all 8 links of its site before it does anything else, one commit group per hop,
-// into [hop][plane][thread] slots (16-byte slots of consecutive threads are consecutive: conflict-free LDS.128).
+// into the slot [hop][warp] of RECON * PREC * 32 bytes that has the tile shape [plane][32 lanes] (conflict-free
+// LDS.128, and load_link reads it with the same offsets as a tile in global memory).
 // The bytes are then in flight without holding registers; hop h waits for group h only (cp.async.wait_group 7-h).
 // A thread reads back only what it copied itself, so no block barrier is needed.
 TM_DEV unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -75,45 +64,22 @@ template <int W> TM_DEV void cp_async(void *smem, const void *g)
 TM_DEV void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> TM_DEV void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-template <int PREC, int RECON>
-TM_DEV void stage_link_nc(char *sm_hop, const char *gauge_blk, int Vh, int idx, int nt, int tid)     // no commit
-{
-    constexpr int NP = link_planes<PREC, RECON>();
-#pragma unroll
-    for (int p = 0; p < NP; p++) {
-        const int w = link_plane_width<PREC, RECON>(p), o = link_plane_offset<PREC, RECON>(p);
-        char *dst = sm_hop + (size_t)o * nt + (size_t)tid * w;
-        const char *src = gauge_blk + (size_t)o * Vh + (size_t)idx * w;
-        if (w == 16) cp_async<16>(dst, src);
-        else if (w == 8) cp_async<8>(dst, src);
-        else cp_async<4>(dst, src);
-    }
-}
-template <int PREC, int RECON>
-TM_DEV void stage_link(char *sm_hop, const char *gauge_blk, int Vh, int idx, int nt, int tid)
-{
-    stage_link_nc<PREC, RECON>(sm_hop, gauge_blk, Vh, idx, nt, tid);
-    cp_async_commit();
-}
-
-// Where hop h finds its link: the staged [plane][thread] slots of the block, or the gauge block in global memory.
 extern __shared__ __align__(16) char tm_smem[];
-struct LinkSrc {
-    const char *base;
-    int stride;     // sites per plane
-    int idx;
-};
-template <bool STG> TM_DEV LinkSrc link_src(int h, int link_bytes, const char *gauge_blk, int Vh, int gidx)
+// the thread's pointer into the staged copy of hop h (plays the role of the link's site pointer)
+template <int PREC, int RECON> TM_DEV char *stage_slot(int h)
 {
-    LinkSrc L;
-    if constexpr (STG) {
-        L.base = tm_smem + (size_t)h * link_bytes * blockDim.x;
-        L.stride = blockDim.x;
-        L.idx = threadIdx.x;
-    } else {
-        L.base = gauge_blk;
-        L.stride = Vh;
-        L.idx = gidx;
-    }
-    return L;
+    const int warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5, lane = threadIdx.x & 31;
+    return tm_smem + (size_t)(h * nwarps + warp) * link_tile_bytes(PREC, RECON) + lane * 16;
+}
+template <int PREC, int RECON>
+TM_DEV void stage_link(int h, const char *lp, int src_lane)      // src_lane = (index of the link's site) & 31
+{
+    constexpr int N16 = link_n16<PREC, RECON>(), TW = link_tailw<PREC, RECON>();
+    const int lane = threadIdx.x & 31;
+    char *dst = stage_slot<PREC, RECON>(h);
+#pragma unroll
+    for (int k = 0; k < N16; k++) cp_async<16>(dst + k * TM_PLANE, lp + k * TM_PLANE);
+    if constexpr (TW == 8) cp_async<8>(dst + tail_off(N16, 8, lane), lp + tail_off(N16, 8, src_lane));
+    if constexpr (TW == 4) cp_async<4>(dst + tail_off(N16, 4, lane), lp + tail_off(N16, 4, src_lane));
+    cp_async_commit();
 }
