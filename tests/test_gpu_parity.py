@@ -57,7 +57,8 @@ def bench_for(dims, kind, seed):
 
 # ---- T1: layouts round trip -----------------------------------------------------------------------
 
-@pytest.mark.parametrize("dims", [(4, 4, 4, 8), (4, 6, 8, 10)])
+# (6, 6, 6, 6): V/2 = 648 sites = 20.25 tiles of 32 (ragged last tile), X/2 = 3 (no power-of-two extents)
+@pytest.mark.parametrize("dims", [(4, 4, 4, 8), (4, 6, 8, 10), (6, 6, 6, 6)])
 @pytest.mark.parametrize("nf", [1, 2])
 def test_t1_spinor_pack_unpack_round_trip(dims, nf):
     lat = tm.Lattice(dims)
@@ -89,7 +90,8 @@ def test_t1_spinor_pack_unpack_round_trip(dims, nf):
 
 # ---- T2: every kernel variant vs the oracle -------------------------------------------------------
 
-@pytest.mark.parametrize("dims,kind", [((4, 4, 4, 8), "haar"), ((4, 6, 8, 10), "near_identity"), ((8, 4, 6, 4), "haar")])
+@pytest.mark.parametrize("dims,kind", [((4, 4, 4, 8), "haar"), ((4, 6, 8, 10), "near_identity"), ((8, 4, 6, 4), "haar"),
+                                       ((6, 6, 6, 6), "haar")])
 @pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
 @pytest.mark.parametrize("variant", VARIANTS, ids=[v[0] for v in VARIANTS])
 def test_t2_every_kernel_variant_matches_oracle(dims, kind, kw, variant):
