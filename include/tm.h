@@ -57,7 +57,10 @@ typedef enum {                       /* the fused kernels of PAPER.md:68 (sectio
     TM_TWIST_INV_DSLASH = 0,         /* A      : out_p = R^-1 D_hop in                                   */
     TM_TWIST_INV_DSLASH_XPAY = 1,    /* A-xpay : out_p = x_p - kappa^2 R^-1 D_hop in                     */
     TM_DSLASH_TWIST_XPAY = 2,        /* B      : out_p = R x_p - kappa^2 D_hop in                        */
-    TM_RECONSTRUCT = 3               /* REC    : out_p = R^-1 (x_p + kappa D_hop in)     (Eq. 2.4)       */
+    TM_RECONSTRUCT = 3,              /* REC    : out_p = R^-1 (x_p + kappa D_hop in)     (Eq. 2.4)       */
+    /* the same hopping kernels with no twist (R = 1): the pieces of M^_sym^dag and of the right-hand sides */
+    TM_DSLASH_XPAY = 4,              /*          out_p = x_p - kappa^2 D_hop in                          */
+    TM_DSLASH_AXPY = 5               /*          out_p = x_p + kappa D_hop in                            */
 } tm_kernel_type;
 /* dagger != 0: D_hop -> D_hop^dag (projectors swapped) and R -> R^dag (a -> -a), order kept.            */
 
@@ -115,10 +118,23 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
 
 /* LHS of Eq. 2.2 (ASYM: out_e = (R_ee - kappa^2 D_eo R_oo^-1 D_oe) in_e) or Eq. 2.3 (SYM:
  * out_e = (1 - kappa^2 R_ee^-1 D_eo R_oo^-1 D_oe) in_e): two launches, tmp_o is the odd
- * intermediate R_oo^-1 D_oe in_e.  dagger: the same two launches with the daggered kernels -- the exact
- * adjoint for ASYM; SYM + dagger returns TM_ERR_UNSUPPORTED.  Asynchronous. */
+ * intermediate R_oo^-1 D_oe in_e.  dagger: the exact adjoint.  ASYM: the same two launches with the daggered
+ * kernels.  SYM: M^_sym^dag = 1 - kappa^2 D^dag_eo R^dag^-1_oo D^dag_oe R^dag^-1_ee (C7) = the local twist
+ * R^dag^-1 (into out_e, used as scratch: out_e must not alias in_e, TM_ERR_ALIAS), kernel A^dag, and the plain
+ * xpay kernel: three launches.  Asynchronous. */
 int tm_mat_pc(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p,
               tm_matpc type, int dagger);
+
+/* The local twist alone, site by site on one parity field ("local operators"):
+ * out = R in (inverse = 0) or R^-1 in (inverse = 1); dagger != 0: R -> R^dag (a -> -a).  out may be in itself
+ * (in place) but must not partially overlap it.  TM_ERR_PARAM if R is singular.  Asynchronous. */
+int tm_twist_apply(tm_field *out, const tm_field *in, const tm_params *p, int inverse, int dagger);
+
+/* Right-hand side of Eq. 2.2 (ASYM: rhs_e = b_e + kappa D_eo R_oo^-1 b_o) or Eq. 2.3 (SYM: rhs_e = R_ee^-1 (b_e +
+ * kappa D_eo R_oo^-1 b_o)), PAPER.md:60-64 in the reading C4 of DESIGN.md.  tmp_o receives R_oo^-1 b_o; it must not
+ * alias b_e or rhs_e (TM_ERR_ALIAS); rhs_e may alias b_e.  Two launches.  Asynchronous. */
+int tm_prepare_rhs(tm_field *rhs_e, const tm_field *b_e, const tm_field *b_o, tm_field *tmp_o, const tm_gauge *g,
+                   const tm_params *p, tm_matpc type);
 
 /* Eq. 2.4 (reading C4): psi_o = R_oo^-1 (b_o + kappa D_oe psi_e).  psi_o may alias b_o. */
 int tm_reconstruct_odd(tm_field *psi_o, const tm_field *psi_e, const tm_field *b_o, const tm_gauge *g,

@@ -195,3 +195,40 @@ def reconstruct_odd(psi_e, b_o, gauge, p):
     _check(lib().tmo_reconstruct_odd(_ptr(out), _ptr(psi_e), _ptr(b_o), _ptr(gauge), ctypes.byref(p)),
            "reconstruct_odd")
     return out
+
+
+# ---- compositions of the primitives above (plain definitions; no new arithmetic) ---------------------------
+
+def _mask(a, p, parity):
+    """Zero the sites of the other parity (full-lattice array in, full-lattice array out)."""
+    par = site_parity([p.X[k] for k in range(4)])
+    out = np.array(a, dtype=np.complex128, copy=True)
+    out[:, par != parity] = 0
+    return out
+
+
+def hop_xpay(inp, x, gauge, p, parity, dagger, coeff):
+    """out_p = x_p + coeff (D_hop in)_p  with no twist: the plain forms the product exposes as TM_DSLASH_XPAY
+    (coeff = -kappa^2) and TM_DSLASH_AXPY (coeff = +kappa)."""
+    return _mask(x, p, parity) + coeff * _mask(dhop(inp, gauge, p, dagger), p, parity)
+
+
+def matpc_adjoint(inp, gauge, p, matpc_type):
+    """The adjoint of the even-even operators written out from D_hop^dag and R^dag (C7):
+    ASYM: (R_ee^dag - kappa^2 D_eo^dag R_oo^dag^-1 D_oe^dag) in_e
+    SYM : (1 - kappa^2 D_eo^dag R_oo^dag^-1 D_oe^dag R_ee^dag^-1) in_e        (adjoint taken term by term)."""
+    in_e = _mask(inp, p, EVEN)
+    k2 = p.kappa * p.kappa
+    if matpc_type == ASYM:
+        t_o = twist(_mask(dhop(in_e, gauge, p, 1), p, ODD), p, 1, 1)
+        return twist(in_e, p, 0, 1) - k2 * _mask(dhop(t_o, gauge, p, 1), p, EVEN)
+    y_e = twist(in_e, p, 1, 1)
+    t_o = twist(_mask(dhop(y_e, gauge, p, 1), p, ODD), p, 1, 1)
+    return in_e - k2 * _mask(dhop(t_o, gauge, p, 1), p, EVEN)
+
+
+def prepare_rhs(b, gauge, p, matpc_type):
+    """Right-hand side of Eq. (2.2) / (2.3) in the reading C4: b_e + kappa D_eo R_oo^-1 b_o, times R_ee^-1 for SYM."""
+    t_o = twist(_mask(b, p, ODD), p, 1, 0)
+    r = _mask(b, p, EVEN) + p.kappa * _mask(dhop(t_o, gauge, p, 0), p, EVEN)
+    return r if matpc_type == ASYM else twist(r, p, 1, 0)

@@ -25,12 +25,14 @@ TM_DOUBLE, TM_SINGLE, TM_HALF = 8, 4, 2
 TM_RECON_18, TM_RECON_12 = 18, 12
 TM_EVEN, TM_ODD = 0, 1
 TM_TWIST_INV_DSLASH, TM_TWIST_INV_DSLASH_XPAY, TM_DSLASH_TWIST_XPAY, TM_RECONSTRUCT = 0, 1, 2, 3
+TM_DSLASH_XPAY, TM_DSLASH_AXPY = 4, 5
 TM_MATPC_ASYM, TM_MATPC_SYM = 0, 1
 
 EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
     "tm_field_device_ptr", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb",
-    "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_last_error",
+    "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_twist_apply",
+    "tm_prepare_rhs", "tm_last_error",
     "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_set_tuning", "tm_timing_enable", "tm_timing_read",
 ]
 
@@ -84,6 +86,8 @@ def lib():
     L.tm_dslash_apply.argtypes = [vp, vp, vp, vp, pp, i, i, i, i]
     L.tm_mat_pc.argtypes = [vp, vp, vp, vp, pp, i, i]
     L.tm_reconstruct_odd.argtypes = [vp, vp, vp, vp, pp]
+    L.tm_twist_apply.argtypes = [vp, vp, pp, i, i]
+    L.tm_prepare_rhs.argtypes = [vp, vp, vp, vp, vp, pp, i]
     L.tm_last_error.restype = ctypes.c_char_p
     L.tm_launch_count.argtypes = [vp]
     L.tm_launch_count.restype = ctypes.c_long
@@ -187,6 +191,14 @@ def tm_mat_pc(out_e, in_e, tmp_o, gauge, p, matpc_type, dagger=0):
 
 def tm_reconstruct_odd(psi_o, psi_e, b_o, gauge, p):
     _check(lib().tm_reconstruct_odd(psi_o, psi_e, b_o, gauge, ctypes.byref(p)))
+
+
+def tm_twist_apply(out, inp, p, inverse=0, dagger=0):
+    _check(lib().tm_twist_apply(out, inp, ctypes.byref(p), int(inverse), int(dagger)))
+
+
+def tm_prepare_rhs(rhs_e, b_e, b_o, tmp_o, gauge, p, matpc_type):
+    _check(lib().tm_prepare_rhs(rhs_e, b_e, b_o, tmp_o, gauge, ctypes.byref(p), int(matpc_type)))
 
 
 def tm_launch_count(ctx):
@@ -320,3 +332,11 @@ def mat_pc(out_e, in_e, tmp_o, gauge, p, matpc_type, dagger=0):
 
 def reconstruct_odd(psi_o, psi_e, b_o, gauge, p):
     tm_reconstruct_odd(psi_o.h, psi_e.h, b_o.h, gauge.h, p)
+
+
+def twist_apply(out, inp, p, inverse=0, dagger=0):
+    tm_twist_apply(out.h, inp.h, p, inverse, dagger)
+
+
+def prepare_rhs(rhs_e, b_e, b_o, tmp_o, gauge, p, matpc_type):
+    tm_prepare_rhs(rhs_e.h, b_e.h, b_o.h, tmp_o.h, gauge.h, p, matpc_type)

@@ -105,7 +105,9 @@ int make_coeffs(const tm_params *p, int nf, int dagger, int kt, Coeffs *c)
     double a = 2.0 * p->kappa * p->mu, b = 2.0 * p->kappa * p->epsilon;
     if (dagger) a = -a;
     if (nf == 1) { a *= (double)p->twist_flavor; b = 0.0; }
-    if (kt == TM_DSLASH_TWIST_XPAY) {
+    if (kt == TM_DSLASH_XPAY || kt == TM_DSLASH_AXPY) {       // no twist: the B / REC kernels with R = 1
+        c->alpha = 0.0; c->beta = 0.0; c->scale = 1.0;
+    } else if (kt == TM_DSLASH_TWIST_XPAY) {
         c->alpha = a; c->beta = b; c->scale = 1.0;
     } else {
         const double den = 1.0 + a * a - b * b;
@@ -361,7 +363,9 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
 {
     if (!out || !in || !g || !p) return fail(TM_ERR_ARG, "tm_dslash_apply: NULL argument");
     if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
-    if ((int)kt < 0 || (int)kt > 3) return fail(TM_ERR_ARG, "bad kernel type %d", (int)kt);
+    if ((int)kt < 0 || (int)kt > 5) return fail(TM_ERR_ARG, "bad kernel type %d", (int)kt);
+    // out = x - kappa^2 D in  and  out = x + kappa D in  run the B / REC kernels with the identity twist
+    const int kcode = kt == TM_DSLASH_XPAY ? (int)TM_DSLASH_TWIST_XPAY : kt == TM_DSLASH_AXPY ? (int)TM_RECONSTRUCT : (int)kt;
     if (kt != TM_TWIST_INV_DSLASH && !x) return fail(TM_ERR_ARG, "kernel type %d needs x", (int)kt);
     tm_ctx *c = out->ctx;
     if (in->ctx != c || g->ctx != c || (x && x->ctx != c)) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
@@ -391,7 +395,7 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     // path 0: fp32 / half run the packed-FP32 kernels, fp64 the scalar kernel; path 1 forces the scalar kernel
     const TmKernelEntry *tab = (c->path == 0 && (int)prec != TM_DOUBLE) ? tm_f2_table((int)prec, out->nf)
                                                                        : tm_generic_table((int)prec, out->nf);
-    const TmKernelEntry &k = tab[(((g->recon == 18 ? 0 : 1) * 4 + (int)kt) * 2 + (dagger ? 1 : 0)) * 2 + stage];
+    const TmKernelEntry &k = tab[(((g->recon == 18 ? 0 : 1) * 4 + kcode) * 2 + (dagger ? 1 : 0)) * 2 + stage];
     cudaError_t e;
     if (c->timing) {
         tm_ctx::TimedLaunch t;
@@ -416,16 +420,53 @@ int tm_mat_pc(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_g
 {
     if (!out_e || !in_e || !tmp_o || !g || !p) return fail(TM_ERR_ARG, "tm_mat_pc: NULL argument");
     if (type != TM_MATPC_ASYM && type != TM_MATPC_SYM) return fail(TM_ERR_ARG, "bad matpc type %d", (int)type);
-    if (type == TM_MATPC_SYM && dagger)
-        return fail(TM_ERR_UNSUPPORTED, "SYM dagger needs the D R^-1 kernel ordering (DESIGN.md C7, NEXT-1)");
     if (overlap(tmp_o, in_e) || overlap(tmp_o, out_e)) return fail(TM_ERR_ALIAS, "tmp_o aliases in_e or out_e");
     const tm_precision prec = (tm_precision)out_e->prec;
+    if (type == TM_MATPC_SYM && dagger) {
+        // M^_sym^dag = 1 - kappa^2 D^dag_eo R^dag^-1_oo D^dag_oe R^dag^-1_ee  (C7): the twist stands in FRONT of
+        // the first hopping term, so it runs as the local kernel, with out_e as scratch.
+        if (overlap(out_e, in_e)) return fail(TM_ERR_ALIAS, "out_e aliases in_e (SYM dagger uses out_e as scratch)");
+        int rc = tm_twist_apply(out_e, in_e, p, 1, 1);                                             // out_e = R^dag^-1 in_e
+        if (!rc) rc = tm_dslash_apply(tmp_o, out_e, nullptr, g, p, TM_ODD, 1, TM_TWIST_INV_DSLASH, prec);   // tmp_o = R^dag^-1 D^dag out_e
+        if (!rc) rc = tm_dslash_apply(out_e, tmp_o, in_e, g, p, TM_EVEN, 1, TM_DSLASH_XPAY, prec);           // out_e = in_e - kappa^2 D^dag tmp_o
+        return rc;
+    }
     // tmp_o = R_oo^-1 D_oe in_e
     int rc = tm_dslash_apply(tmp_o, in_e, nullptr, g, p, TM_ODD, dagger, TM_TWIST_INV_DSLASH, prec);
     if (rc) return rc;
     // ASYM: out_e = R_ee in_e - kappa^2 D_eo tmp_o ;  SYM: out_e = in_e - kappa^2 R_ee^-1 D_eo tmp_o
     return tm_dslash_apply(out_e, tmp_o, in_e, g, p, TM_EVEN, dagger,
                            type == TM_MATPC_ASYM ? TM_DSLASH_TWIST_XPAY : TM_TWIST_INV_DSLASH_XPAY, prec);
+}
+
+int tm_twist_apply(tm_field *out, const tm_field *in, const tm_params *p, int inverse, int dagger)
+{
+    if (!out || !in || !p) return fail(TM_ERR_ARG, "tm_twist_apply: NULL argument");
+    tm_ctx *c = out->ctx;
+    if (in->ctx != c) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
+    if (in->prec != out->prec || in->nf != out->nf) return fail(TM_ERR_MISMATCH, "precision or flavor count mismatch");
+    if (overlap(out, in) && out->ptr != in->ptr) return fail(TM_ERR_ALIAS, "out partially overlaps in");
+    Coeffs co;
+    int rc = make_coeffs(p, out->nf, dagger ? 1 : 0, inverse ? (int)TM_TWIST_INV_DSLASH : (int)TM_DSLASH_TWIST_XPAY, &co);
+    if (rc) return rc;
+    cudaError_t e = tm_launch_twist(out, in, co.alpha, co.beta, co.scale, c->stream);
+    if (e != cudaSuccess) return cuda_fail(e, "tm_twist_kernel");
+    c->launches++;
+    c->last_kernel = "twist";
+    return TM_OK;
+}
+
+int tm_prepare_rhs(tm_field *rhs_e, const tm_field *b_e, const tm_field *b_o, tm_field *tmp_o, const tm_gauge *g,
+                   const tm_params *p, tm_matpc type)
+{
+    if (!rhs_e || !b_e || !b_o || !tmp_o || !g || !p) return fail(TM_ERR_ARG, "tm_prepare_rhs: NULL argument");
+    if (type != TM_MATPC_ASYM && type != TM_MATPC_SYM) return fail(TM_ERR_ARG, "bad matpc type %d", (int)type);
+    if (overlap(tmp_o, b_e) || overlap(tmp_o, rhs_e)) return fail(TM_ERR_ALIAS, "tmp_o aliases b_e or rhs_e");
+    const tm_precision prec = (tm_precision)rhs_e->prec;
+    int rc = tm_twist_apply(tmp_o, b_o, p, 1, 0);                                     // tmp_o = R_oo^-1 b_o
+    if (rc) return rc;
+    // Eq. 2.2: b_e + kappa D_eo tmp_o ;  Eq. 2.3: R_ee^-1 (b_e + kappa D_eo tmp_o)   (reading C4)
+    return tm_dslash_apply(rhs_e, tmp_o, b_e, g, p, TM_EVEN, 0, type == TM_MATPC_ASYM ? TM_DSLASH_AXPY : TM_RECONSTRUCT, prec);
 }
 
 int tm_reconstruct_odd(tm_field *psi_o, const tm_field *psi_e, const tm_field *b_o, const tm_gauge *g, const tm_params *p)

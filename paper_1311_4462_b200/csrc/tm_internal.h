@@ -111,6 +111,9 @@ struct TmKernelEntry {
 // index: [recon18?0:1][kt 0..3][dagger 0..1][staged 0..1]
 const TmKernelEntry *tm_generic_table(int prec, int nf);
 
+// out = scale (1 + i alpha gamma5 tau3 + beta tau1) in, site by site (tm_twist.cu)
+cudaError_t tm_launch_twist(const tm_field *out, const tm_field *in, double alpha, double beta, double scale, cudaStream_t s);
+
 // pack / unpack (tm_pack.cu)
 cudaError_t tm_pack_spinor(const tm_field *f, int parity, const double *dev_src, bool src_is_cb, cudaStream_t s);
 cudaError_t tm_unpack_spinor(const tm_field *f, int parity, double *dev_dst, bool dst_is_cb, cudaStream_t s);

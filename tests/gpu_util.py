@@ -52,3 +52,21 @@ class Bench:
         tm.reconstruct_odd(fo, fe, fb, self.gauge(prec, recon), p)
         lat.sync()
         return fo.download(tm.TM_ODD)
+
+    def twist(self, inp, parity, p, inverse, dagger, prec, nf, in_place=False):
+        lat = self.lat
+        fin = lat.field(prec, nf).upload(parity, inp)
+        fout = fin if in_place else lat.field(prec, nf)
+        tm.twist_apply(fout, fin, p, inverse, dagger)
+        lat.sync()
+        return fout.download(parity)
+
+    def prepare_rhs(self, b, p, typ, prec, recon, nf, alias=False):
+        lat = self.lat
+        fbe = lat.field(prec, nf).upload(tm.TM_EVEN, b)
+        fbo = lat.field(prec, nf).upload(tm.TM_ODD, b)
+        ftmp = lat.field(prec, nf)
+        frhs = fbe if alias else lat.field(prec, nf)
+        tm.prepare_rhs(frhs, fbe, fbo, ftmp, self.gauge(prec, recon), p, typ)
+        lat.sync()
+        return frhs.download(tm.TM_EVEN)

@@ -172,6 +172,75 @@ def test_t3b_config1_solve_check():
         assert rel_l2(rec, psi_o) <= 1e-12
 
 
+# ---- T3c: the local twist, the twist-free hopping forms, the adjoint of SYM, right-hand sides ----------
+
+@pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
+def test_t3c_twist_apply_matches_oracle(kw):
+    dims = (6, 6, 6, 6)
+    nf = nf_of(kw)
+    bench = bench_for(dims, "haar", 1)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    for parity in (0, 1):
+        v = si.mask_parity(si.spinor_field(dims, nf, 21), dims, parity)
+        for inverse, dagger in itertools.product((0, 1), (0, 1)):
+            want = oracle.twist(v, po, inverse, dagger)
+            for prec in PRECS:
+                assert rel_l2(bench.twist(v, parity, pg, inverse, dagger, prec, nf), want) <= TOL[prec]
+            assert rel_l2(bench.twist(v, parity, pg, inverse, dagger, tm.TM_DOUBLE, nf, in_place=True), want) <= 1e-12
+
+
+@pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
+def test_t3d_plain_xpay_axpy_kernels_match_oracle(kw):
+    dims = (4, 6, 8, 10)
+    nf = nf_of(kw)
+    bench = bench_for(dims, "near_identity", 1)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    for parity, dagger in itertools.product((0, 1), (0, 1)):
+        inp = si.mask_parity(si.spinor_field(dims, nf, 22), dims, 1 - parity)
+        x = si.mask_parity(si.spinor_field(dims, nf, 23), dims, parity)
+        for kt, coeff in ((tm.TM_DSLASH_XPAY, -KAPPA * KAPPA), (tm.TM_DSLASH_AXPY, KAPPA)):
+            want = oracle.hop_xpay(inp, x, bench.U, po, parity, dagger, coeff)
+            for prec, recon in itertools.product(PRECS, RECONS):
+                got = bench.kernel(inp, x, pg, parity, dagger, kt, prec, recon, nf)
+                assert rel_l2(got, want) <= TOL[prec], (PREC_NAME[prec], recon, parity, dagger, kt)
+
+
+@pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
+def test_t3e_sym_dagger_is_the_adjoint_and_rhs_preparation(kw):
+    dims = (4, 4, 4, 8)
+    nf = nf_of(kw)
+    bench = bench_for(dims, "haar", 1)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    phi = si.mask_parity(si.spinor_field(dims, nf, 24), dims, 0)
+    b = si.spinor_field(dims, nf, 25)
+    for prec, recon in itertools.product(PRECS, RECONS):
+        for typ in (tm.TM_MATPC_ASYM, tm.TM_MATPC_SYM):
+            want = oracle.matpc_adjoint(phi, bench.U, po, typ)
+            assert rel_l2(bench.matpc(phi, pg, typ, 1, prec, recon, nf), want) <= TOL[prec], (PREC_NAME[prec], recon, typ)
+            want = oracle.prepare_rhs(b, bench.U, po, typ)
+            assert rel_l2(bench.prepare_rhs(b, pg, typ, prec, recon, nf), want) <= TOL[prec], (PREC_NAME[prec], recon, typ)
+        assert rel_l2(bench.prepare_rhs(b, pg, tm.TM_MATPC_SYM, prec, recon, nf, alias=True),
+                      oracle.prepare_rhs(b, bench.U, po, tm.TM_MATPC_SYM)) <= TOL[prec]
+
+
+def test_t3f_full_solve_pipeline_on_gpu():
+    """b = M psi (oracle, full operator); on the GPU: rhs = tm_prepare_rhs(b), then M^ psi_e == rhs for both
+    preconditionings and tm_reconstruct_odd(psi_e, b_o) == psi_o.  fp64, non-degenerate doublet, 4x6x8x10."""
+    dims = (4, 6, 8, 10)
+    kw = FLAVORS[2]
+    bench = bench_for(dims, "near_identity", 1)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    psi = si.spinor_field(dims, 2, 26)
+    b = oracle.mat(psi, bench.U, po)
+    psi_e, psi_o = si.mask_parity(psi, dims, 0), si.mask_parity(psi, dims, 1)
+    for typ in (tm.TM_MATPC_ASYM, tm.TM_MATPC_SYM):
+        rhs = bench.prepare_rhs(b, pg, typ, tm.TM_DOUBLE, tm.TM_RECON_12, 2)
+        lhs = bench.matpc(psi_e, pg, typ, 0, tm.TM_DOUBLE, tm.TM_RECON_12, 2)
+        assert rel_l2(lhs, rhs) <= 1e-12
+    rec = bench.reconstruct_odd(psi_e, si.mask_parity(b, dims, 1), pg, tm.TM_DOUBLE, tm.TM_RECON_12, 2)
+    assert rel_l2(rec, psi_o) <= 1e-12
+
+
 # ---- T4: GPU-side properties that need no oracle --------------------------------------------------
 
 @pytest.mark.parametrize("kw", [FLAVORS[0], FLAVORS[2]], ids=["deg", "ndeg"])
@@ -216,7 +285,12 @@ def test_t6_error_paths():
     sing = tm.params(KAPPA, 0.0, epsilon=1.0 / (2 * KAPPA), twist_flavor=0)     # 1 + a^2 - b^2 = 0
     t2, t3 = lat.field(tm.TM_SINGLE, 2), lat.field(tm.TM_SINGLE, 2)
     assert status(lambda: tm.dslash_apply(t2, t3, None, g, sing, 0, 0, 0)) == tm.TM_ERR_PARAM
-    assert status(lambda: tm.mat_pc(a, b, c, g, p, tm.TM_MATPC_SYM, 1)) == tm.TM_ERR_UNSUPPORTED
+    assert status(lambda: tm.mat_pc(a, a, c, g, p, tm.TM_MATPC_SYM, 1)) == tm.TM_ERR_ALIAS          # out_e is scratch
+    assert status(lambda: tm.twist_apply(t2, t3, sing, 1, 0)) == tm.TM_ERR_PARAM
+    assert status(lambda: tm.twist_apply(a, t3, p, 0, 0)) == tm.TM_ERR_MISMATCH
+    assert status(lambda: tm.dslash_apply(a, b, None, g, p, 0, 0, tm.TM_DSLASH_XPAY)) == tm.TM_ERR_ARG   # needs x
+    assert status(lambda: tm.dslash_apply(a, b, c, g, p, 0, 0, 6)) == tm.TM_ERR_ARG
+    assert status(lambda: tm.prepare_rhs(a, b, c, b, g, p, tm.TM_MATPC_ASYM)) == tm.TM_ERR_ALIAS
     assert status(lambda: tm.mat_pc(a, b, b, g, p, tm.TM_MATPC_ASYM, 0)) == tm.TM_ERR_ALIAS
     assert status(lambda: tm.tm_init((4, 4, 4, 7))) == tm.TM_ERR_DIMS
     assert status(lambda: tm.tm_init((2, 4, 4, 8))) == tm.TM_ERR_DIMS

@@ -313,6 +313,52 @@ def test_p6_composite_adjoint_and_dagger_identities(kw):
         assert rel(d, e) < 1e-13
 
 
+# ---- P13 / P14: the adjoint and right-hand-side compositions (NEXT-1 rows) -------------------------------
+
+@pytest.mark.parametrize("kw", PARAMS)
+@pytest.mark.parametrize("typ", [0, 1])
+def test_p13_matpc_adjoint_is_the_adjoint(kw, typ):
+    dims = (4, 4, 4, 6)
+    nf = nf_of(kw)
+    p = oracle.params(dims, KAPPA, **kw)
+    U = si.gauge_field(dims, 61, "haar")
+    psi = si.mask_parity(si.spinor_field(dims, nf, 62), dims, 0)
+    phi = si.mask_parity(si.spinor_field(dims, nf, 63), dims, 0)
+    adj = oracle.matpc_adjoint(phi, U, p, typ)
+    assert np.abs(si.mask_parity(adj, dims, 1)).max() == 0
+    assert abs(ip(phi, oracle.matpc(psi, U, p, typ)) - ip(adj, psi)) < 1e-9 * abs(ip(phi, phi))
+    if typ == oracle.ASYM:      # C7: the daggered two-launch composite is this adjoint
+        assert rel(oracle.matpc(phi, U, p, oracle.ASYM, dagger=1), adj) < 1e-13
+    else:                       # C7: it is NOT for SYM (the twist changes sides) ...
+        assert rel(oracle.matpc(phi, U, p, oracle.SYM, dagger=1), adj) > 1e-4      # 7e-4 already at mu = 0.004
+        # ... but conjugating with R^dag relates the two
+        conj = oracle.twist(oracle.matpc(oracle.twist(phi, p, 1, 1), U, p, oracle.SYM, dagger=1), p, 0, 1)
+        assert rel(conj, adj) < 1e-12
+
+
+@pytest.mark.parametrize("kw", PARAMS)
+def test_p14_rhs_preparation_against_the_full_operator(kw):
+    """b = M psi with the FULL operator (pinned by P1-P3); then M^ psi_e must equal the prepared right-hand side and
+    Eq. (2.4) must give back psi_o: ties prepare_rhs, matpc and reconstruct_odd to oracle.mat on a lattice with
+    every extent different."""
+    dims = (4, 6, 8, 10)
+    nf = nf_of(kw)
+    p = oracle.params(dims, KAPPA, **kw)
+    U = si.gauge_field(dims, 71, "near_identity")
+    psi = si.spinor_field(dims, nf, 72)
+    b = oracle.mat(psi, U, p)
+    psi_e, psi_o = si.mask_parity(psi, dims, 0), si.mask_parity(psi, dims, 1)
+    for typ in (oracle.ASYM, oracle.SYM):
+        rhs = oracle.prepare_rhs(b, U, p, typ)
+        assert np.abs(si.mask_parity(rhs, dims, 1)).max() == 0
+        assert rel(oracle.matpc(psi_e, U, p, typ), rhs) < 1e-12
+    assert rel(oracle.reconstruct_odd(psi_e, si.mask_parity(b, dims, 1), U, p), psi_o) < 1e-12
+    # the plain xpay / axpy forms are what their names say
+    x = si.mask_parity(si.spinor_field(dims, nf, 73), dims, 0)
+    got = oracle.hop_xpay(psi_o, x, U, p, 0, 0, -KAPPA * KAPPA)
+    assert rel(got, x - KAPPA * KAPPA * si.mask_parity(oracle.dhop(psi_o, U, p), dims, 0)) < 1e-14
+
+
 # ---- P7 / P8: special cases -----------------------------------------------------------------------
 
 def test_p7_wilson_and_decoupled_flavors():
