@@ -140,6 +140,38 @@ int tm_prepare_rhs(tm_field *rhs_e, const tm_field *b_e, const tm_field *b_o, tm
 int tm_reconstruct_odd(tm_field *psi_o, const tm_field *psi_e, const tm_field *b_o, const tm_gauge *g,
                        const tm_params *p);
 
+/* ---- vector operations and the mixed-precision CG --- */
+/* z = a x + b y on single-parity fields (y may be NULL: z = a x).  z may be x or y itself.  Precisions may differ in
+ * these combinations: all equal; z double, x single / half, y double; z single / half, x double, y NULL or like z
+ * (anything else: TM_ERR_UNSUPPORTED).  Half operands are dequantised / requantised site by site.  Asynchronous. */
+int tm_field_axpby(tm_field *z, double a, const tm_field *x, double b, const tm_field *y);
+/* *result (HOST) = Re <x, y> = sum over sites, flavors, spin, color of re x re y + im x im y, accumulated in double in
+ * a fixed order (deterministic).  x = y gives |x|^2.  Synchronises the context stream. */
+int tm_field_redot(const tm_field *x, const tm_field *y, double *result);
+
+typedef struct {
+    double tol;                    /* stop when |b - A x| / |b| <= tol, the residual formed in double                 */
+    int max_iter;                  /* cap on the total number of inner CG iterations                                  */
+    tm_precision sloppy_precision; /* precision of the inner CG (TM_DOUBLE: plain double CG)                          */
+    double delta;                  /* each inner solve reduces its residual by this factor before the next double
+                                      precision residual (0 < delta < 1; e.g. 0.1 for single, 0.3 for half)          */
+} tm_cg_params;
+typedef struct {
+    int iterations;                /* inner CG iterations (applications of A = M^dag M in the sloppy precision)       */
+    int restarts;                  /* double-precision residual computations                                           */
+    double residual;               /* last true relative residual |b - A x| / |b|                                      */
+    int converged;                 /* 1 if residual <= tol                                                            */
+} tm_cg_info;
+/* Mixed-precision conjugate gradient on the normal equations of the even-odd preconditioned operator (the paper's
+ * "double-single" / "double-half" CG, as defect correction): solves
+ *     M^dag M x_e = b_e ,   M = the LHS of Eq. 2.2 (ASYM) or Eq. 2.3 (SYM),
+ * starting from x_e = 0 (the content of x_e on entry is ignored).  x_e, b_e and g_precise are double; g_sloppy is the
+ * same gauge field loaded in sloppy_precision (ignored, may be NULL, when that is TM_DOUBLE).  Work fields are
+ * allocated and freed inside the call.  Returns TM_OK also when max_iter was reached (see info->converged);
+ * TM_ERR_PARAM on breakdown (<p, A p> <= 0).  Synchronous (every iteration reads two sums back). */
+int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, const tm_gauge *g_sloppy,
+                 const tm_params *p, tm_matpc type, const tm_cg_params *cp, tm_cg_info *info);
+
 /* ---- diagnostics ----------------------------------------------------------------------------------- */
 const char *tm_last_error(void);       /* thread-local, never NULL */
 /* Number of dslash kernel launches issued through this context so far (bench.py's gpu_launches). */

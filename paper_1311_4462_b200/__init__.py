@@ -32,7 +32,7 @@ EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
     "tm_field_device_ptr", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb",
     "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_twist_apply",
-    "tm_prepare_rhs", "tm_last_error",
+    "tm_prepare_rhs", "tm_field_axpby", "tm_field_redot", "tm_invert_cg", "tm_last_error",
     "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_set_tuning", "tm_timing_enable", "tm_timing_read",
 ]
 
@@ -41,6 +41,16 @@ class TmError(RuntimeError):
     def __init__(self, status, message):
         super().__init__("tm status %d: %s" % (status, message))
         self.status = status
+
+
+class tm_cg_params(ctypes.Structure):
+    _fields_ = [("tol", ctypes.c_double), ("max_iter", ctypes.c_int), ("sloppy_precision", ctypes.c_int),
+                ("delta", ctypes.c_double)]
+
+
+class tm_cg_info(ctypes.Structure):
+    _fields_ = [("iterations", ctypes.c_int), ("restarts", ctypes.c_int), ("residual", ctypes.c_double),
+                ("converged", ctypes.c_int)]
 
 
 class tm_params(ctypes.Structure):
@@ -88,6 +98,9 @@ def lib():
     L.tm_reconstruct_odd.argtypes = [vp, vp, vp, vp, pp]
     L.tm_twist_apply.argtypes = [vp, vp, pp, i, i]
     L.tm_prepare_rhs.argtypes = [vp, vp, vp, vp, vp, pp, i]
+    L.tm_field_axpby.argtypes = [vp, d, vp, d, vp]
+    L.tm_field_redot.argtypes = [vp, vp, ctypes.POINTER(d)]
+    L.tm_invert_cg.argtypes = [vp, vp, vp, vp, pp, i, ctypes.POINTER(tm_cg_params), ctypes.POINTER(tm_cg_info)]
     L.tm_last_error.restype = ctypes.c_char_p
     L.tm_launch_count.argtypes = [vp]
     L.tm_launch_count.restype = ctypes.c_long
@@ -199,6 +212,25 @@ def tm_twist_apply(out, inp, p, inverse=0, dagger=0):
 
 def tm_prepare_rhs(rhs_e, b_e, b_o, tmp_o, gauge, p, matpc_type):
     _check(lib().tm_prepare_rhs(rhs_e, b_e, b_o, tmp_o, gauge, ctypes.byref(p), int(matpc_type)))
+
+
+def tm_field_axpby(z, a, x, b, y):
+    _check(lib().tm_field_axpby(z, float(a), x, float(b), y))
+
+
+def tm_field_redot(x, y):
+    r = ctypes.c_double(0.0)
+    _check(lib().tm_field_redot(x, y, ctypes.byref(r)))
+    return r.value
+
+
+def tm_invert_cg(x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol, max_iter, sloppy_precision, delta):
+    """-> dict(iterations, restarts, residual, converged)"""
+    cp = tm_cg_params(float(tol), int(max_iter), int(sloppy_precision), float(delta))
+    info = tm_cg_info()
+    _check(lib().tm_invert_cg(x_e, b_e, g_precise, g_sloppy, ctypes.byref(p), int(matpc_type), ctypes.byref(cp),
+                              ctypes.byref(info)))
+    return dict(iterations=info.iterations, restarts=info.restarts, residual=info.residual, converged=bool(info.converged))
 
 
 def tm_launch_count(ctx):
@@ -340,3 +372,16 @@ def twist_apply(out, inp, p, inverse=0, dagger=0):
 
 def prepare_rhs(rhs_e, b_e, b_o, tmp_o, gauge, p, matpc_type):
     tm_prepare_rhs(rhs_e.h, b_e.h, b_o.h, tmp_o.h, gauge.h, p, matpc_type)
+
+
+def field_axpby(z, a, x, b=0.0, y=None):
+    tm_field_axpby(z.h, a, x.h, b, None if y is None else y.h)
+
+
+def field_redot(x, y):
+    return tm_field_redot(x.h, y.h)
+
+
+def invert_cg(x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol=1e-10, max_iter=10000, sloppy_precision=TM_SINGLE, delta=0.1):
+    return tm_invert_cg(x_e.h, b_e.h, g_precise.h, None if g_sloppy is None else g_sloppy.h, p, matpc_type, tol, max_iter,
+                        sloppy_precision, delta)

@@ -1,6 +1,7 @@
 // tm_api.cu -- the C-ABI boundary declared in include/tm.h: handles, validation, dispatch.
 // No arithmetic of the method lives here except forming a = 2 kappa mu, b = 2 kappa epsilon and the
 // twist coefficients in double (reading C2, C10-ii).
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -150,6 +151,8 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->sm_count = 0;
     c->staging = nullptr;
     c->staging_bytes = 0;
+    c->red = nullptr;
+    c->red_n = 0;
     c->timing = false;
     e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
     if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaDeviceGetAttribute"); }
@@ -176,6 +179,7 @@ void tm_finalize(tm_ctx *ctx)
 {
     if (!ctx) return;
     if (ctx->staging) cudaFree(ctx->staging);
+    if (ctx->red) cudaFree(ctx->red);
     for (auto &t : ctx->timed) { cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
     delete ctx;
 }
@@ -473,6 +477,126 @@ int tm_reconstruct_odd(tm_field *psi_o, const tm_field *psi_e, const tm_field *b
 {
     if (!psi_o || !psi_e || !b_o || !g || !p) return fail(TM_ERR_ARG, "tm_reconstruct_odd: NULL argument");
     return tm_dslash_apply(psi_o, psi_e, b_o, g, p, TM_ODD, 0, TM_RECONSTRUCT, (tm_precision)psi_o->prec);
+}
+
+// ---- vector operations and the mixed-precision CG --------------------
+
+int tm_field_axpby(tm_field *z, double a, const tm_field *x, double b, const tm_field *y)
+{
+    if (!z || !x) return fail(TM_ERR_ARG, "tm_field_axpby: NULL argument");
+    if (x->ctx != z->ctx || (y && y->ctx != z->ctx)) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
+    if (x->nf != z->nf || (y && y->nf != z->nf)) return fail(TM_ERR_MISMATCH, "flavor count mismatch");
+    if ((overlap(z, x) && z->ptr != x->ptr) || (y && overlap(z, y) && z->ptr != y->ptr))
+        return fail(TM_ERR_ALIAS, "z partially overlaps an input");
+    cudaError_t e = tm_blas_axpbyz(z, a, x, b, y, nullptr);
+    if (e == cudaErrorInvalidValue) return fail(TM_ERR_UNSUPPORTED, "precision mix (z %d, x %d, y %d) not supported", z->prec, x->prec, y ? y->prec : 0);
+    if (e != cudaSuccess) return cuda_fail(e, "tm_field_axpby");
+    return TM_OK;
+}
+
+int tm_field_redot(const tm_field *x, const tm_field *y, double *result)
+{
+    if (!x || !y || !result) return fail(TM_ERR_ARG, "tm_field_redot: NULL argument");
+    if (x->ctx != y->ctx) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
+    if (x->nf != y->nf || x->prec != y->prec) return fail(TM_ERR_MISMATCH, "precision or flavor count mismatch");
+    cudaError_t e = tm_blas_redot(x, y, result);
+    if (e != cudaSuccess) return cuda_fail(e, "tm_field_redot");
+    return TM_OK;
+}
+
+namespace {
+
+// work fields of one solve (library-owned device memory, zero-filled so that tile padding is defined)
+struct WorkFields {
+    std::vector<tm_field *> f;
+    ~WorkFields() { for (tm_field *p : f) tm_field_free(p); }
+    tm_field *make(tm_ctx *c, int prec, int nf)
+    {
+        tm_field *p = nullptr;
+        if (tm_field_alloc(c, (tm_precision)prec, nf, nullptr, 0, &p) != TM_OK) return nullptr;
+        f.push_back(p);
+        if (cudaMemsetAsync(p->ptr, 0, p->bytes, c->stream) != cudaSuccess) return nullptr;
+        return p;
+    }
+};
+
+// out = M^dag M in on the even sites; t_e and tmp_o are scratch of in's precision
+int apply_normal(tm_field *out, const tm_field *in, tm_field *t_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p, tm_matpc type)
+{
+    int rc = tm_mat_pc(t_e, in, tmp_o, g, p, type, 0);
+    if (!rc) rc = tm_mat_pc(out, t_e, tmp_o, g, p, type, 1);
+    return rc;
+}
+
+#define TM_TRY_CUDA(call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, what); } while (0)
+#define TM_TRY(call) do { int rc_ = (call); if (rc_) return rc_; } while (0)
+
+}  // namespace
+
+int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, const tm_gauge *g_sloppy, const tm_params *p,
+                 tm_matpc type, const tm_cg_params *cp, tm_cg_info *info)
+{
+    if (!x_e || !b_e || !g_precise || !p || !cp || !info) return fail(TM_ERR_ARG, "tm_invert_cg: NULL argument");
+    info->iterations = 0; info->restarts = 0; info->residual = 0.0; info->converged = 0;
+    tm_ctx *c = x_e->ctx;
+    if (b_e->ctx != c || g_precise->ctx != c) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
+    if (x_e->prec != TM_DOUBLE || b_e->prec != TM_DOUBLE || g_precise->prec != TM_DOUBLE)
+        return fail(TM_ERR_MISMATCH, "x_e, b_e and g_precise must be double precision");
+    if (x_e->nf != b_e->nf) return fail(TM_ERR_MISMATCH, "flavor count mismatch");
+    if (overlap(x_e, b_e)) return fail(TM_ERR_ALIAS, "x_e aliases b_e");
+    const int ps = (int)cp->sloppy_precision;
+    if (!valid_prec(ps)) return fail(TM_ERR_ARG, "bad sloppy precision %d", ps);
+    const tm_gauge *gs = ps == TM_DOUBLE ? g_precise : g_sloppy;
+    if (!gs || gs->ctx != c || gs->prec != ps) return fail(TM_ERR_MISMATCH, "g_sloppy must be a gauge handle of the sloppy precision");
+    if (!(cp->tol > 0.0) || cp->max_iter < 1 || !(cp->delta > 0.0 && cp->delta < 1.0))
+        return fail(TM_ERR_ARG, "need tol > 0, max_iter >= 1, 0 < delta < 1");
+    if (type != TM_MATPC_ASYM && type != TM_MATPC_SYM) return fail(TM_ERR_ARG, "bad matpc type %d", (int)type);
+    const int nf = x_e->nf;
+
+    WorkFields w;
+    tm_field *r_d = w.make(c, TM_DOUBLE, nf), *t_d = w.make(c, TM_DOUBLE, nf), *te_d = w.make(c, TM_DOUBLE, nf), *to_d = w.make(c, TM_DOUBLE, nf);
+    tm_field *r_s = w.make(c, ps, nf), *p_s = w.make(c, ps, nf), *ap_s = w.make(c, ps, nf), *x_s = w.make(c, ps, nf);
+    tm_field *te_s = w.make(c, ps, nf), *to_s = w.make(c, ps, nf);
+    if (!r_d || !t_d || !te_d || !to_d || !r_s || !p_s || !ap_s || !x_s || !te_s || !to_s) return fail(TM_ERR_NOMEM, "tm_invert_cg: work fields");
+
+    double bnorm2 = 0.0, rnorm2 = 0.0;
+    TM_TRY_CUDA(tm_blas_redot(b_e, b_e, &bnorm2), "redot");
+    TM_TRY_CUDA(tm_blas_axpbyz(x_e, 0.0, b_e, 0.0, nullptr, nullptr), "zero x");        // x = 0
+    if (bnorm2 == 0.0) { info->converged = 1; return TM_OK; }
+    TM_TRY_CUDA(tm_blas_axpbyz(r_d, 1.0, b_e, 0.0, nullptr, &rnorm2), "copy b");          // r = b
+
+    // defect correction: the inner CG runs in the sloppy precision on A e = r / |r| until the residual has dropped by
+    // delta (or as far as the outer tolerance needs); x += |r| e and the residual b - A x are formed in double.
+    for (;;) {
+        const double relres = std::sqrt(rnorm2 / bnorm2);
+        info->residual = relres;
+        if (relres <= cp->tol) { info->converged = 1; break; }
+        if (info->iterations >= cp->max_iter) break;
+        const double rn = std::sqrt(rnorm2);
+        double rr = 0.0, rr0;
+        TM_TRY_CUDA(tm_blas_axpbyz(r_s, 1.0 / rn, r_d, 0.0, nullptr, &rr), "scale r");                // r_s = r / |r|
+        TM_TRY_CUDA(tm_blas_axpbyz(x_s, 0.0, r_s, 0.0, nullptr, nullptr), "zero e");                  // e = 0
+        TM_TRY_CUDA(tm_blas_axpbyz(p_s, 1.0, r_s, 0.0, nullptr, nullptr), "copy p");                  // p = r_s
+        rr0 = rr;
+        const double target = std::max(cp->delta, 0.5 * cp->tol / relres);
+        for (;;) {
+            TM_TRY(apply_normal(ap_s, p_s, te_s, to_s, gs, p, type));                                  // Ap
+            double pap = 0.0, rr_new = 0.0;
+            TM_TRY_CUDA(tm_blas_redot(p_s, ap_s, &pap), "redot");
+            if (!(pap > 0.0)) return fail(TM_ERR_PARAM, "tm_invert_cg: <p, A p> = %g is not positive (breakdown)", pap);
+            const double alpha = rr / pap;
+            TM_TRY_CUDA(tm_blas_cg_update(x_s, r_s, p_s, ap_s, alpha, &rr_new), "cg_update");          // e += a p, r_s -= a Ap
+            info->iterations++;
+            if (std::sqrt(rr_new / rr0) <= target || info->iterations >= cp->max_iter) break;
+            TM_TRY_CUDA(tm_blas_axpbyz(p_s, 1.0, r_s, rr_new / rr, p_s, nullptr), "xpay");             // p = r_s + beta p
+            rr = rr_new;
+        }
+        TM_TRY_CUDA(tm_blas_axpbyz(x_e, rn, x_s, 1.0, x_e, nullptr), "x += |r| e");
+        TM_TRY(apply_normal(t_d, x_e, te_d, to_d, g_precise, p, type));                                // true residual in double
+        TM_TRY_CUDA(tm_blas_axpbyz(r_d, 1.0, b_e, -1.0, t_d, &rnorm2), "r = b - A x");
+        info->restarts++;
+    }
+    return TM_OK;
 }
 
 }  // extern "C"

@@ -37,6 +37,8 @@ struct tm_ctx {
     int block_threads;   // tm_set_tuning("block_threads"): 0 library default, else 32 / 64 / 128
     int sm_count;
     void *staging;        // device staging for upload / download
+    double *red;          // reduction scratch of tm_blas.cu: [0] result, [1..] per-block partial sums
+    size_t red_n;
     size_t staging_bytes;
     bool timing;          // tm_timing_enable
     struct TimedLaunch { cudaEvent_t start, stop; const char *name; };
@@ -113,6 +115,11 @@ const TmKernelEntry *tm_generic_table(int prec, int nf);
 
 // out = scale (1 + i alpha gamma5 tau3 + beta tau1) in, site by site (tm_twist.cu)
 cudaError_t tm_launch_twist(const tm_field *out, const tm_field *in, double alpha, double beta, double scale, cudaStream_t s);
+
+// vector operations of the CG (tm_blas.cu); the ones that return a sum synchronise the stream
+cudaError_t tm_blas_axpbyz(tm_field *z, double a, const tm_field *x, double b, const tm_field *y, double *norm2);
+cudaError_t tm_blas_redot(const tm_field *x, const tm_field *y, double *out);
+cudaError_t tm_blas_cg_update(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr);
 
 // pack / unpack (tm_pack.cu)
 cudaError_t tm_pack_spinor(const tm_field *f, int parity, const double *dev_src, bool src_is_cb, cudaStream_t s);
