@@ -389,9 +389,9 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.alpha = co.alpha; a.beta = co.beta; a.scale = co.scale;
     a.kappa = p->kappa; a.kappa2 = p->kappa * p->kappa;
     a.tbound = (double)p->t_boundary;
-    // measured defaults (profiles/): the fp64 doublet kernels gain from an L2 prefetch 8 tiles ahead, the half
+    // measured defaults (profiles/): the fp64 doublet kernels with 12-real links gain from an L2 prefetch 8 tiles ahead, the half
     // kernels from staging the link stream through shared memory; everything else runs plain
-    a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_DOUBLE && out->nf == 2 ? 8 : 0);
+    a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_DOUBLE && out->nf == 2 && g->recon == 12 ? 8 : 0);
     int stage = c->stage >= 0 ? c->stage : ((int)prec == TM_HALF ? 1 : 0);
     a.block_threads = c->block_threads ? c->block_threads : 128;
     while (stage && (size_t)8 * g->recon * (int)prec * a.block_threads > 96 * 1024 && a.block_threads > 32) a.block_threads /= 2;
