@@ -48,8 +48,13 @@ typedef enum { TM_DOUBLE = 8, TM_SINGLE = 4, TM_HALF = 2 } tm_precision;
 /* TM_HALF: 16-bit fixed point, one float norm per (site, flavor): q = rint(v * 32767 / max|v|)
  * (Table 1 "half"; format per DESIGN.md reading C9); arithmetic in fp32.              */
 
-typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12 } tm_recon;
-/* TM_RECON_12: rows 0 and 1 stored, row 2 = conj(row0 x row1) rebuilt in the kernel.      */
+typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12, TM_RECON_8 = 8 } tm_recon;
+/* TM_RECON_12: rows 0 and 1 stored, row 2 = conj(row0 x row1) rebuilt in the kernel.
+ * TM_RECON_8 : "8 ... parameter reconstruct" (Table 1 rows "8").  Stored per link: U01, U02, U10
+ *   (complex) and arg(U00)/pi, arg(U20)/pi; the kernel rebuilds |U00|, |U20| from the unit norm of row 0 and
+ *   column 0, U11 and U12 from <row0,row1> = 0 and U20 = conj(U01 U12 - U02 U11), then row 2 as for 12-real
+ *   (chart: DESIGN.md reading C11).  The chart divides by N = |U01|^2 + |U02|^2: rounding errors grow like
+ *   eps / N and a link with N < 1e-10 (e.g. the unit matrix) makes tm_gauge_load return TM_ERR_PARAM.    */
 
 typedef enum { TM_EVEN = 0, TM_ODD = 1 } tm_parity;
 

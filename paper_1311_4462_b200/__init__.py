@@ -22,7 +22,7 @@ TM_OK = 0
 TM_ERR_ARG, TM_ERR_DIMS, TM_ERR_MISMATCH, TM_ERR_ALIAS = -1, -2, -3, -4
 TM_ERR_PARAM, TM_ERR_NOMEM, TM_ERR_CUDA, TM_ERR_UNSUPPORTED = -5, -6, -7, -8
 TM_DOUBLE, TM_SINGLE, TM_HALF = 8, 4, 2
-TM_RECON_18, TM_RECON_12 = 18, 12
+TM_RECON_18, TM_RECON_12, TM_RECON_8 = 18, 12, 8
 TM_EVEN, TM_ODD = 0, 1
 TM_TWIST_INV_DSLASH, TM_TWIST_INV_DSLASH_XPAY, TM_DSLASH_TWIST_XPAY, TM_RECONSTRUCT = 0, 1, 2, 3
 TM_DSLASH_XPAY, TM_DSLASH_AXPY = 4, 5

@@ -336,7 +336,19 @@ int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_r
     if (!ctx || !host_links || !g) return fail(TM_ERR_ARG, "tm_gauge_load: NULL argument");
     *g = nullptr;
     if (!valid_prec(prec)) return fail(TM_ERR_ARG, "bad precision %d", (int)prec);
-    if (recon != TM_RECON_18 && recon != TM_RECON_12) return fail(TM_ERR_ARG, "bad recon %d", (int)recon);
+    if (recon != TM_RECON_18 && recon != TM_RECON_12 && recon != TM_RECON_8) return fail(TM_ERR_ARG, "bad recon %d", (int)recon);
+    if (recon == TM_RECON_8) {
+        // the 8-real chart divides by N = |U01|^2 + |U02|^2 (tm_layout.cuh: rebuild_from8); its error grows like eps / N
+        const size_t nl = (size_t)4 * ctx->g.V;
+        double nmin = 1.0;
+        for (size_t l = 0; l < nl; l++) {
+            const double *u = host_links + l * 18;
+            const double N = u[2] * u[2] + u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
+            if (N < nmin) nmin = N;
+        }
+        if (!(nmin >= 1e-10))
+            return fail(TM_ERR_PARAM, "8-real links: a link has |U01|^2 + |U02|^2 = %.3g, at the chart's singular point (use 12- or 18-real)", nmin);
+    }
     tm_gauge *gg = new (std::nothrow) tm_gauge();
     if (!gg) return fail(TM_ERR_NOMEM, "out of host memory");
     gg->ctx = ctx; gg->prec = prec; gg->recon = recon;
@@ -394,12 +406,15 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_DOUBLE && out->nf == 2 && g->recon == 12 ? 8 : 0);
     int stage = c->stage >= 0 ? c->stage : ((int)prec == TM_HALF ? 1 : 0);
     a.block_threads = c->block_threads ? c->block_threads : 128;
+    if (g->recon == 8) stage = 0;        // 8-real links: direct loads
     while (stage && (size_t)8 * g->recon * (int)prec * a.block_threads > 96 * 1024 && a.block_threads > 32) a.block_threads /= 2;
 
     // path 0: fp32 / half run the packed-FP32 kernels, fp64 the scalar kernel; path 1 forces the scalar kernel
-    const TmKernelEntry *tab = (c->path == 0 && (int)prec != TM_DOUBLE) ? tm_f2_table((int)prec, out->nf)
-                                                                       : tm_generic_table((int)prec, out->nf);
-    const TmKernelEntry &k = tab[(((g->recon == 18 ? 0 : 1) * 4 + kcode) * 2 + (dagger ? 1 : 0)) * 2 + stage];
+    // (8-real links: packed kernels exist for fp32 only; half takes the scalar kernel)
+    const int kidx = (((g->recon == 18 ? 0 : g->recon == 12 ? 1 : 2) * 4 + kcode) * 2 + (dagger ? 1 : 0)) * 2 + stage;
+    const TmKernelEntry *tab = (c->path == 0 && (int)prec != TM_DOUBLE) ? tm_f2_table((int)prec, out->nf) : nullptr;
+    if (!tab || !tab[kidx].fn) tab = tm_generic_table((int)prec, out->nf);
+    const TmKernelEntry &k = tab[kidx];
     cudaError_t e;
     if (c->timing) {
         tm_ctx::TimedLaunch t;

@@ -274,15 +274,21 @@ cudaError_t tm_launch_generic(const DslashArgs &a, cudaStream_t s)
     return cudaGetLastError();
 }
 
-// table index: [recon18?0:1][kt 0..3][dagger 0..1][staged 0..1]
+// table index: [recon 18 / 12 / 8 -> 0 / 1 / 2][kt 0..3][dagger 0..1][staged 0..1]; 8-real links are never staged
+#define TM_GENERIC_ROW8(P, N, K)                                                                            \
+    {tm_launch_generic<P, N, 8, K, false, false>, "generic<" #P "," #N ",8," #K ",plain>"},                \
+    {tm_launch_generic<P, N, 8, K, false, false>, "generic<" #P "," #N ",8," #K ",plain>"},                \
+    {tm_launch_generic<P, N, 8, K, true, false>, "generic<" #P "," #N ",8," #K ",dagger>"},                \
+    {tm_launch_generic<P, N, 8, K, true, false>, "generic<" #P "," #N ",8," #K ",dagger>"}
 #define TM_GENERIC_ROW(P, N, R, K)                                                                          \
     {tm_launch_generic<P, N, R, K, false, false>, "generic<" #P "," #N "," #R "," #K ",plain>"},           \
     {tm_launch_generic<P, N, R, K, false, true>, "generic_staged<" #P "," #N "," #R "," #K ",plain>"},     \
     {tm_launch_generic<P, N, R, K, true, false>, "generic<" #P "," #N "," #R "," #K ",dagger>"},           \
     {tm_launch_generic<P, N, R, K, true, true>, "generic_staged<" #P "," #N "," #R "," #K ",dagger>"}
 #define TM_GENERIC_TABLE(P, N)                                                                        \
-    static const TmKernelEntry table_##P##_##N[32] = {                                               \
+    static const TmKernelEntry table_##P##_##N[48] = {                                               \
         TM_GENERIC_ROW(P, N, 18, 0), TM_GENERIC_ROW(P, N, 18, 1), TM_GENERIC_ROW(P, N, 18, 2),       \
         TM_GENERIC_ROW(P, N, 18, 3), TM_GENERIC_ROW(P, N, 12, 0), TM_GENERIC_ROW(P, N, 12, 1),       \
-        TM_GENERIC_ROW(P, N, 12, 2), TM_GENERIC_ROW(P, N, 12, 3)};                                   \
+        TM_GENERIC_ROW(P, N, 12, 2), TM_GENERIC_ROW(P, N, 12, 3), TM_GENERIC_ROW8(P, N, 0),          \
+        TM_GENERIC_ROW8(P, N, 1), TM_GENERIC_ROW8(P, N, 2), TM_GENERIC_ROW8(P, N, 3)};               \
     const TmKernelEntry *tm_generic_table_##P##_##N() { return table_##P##_##N; }

@@ -66,7 +66,7 @@ template <int PREC, int NF> __host__ __device__ constexpr int f2_pipeline_depth(
 // in flight costs 19 registers per flavor-site, in fp32 36 + 24 NF.
 template <int PREC, int NF, int RECON>
 struct HopRaw {
-    static constexpr int NL = (PREC == 4) ? (RECON == 18 ? 4 : 3) : (RECON == 18 ? 2 : 1);   // 128-bit link words
+    static constexpr int NL = (PREC == 4) ? (RECON == 18 ? 4 : RECON == 12 ? 3 : 2) : (RECON == 18 ? 2 : 1);   // 128-bit link words
     static constexpr int NS = (PREC == 4) ? 6 : 3;                                          // 128-bit spinor words
     uint4 l[NL];
     uint2 lt;            // link tail: fp32/18 float2, half/12 int2, half/18 int (.x)
@@ -157,10 +157,40 @@ TM_DEV void raw_to_spinor(f2 *S, const uint4 *s)
 
 // a4 (rebuild): link as 9 (re, im) pairs W[row*3+col]; half: RAW integers for rows 0,1; 12-real: row 2 is rebuilt and,
 // in half, left at raw x raw scale: the factor 1/32767 is applied where it is cheapest (consume_hop).
+// 8-real links, fp32 (chart: tm_layout.cuh rebuild_from8): rows 0 and 1 from the 8 stored reals with the fast
+// special-function unit (sin / cos / rsqrt / rcp approximations, abs. error ~5e-7: inside the fp32 tolerance; the
+// scalar kernels use the IEEE forms).  Scalar arithmetic: the link is per site, not per spin pair.
+TM_DEV void rows01_from8_fast(f2 *W, const float *p)
+{
+    const float a2r = p[0], a2i = p[1], a3r = p[2], a3i = p[3], b1r = p[4], b1i = p[5];
+    const float N = fmaf(a2r, a2r, fmaf(a2i, a2i, fmaf(a3r, a3r, a3i * a3i)));
+    const float t1 = p[6] * 3.14159265358979f, t2 = p[7] * 3.14159265358979f;
+    const float s1 = __sinf(t1), c1 = __cosf(t1), s2 = __sinf(t2), c2 = __cosf(t2);
+    const float q1 = fmaxf(1.f - N, 0.f), q2 = fmaxf(N - fmaf(b1r, b1r, b1i * b1i), 0.f);
+    const float m1 = q1 * rsqrtf(fmaxf(q1, 1e-30f)), m2 = q2 * rsqrtf(fmaxf(q2, 1e-30f));
+    const float a1r = m1 * c1, a1i = m1 * s1;
+    const float r2r = m2 * c2, r2i = -(m2 * s2);                                        // conj(c1)
+    const float r1r = -fmaf(a1r, b1r, a1i * b1i), r1i = fmaf(a1i, b1r, -(a1r * b1i));   // -conj(a1) b1
+    const float iN = __fdividef(1.f, N);
+    W[0] = mk2(a1r, a1i);
+    W[1] = mk2(a2r, a2i);
+    W[2] = mk2(a3r, a3i);
+    W[3] = mk2(b1r, b1i);
+    W[4] = mk2((fmaf(r1r, a2r, -(r1i * a2i)) - fmaf(a3r, r2r, a3i * r2i)) * iN,
+               (fmaf(r1r, a2i, r1i * a2r) - fmaf(a3r, r2i, -(a3i * r2r))) * iN);
+    W[5] = mk2((fmaf(a2r, r2r, a2i * r2i) + fmaf(a3r, r1r, -(a3i * r1i))) * iN,
+               (fmaf(a2r, r2i, -(a2i * r2r)) + fmaf(a3r, r1i, a3i * r1r)) * iN);
+}
+
 template <int PREC, int NF, int RECON>
 TM_DEV void raw_to_link(f2 *W, const HopRaw<PREC, NF, RECON> &r)
 {
-    if constexpr (PREC == 4) {
+    if constexpr (RECON == 8) {
+        static_assert(PREC == 4, "packed kernels take 8-real links in fp32 only");
+        const float p[8] = {__uint_as_float(r.l[0].x), __uint_as_float(r.l[0].y), __uint_as_float(r.l[0].z), __uint_as_float(r.l[0].w),
+                            __uint_as_float(r.l[1].x), __uint_as_float(r.l[1].y), __uint_as_float(r.l[1].z), __uint_as_float(r.l[1].w)};
+        rows01_from8_fast(W, p);
+    } else if constexpr (PREC == 4) {
 #pragma unroll
         for (int k = 0; k < HopRaw<PREC, NF, RECON>::NL; k++) {
             W[2 * k] = mk2(__uint_as_float(r.l[k].x), __uint_as_float(r.l[k].y));
@@ -176,7 +206,7 @@ TM_DEV void raw_to_link(f2 *W, const HopRaw<PREC, NF, RECON> &r)
             W[4] = cvt_pair(r.lt.x); W[5] = cvt_pair(r.lt.y);
         }
     }
-    if constexpr (RECON == 12) {
+    if constexpr (RECON != 18) {
         // row2[c] = conj(row0[c1] row1[c2] - row0[c2] row1[c1]),  pairs are (re, im):
         //   S = a.re*b - c.re*d ,  T = a.im*sw(b) - c.im*sw(d) ;  a*b - c*d = (S.x - T.x, S.y + T.y)
 #pragma unroll
@@ -550,14 +580,23 @@ cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
 #define TM_F2_ROW0 TM_F2_NONE, TM_F2_NONE, TM_F2_NONE, TM_F2_NONE
 #define TM_F2_ROWS(P, N, R, K) {tm_launch_f2<P, N, R, K, false, false>, "f2<" #P "," #N "," #R "," #K ",plain>"}, {tm_launch_f2<P, N, R, K, false, true>, "f2_staged<" #P "," #N "," #R "," #K ",plain>"}, TM_F2_NONE, TM_F2_NONE
 #define TM_F2_TABLE(P, N)                                                                    \
-    static const TmKernelEntry f2table_##P##_##N[32] = {                                    \
+    static const TmKernelEntry f2table_##P##_##N[48] = {                                    \
         TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROWS(P, N, 12, 0), TM_F2_ROW0, TM_F2_ROWS(P, N, 12, 2), TM_F2_ROW0}; \
     const TmKernelEntry *tm_f2_table_##P##_##N() { return f2table_##P##_##N; }
 #else
+// 8-real links: fp32 only, direct loads only (both staging slots hold the direct kernel); half has no entry (nullptr ->
+// tm_dslash_apply takes the scalar kernel)
+#define TM_F2_ROW8(N, K)                                                                           \
+    {tm_launch_f2<4, N, 8, K, false, false>, "f2<4," #N ",8," #K ",plain>"},                      \
+    {tm_launch_f2<4, N, 8, K, false, false>, "f2<4," #N ",8," #K ",plain>"},                      \
+    {tm_launch_f2<4, N, 8, K, true, false>, "f2<4," #N ",8," #K ",dagger>"},                      \
+    {tm_launch_f2<4, N, 8, K, true, false>, "f2<4," #N ",8," #K ",dagger>"}
+#define TM_F2_ROWS8_4(N) , TM_F2_ROW8(N, 0), TM_F2_ROW8(N, 1), TM_F2_ROW8(N, 2), TM_F2_ROW8(N, 3)
+#define TM_F2_ROWS8_2(N)
 #define TM_F2_TABLE(P, N)                                                                    \
-    static const TmKernelEntry f2table_##P##_##N[32] = {                                    \
+    static const TmKernelEntry f2table_##P##_##N[48] = {                                    \
         TM_F2_ROW(P, N, 18, 0), TM_F2_ROW(P, N, 18, 1), TM_F2_ROW(P, N, 18, 2),             \
         TM_F2_ROW(P, N, 18, 3), TM_F2_ROW(P, N, 12, 0), TM_F2_ROW(P, N, 12, 1),             \
-        TM_F2_ROW(P, N, 12, 2), TM_F2_ROW(P, N, 12, 3)};                                    \
+        TM_F2_ROW(P, N, 12, 2), TM_F2_ROW(P, N, 12, 3) TM_F2_ROWS8_##P(N)};                 \
     const TmKernelEntry *tm_f2_table_##P##_##N() { return f2table_##P##_##N; }
 #endif

@@ -9,6 +9,7 @@
 //        fp64: recon/2 planes of double2
 //        fp32: 18 -> 4 x float4 + 1 x float2 ; 12 -> 3 x float4
 //        half: 18 -> 2 x int4(8 x int16) + 1 x int(2 x int16) ; 12 -> 1 x int4 + 1 x int2
+//        8-real (tm_layout.cuh: rebuild_from8): 4 x double2 / 2 x float4 / 1 x int4
 //   the [parity] block holds U_mu(x) for the sites x of that parity.
 #pragma once
 #include <cuda_runtime.h>
@@ -110,7 +111,7 @@ struct TmKernelEntry {
     tm_launch_fn fn;
     const char *name;
 };
-// index: [recon18?0:1][kt 0..3][dagger 0..1][staged 0..1]
+// index: [recon 18 / 12 / 8 -> 0 / 1 / 2][kt 0..3][dagger 0..1][staged 0..1]  (8-real: scalar kernels only)
 const TmKernelEntry *tm_generic_table(int prec, int nf);
 
 // out = scale (1 + i alpha gamma5 tau3 + beta tau1) in, site by site (tm_twist.cu)

@@ -207,14 +207,47 @@ TM_DEV void rebuild_row2(real *u)
     }
 }
 
+// 8-real ("8 or 12 parameter reconstruct"; the chart is DESIGN.md reading C11).  Stored, with rows a, b, c:
+//   p[0..5] = a2, a3, b1 (re, im)   p[6] = arg(a1) / pi   p[7] = arg(c1) / pi      (all in [-1, 1])
+// Rebuilt:  N = |a2|^2 + |a3|^2,  a1 = sqrt(1 - N) e^{i pi p6},  c1 = sqrt(N - |b1|^2) e^{i pi p7}  (row 0 and column 0
+// have unit norm), then the two linear conditions  <a, b> = 0  and  c1 = conj(a2 b3 - a3 b2)  give
+//   b2 = (r1 a2 - conj(a3) r2) / N ,  b3 = (conj(a2) r2 + a3 r1) / N ,   r1 = -conj(a1) b1 ,  r2 = conj(c1),
+// and row 2 = conj(row0 x row1) as for 12-real.  The chart is singular at N = 0 (tm_gauge_load refuses such links).
+TM_DEV void tm_sincospi(float x, float *s, float *c) { sincospif(x, s, c); }
+TM_DEV void tm_sincospi(double x, double *s, double *c) { sincospi(x, s, c); }
+TM_DEV float tm_sqrt(float x) { return sqrtf(x); }
+TM_DEV double tm_sqrt(double x) { return sqrt(x); }
+template <typename real>
+TM_DEV void rebuild_from8(real *u, const real *p)
+{
+    const real a2r = p[0], a2i = p[1], a3r = p[2], a3i = p[3], b1r = p[4], b1i = p[5];
+    const real N = tm_fma(a2r, a2r, tm_fma(a2i, a2i, tm_fma(a3r, a3r, a3i * a3i)));
+    real s1, c1, s2, c2;
+    tm_sincospi(p[6], &s1, &c1);
+    tm_sincospi(p[7], &s2, &c2);
+    const real m1 = tm_sqrt(max((real)1 - N, (real)0));
+    const real m2 = tm_sqrt(max(N - tm_fma(b1r, b1r, b1i * b1i), (real)0));
+    const real a1r = m1 * c1, a1i = m1 * s1;
+    const real r2r = m2 * c2, r2i = -(m2 * s2);                               // conj(c1)
+    const real r1r = -tm_fma(a1r, b1r, a1i * b1i), r1i = tm_fma(a1i, b1r, -(a1r * b1i));   // -conj(a1) b1
+    const real iN = (real)1 / N;
+    u[0] = a1r; u[1] = a1i; u[2] = a2r; u[3] = a2i; u[4] = a3r; u[5] = a3i;
+    u[6] = b1r; u[7] = b1i;
+    u[8] = (tm_fma(r1r, a2r, -(r1i * a2i)) - tm_fma(a3r, r2r, a3i * r2i)) * iN;
+    u[9] = (tm_fma(r1r, a2i, r1i * a2r) - tm_fma(a3r, r2i, -(a3i * r2r))) * iN;
+    u[10] = (tm_fma(a2r, r2r, a2i * r2i) + tm_fma(a3r, r1r, -(a3i * r1i))) * iN;
+    u[11] = (tm_fma(a2r, r2i, -(a2i * r2r)) + tm_fma(a3r, r1i, a3i * r1r)) * iN;
+    rebuild_row2(u);
+}
+
 // Planes of a stored link: n16 planes of 16 bytes per site, then (maybe) one tail plane of `tailw` bytes per site.
 template <int PREC, int RECON> __host__ __device__ constexpr int link_n16()
 {
-    return PREC == 8 ? RECON / 2 : PREC == 4 ? (RECON == 18 ? 4 : 3) : (RECON == 18 ? 2 : 1);
+    return PREC == 8 ? RECON / 2 : PREC == 4 ? (RECON == 18 ? 4 : RECON == 12 ? 3 : 2) : (RECON == 18 ? 2 : 1);
 }
 template <int PREC, int RECON> __host__ __device__ constexpr int link_tailw()
 {
-    return PREC == 8 ? 0 : PREC == 4 ? (RECON == 18 ? 8 : 0) : (RECON == 18 ? 4 : 8);
+    return PREC == 8 ? 0 : PREC == 4 ? (RECON == 18 ? 8 : 0) : (RECON == 18 ? 4 : RECON == 12 ? 8 : 0);
 }
 
 // `lp` = the link's site pointer (gauge parity block + link_site_off) or, SM = true, the thread's slot in the staged
@@ -223,7 +256,33 @@ template <int PREC, int RECON, bool SM = false>
 TM_DEV void load_link(typename PrecTraits<PREC>::real *u, const char *lp, int lane)
 {
     constexpr int N16 = link_n16<PREC, RECON>();
-    if constexpr (PREC == 8) {
+    if constexpr (RECON == 8) {
+        typename PrecTraits<PREC>::real p[8];
+        if constexpr (PREC == 8) {
+#pragma unroll
+            for (int k = 0; k < 4; k++) {
+                double2 c = ld_d2<SM>(lp + k * TM_PLANE);
+                p[2 * k] = c.x;
+                p[2 * k + 1] = c.y;
+            }
+        } else if constexpr (PREC == 4) {
+#pragma unroll
+            for (int k = 0; k < 2; k++) {
+                float4 c = ld_f4<SM>(lp + k * TM_PLANE);
+                p[4 * k] = c.x;
+                p[4 * k + 1] = c.y;
+                p[4 * k + 2] = c.z;
+                p[4 * k + 3] = c.w;
+            }
+        } else {
+            int4 c = ld_i4<SM>(lp);
+            unpack2(c.x, TM_HALF_INV, p[0], p[1]);
+            unpack2(c.y, TM_HALF_INV, p[2], p[3]);
+            unpack2(c.z, TM_HALF_INV, p[4], p[5]);
+            unpack2(c.w, TM_HALF_INV, p[6], p[7]);
+        }
+        rebuild_from8(u, p);
+    } else if constexpr (PREC == 8) {
 #pragma unroll
         for (int k = 0; k < N16; k++) {
             double2 c = ld_d2<SM>(lp + k * TM_PLANE);

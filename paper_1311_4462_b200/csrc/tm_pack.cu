@@ -60,7 +60,24 @@ __global__ void pack_gauge_kernel(char *dst, const double *src, PackGeom g)
     const double *s = src + ((size_t)mu * g.V + cb_to_lex(g, i, parity)) * 18;
     char *lp = dst + (size_t)parity * tm_tiles(g.Vh) * 4 * link_tile_bytes(PREC, RECON) + link_site_off(PREC, RECON, i, mu);
     const int lane = i & (TM_TILE - 1);
-    if constexpr (PREC == 8) {
+    if constexpr (RECON == 8) {
+        // the chart of rebuild_from8 (tm_layout.cuh): a2, a3, b1, arg(a1) / pi, arg(c1) / pi
+        const double p[8] = {s[2], s[3], s[4], s[5], s[6], s[7], atan2(s[1], s[0]) / M_PI, atan2(s[13], s[12]) / M_PI};
+        if constexpr (PREC == 8) {
+#pragma unroll
+            for (int k = 0; k < 4; k++) *reinterpret_cast<double2 *>(lp + k * TM_PLANE) = make_double2(p[2 * k], p[2 * k + 1]);
+        } else if constexpr (PREC == 4) {
+#pragma unroll
+            for (int k = 0; k < 2; k++)
+                *reinterpret_cast<float4 *>(lp + k * TM_PLANE) =
+                    make_float4((float)p[4 * k], (float)p[4 * k + 1], (float)p[4 * k + 2], (float)p[4 * k + 3]);
+        } else {
+            int w[4];
+#pragma unroll
+            for (int k = 0; k < 4; k++) w[k] = pack2((float)p[2 * k] * TM_HALF_MAX, (float)p[2 * k + 1] * TM_HALF_MAX);
+            *reinterpret_cast<int4 *>(lp) = make_int4(w[0], w[1], w[2], w[3]);
+        }
+    } else if constexpr (PREC == 8) {
 #pragma unroll
         for (int k = 0; k < RECON / 2; k++)
             *reinterpret_cast<double2 *>(lp + k * TM_PLANE) = make_double2(s[2 * k], s[2 * k + 1]);
@@ -131,9 +148,9 @@ cudaError_t tm_pack_gauge(const tm_gauge *gg, const double *dev_src, cudaStream_
     const int threads = 128, blocks = (int)((n + threads - 1) / threads);
     char *dst = static_cast<char *>(gg->ptr);
 #define TM_PG(P, R) pack_gauge_kernel<P, R><<<blocks, threads, 0, s>>>(dst, dev_src, g)
-    if (gg->prec == 8) { if (gg->recon == 18) TM_PG(8, 18); else TM_PG(8, 12); }
-    else if (gg->prec == 4) { if (gg->recon == 18) TM_PG(4, 18); else TM_PG(4, 12); }
-    else { if (gg->recon == 18) TM_PG(2, 18); else TM_PG(2, 12); }
+    if (gg->prec == 8) { if (gg->recon == 18) TM_PG(8, 18); else if (gg->recon == 12) TM_PG(8, 12); else TM_PG(8, 8); }
+    else if (gg->prec == 4) { if (gg->recon == 18) TM_PG(4, 18); else if (gg->recon == 12) TM_PG(4, 12); else TM_PG(4, 8); }
+    else { if (gg->recon == 18) TM_PG(2, 18); else if (gg->recon == 12) TM_PG(2, 12); else TM_PG(2, 8); }
 #undef TM_PG
     return cudaGetLastError();
 }

@@ -133,6 +133,52 @@ def test_t2b_periodic_time_and_wilson_limit():
                 assert rel_l2(got, want) <= TOL[prec]
 
 
+# ---- T2c: 8-real links ------------------------------------
+
+@pytest.mark.parametrize("dims,kind", [((4, 4, 4, 8), "haar"), ((4, 6, 8, 10), "near_identity"), ((6, 6, 6, 6), "haar")])
+@pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
+def test_t2c_recon8_every_kernel_matches_oracle(dims, kind, kw):
+    """The oracle multiplies the full 18-real double links; the library stores 8 reals per link and rebuilds the
+    matrix in the kernel, so this checks the chart, its packing and the rebuild in all three precisions."""
+    nf = nf_of(kw)
+    bench = bench_for(dims, kind, 1)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    full_in, full_x = si.spinor_field(dims, nf, 12), si.spinor_field(dims, nf, 13)
+    worst = {}
+    for parity, dagger, kt in itertools.product((0, 1), (0, 1), (0, 1, 2, 3)):
+        inp = si.mask_parity(full_in, dims, 1 - parity)
+        x = si.mask_parity(full_x, dims, parity)
+        want = oracle.kernel(inp, x, bench.U, po, parity, dagger, kt)
+        for prec in PRECS:
+            got = bench.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, prec, tm.TM_RECON_8, nf)
+            assert ",8," in tm.tm_last_kernel_name(bench.lat.ctx)
+            err = rel_l2(got, want)
+            worst[prec] = max(worst.get(prec, 0.0), err)
+            assert err <= TOL[prec], (PREC_NAME[prec], parity, dagger, kt, err)
+    print("worst rel L2 (8-real):", {PREC_NAME[k]: v for k, v in worst.items()})
+
+
+def test_t2c_recon8_composites_and_singular_chart():
+    dims = (4, 4, 6, 8)
+    bench = bench_for(dims, "haar", 7)
+    kw = dict(mu=0.15, epsilon=0.19, twist_flavor=0)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    psi_e = si.mask_parity(si.spinor_field(dims, 2, 14), dims, 0)
+    b_o = si.mask_parity(si.spinor_field(dims, 2, 15), dims, 1)
+    for prec in PRECS:
+        for typ, dagger in ((tm.TM_MATPC_ASYM, 0), (tm.TM_MATPC_ASYM, 1), (tm.TM_MATPC_SYM, 0), (tm.TM_MATPC_SYM, 1)):
+            want = oracle.matpc_adjoint(psi_e, bench.U, po, typ) if dagger else oracle.matpc(psi_e, bench.U, po, typ, 0)
+            assert rel_l2(bench.matpc(psi_e, pg, typ, dagger, prec, tm.TM_RECON_8, 2), want) <= TOL[prec], (PREC_NAME[prec], typ, dagger)
+        want = oracle.reconstruct_odd(psi_e, b_o, bench.U, po)
+        assert rel_l2(bench.reconstruct_odd(psi_e, b_o, pg, prec, tm.TM_RECON_8, 2), want) <= TOL[prec]
+    # the unit matrix sits on the chart's singular point: refused at load time, not NaN at run time
+    unit = np.zeros((4, bench.lat.V, 3, 3), dtype=np.complex128)
+    unit[:, :, [0, 1, 2], [0, 1, 2]] = 1.0
+    with pytest.raises(tm.TmError) as ei:
+        bench.lat.gauge(unit, tm.TM_DOUBLE, tm.TM_RECON_8)
+    assert ei.value.status == tm.TM_ERR_PARAM
+
+
 # ---- T3: composites; BASELINE.json config 1 -------------------------------------------------------
 
 @pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
