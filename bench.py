@@ -252,7 +252,7 @@ def run_reference(args, log):
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": "GFLOPS", "n_gpus": args.gpus, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": WORKLOAD, "sample": sample},
+           "config": {"workload": WORKLOAD % (RECON, RECON), "sample": sample},
            "cpu_baseline": {"value": val, "unit": "GFLOPS", "cores": cores, "kind": "oracle", "sample": sample},
            "e2e": {"value": val, "unit": "GFLOPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
@@ -260,8 +260,10 @@ def run_reference(args, log):
 
 
 METRIC = "twisted-mass dslash GFLOPS (even-odd preconditioned operators, Eq. 2.2/2.3, 32^3x64, fp64+fp32+half sweep)"
-WORKLOAD = ("32^3x64: configs[2] degenerate (Haar links, 12-real, mu=0.0015) ASYM+SYM in fp64/fp32/half + configs[3] "
-            "non-degenerate (exp(i0.3H) links, 12-real, mu=0.15, eps=0.19) ASYM plain+dagger in fp32/half")
+WORKLOAD = ("32^3x64: configs[2] degenerate (Haar links, %d-real, mu=0.0015) ASYM+SYM in fp64/fp32/half + configs[3] "
+            "non-degenerate (exp(i0.3H) links, %d-real, mu=0.15, eps=0.19) ASYM plain+dagger in fp32/half")
+# plain-ALU peak: 128 FP32 / 64 FP64 FMA lanes per SM, 148 SMs, 2 flop per FMA, at the SM clock under load
+SMS, LANES = 148, {8: 64, 4: 128, 2: 128}
 
 
 def run_ours(args, log):
@@ -336,7 +338,7 @@ def run_ours(args, log):
                         "launches": cnt, "us": 1e3 * avg_ms, "gflops": f / (avg_ms * 1e-3) / 1e9,
                         "alg_gbs": gbs, "frac_of_measured_peak": gbs / peak, "frac_of_8TBs": gbs / 8000.0,
                         "bytes_per_site": bytes_per_site(nf, prec, RECON, kt), "flops_per_site": flops_per_site(nf, kt),
-                        "share_of_step": tot / total_ms})
+                        "share_of_step": tot / total_ms, "prec_bytes": prec})
     dom = max(kernels, key=lambda k: k["share_of_step"]) if kernels else None
     roofline = None
     if dom:
@@ -373,11 +375,17 @@ def run_ours(args, log):
         cpu = {"value": f / s / 1e9, "unit": "GFLOPS", "cores": ora.num_threads(), "kind": "oracle", "sample": sample,
                "seconds": s}
 
+    # second roofline per kernel: useful flops against the plain-ALU peak at the clock seen under load
+    sm_mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0
+    for k in kernels:
+        alu_peak = SMS * LANES[k.pop("prec_bytes")] * 2 * sm_mhz * 1e-3      # GFLOPS
+        k["alu_peak_gflops"] = alu_peak
+        k["frac_of_alu_peak"] = k["gflops"] / alu_peak
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": "GFLOPS", "n_gpus": world, "steps": args.steps,
                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                "vs_baseline": None, "dtype": "f64+f32+i16/f32", "data": "synthetic",
-               "config": {"workload": WORKLOAD, "lattice": list(DIMS), "recon": RECON, "kappa": KAPPA,
+               "config": {"workload": WORKLOAD % (RECON, RECON), "lattice": list(DIMS), "recon": RECON, "kappa": KAPPA,
                           "parallelism": "replicas only (path does not shard)" if world > 1 else "single GPU",
                           "l2": "inputs larger than L2 (gauge fields 201-805 MB each, 2.3 GB touched per step)"},
                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
@@ -399,7 +407,11 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--path", type=int, default=0, help="tm_set_path: 0 = default kernel selection, 1 = scalar kernels only")
+    ap.add_argument("--recon", type=int, default=12, choices=[18, 12, 8],
+                    help="reals stored per link (BASELINE.json configs[2], configs[3]: 12); 18 and 8 are the other rows of the paper's Table 1")
     args = ap.parse_args()
+    global RECON
+    RECON = args.recon
     rank = int(os.environ.get("RANK", "0"))
 
     def log(msg):
