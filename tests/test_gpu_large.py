@@ -131,6 +131,14 @@ def test_config3_32c64_degenerate_precision_sweep(case3, prec, typ):
     print("config3", PREC_NAME[prec], typ, "rel L2 on samples = %.3e" % err)
 
 
+@pytest.mark.parametrize("prec", [tm.TM_DOUBLE, tm.TM_SINGLE], ids=["fp64", "fp32"])
+def test_config3_32c64_8real_links(case3, prec):
+    """The same Eq. 2.2 operator with 8-real links (Table 1's "8" rows; `python bench.py --recon 8` times this launch
+    configuration): fp64 = scalar kernel, fp32 = packed kernel with the fast special-function rebuild."""
+    err = case3.check_matpc(dict(mu=0.0015, epsilon=0.0, twist_flavor=1), prec, tm.TM_RECON_8, tm.TM_MATPC_ASYM, 0, 33)
+    print("config3 8-real", PREC_NAME[prec], "rel L2 on samples = %.3e" % err)
+
+
 @pytest.mark.parametrize("prec", [tm.TM_SINGLE, tm.TM_HALF], ids=["fp32", "half"])
 @pytest.mark.parametrize("dagger", [0, 1], ids=["plain", "dagger"])
 def test_config4_32c64_nondegenerate_doublet(case4, prec, dagger):

@@ -218,6 +218,29 @@ def test_t3b_config1_solve_check():
         assert rel_l2(rec, psi_o) <= 1e-12
 
 
+def test_t3b2_config1_against_the_stored_oracle_samples():
+    """The same configs[0] inputs against tests/golden/config1_matpc_asym.txt (oracle outputs stored by a committed
+    script that calls only oracle/): sampled components of the LHS of Eq. 2.2 and of Eq. 2.4, fp64, every recon."""
+    import os
+    dims = (4, 4, 4, 8)
+    kw = dict(mu=0.004, epsilon=0.0, twist_flavor=1)
+    bench = bench_for(dims, "haar", 1)
+    pg = tm.params(KAPPA, **kw)
+    psi_e = si.mask_parity(si.spinor_field(dims, 1, 1), dims, 0)
+    b_o = si.mask_parity(si.spinor_field(dims, 1, 2), dims, 1)
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config1_matpc_asym.txt"))
+            if not l.startswith("#")]
+    for recon in RECONS + [tm.TM_RECON_8]:
+        got = {"matpc_asym": bench.matpc(psi_e, pg, tm.TM_MATPC_ASYM, 0, tm.TM_DOUBLE, recon, 1),
+               "reconstruct_odd": bench.reconstruct_odd(psi_e, b_o, pg, tm.TM_DOUBLE, recon, 1)}
+        for name, s, sp, c, re, im in rows:
+            a = got[name]
+            if int(s) < 0:
+                assert abs(np.linalg.norm(a.ravel()) - float(re)) <= 1e-12 * float(re)
+            else:
+                assert abs(a[0, int(s), int(sp), int(c)] - complex(float(re), float(im))) <= 1e-12 * 10
+
+
 # ---- T3c: the local twist, the twist-free hopping forms, the adjoint of SYM, right-hand sides ----------
 
 @pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])

@@ -537,3 +537,27 @@ def test_input_generators_are_special_unitary_and_seeded():
     h = si.haar_su3(20000, 3)
     assert np.abs(h.mean(axis=0)).max() < 0.02
     assert np.abs((np.abs(h) ** 2).mean(axis=0) - 1 / 3).max() < 0.01
+
+
+def test_golden_config1_file_is_what_the_oracle_computes():
+    """tests/golden/config1_matpc_asym.txt (written by tests/golden/make_config1_golden.py from oracle/ only) guards the
+    oracle's arithmetic against silent changes; it is a regression guard, not a pin (the paper prints no values)."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_config1_golden", os.path.join(here, "make_config1_golden.py"))
+    mk = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mk)
+    fields = dict(zip(("matpc_asym", "reconstruct_odd"), mk.compute()))
+    n = 0
+    for line in open(os.path.join(here, "config1_matpc_asym.txt")):
+        if line.startswith("#"):
+            continue
+        name, s, sp, c, re, im = line.split()
+        a = fields[name]
+        if int(s) < 0:
+            assert abs(np.linalg.norm(a.ravel()) - float(re)) <= 1e-13 * float(re)
+        else:
+            assert abs(a[0, int(s), int(sp), int(c)] - complex(float(re), float(im))) <= 1e-13
+        n += 1
+    assert n == 26
