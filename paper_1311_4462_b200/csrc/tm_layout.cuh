@@ -214,9 +214,47 @@ TM_DEV void rebuild_row2(real *u)
 //   b2 = (r1 a2 - conj(a3) r2) / N ,  b3 = (conj(a2) r2 + a3 r1) / N ,   r1 = -conj(a1) b1 ,  r2 = conj(c1),
 // and row 2 = conj(row0 x row1) as for 12-real.  The chart is singular at N = 0 (tm_gauge_load refuses such links).
 TM_DEV void tm_sincospi(float x, float *s, float *c) { sincospif(x, s, c); }
-TM_DEV void tm_sincospi(double x, double *s, double *c) { sincospi(x, s, c); }
-TM_DEV float tm_sqrt(float x) { return sqrtf(x); }
-TM_DEV double tm_sqrt(double x) { return sqrt(x); }
+TM_DEV float tm_sqrt_pos(float x) { return sqrtf(x); }
+TM_DEV float tm_rcp(float x) { return 1.f / x; }
+// fp64: branch-free forms (the library sincospi / sqrt / division carry slow paths and made the 8-real kernel FP64-pipe
+// and branch bound).  |x| <= 1: q = rint(2x), r = x - q/2 in [-1/4, 1/4] (exact), Taylor polynomials of sin(pi r) and
+// cos(pi r) to r^17 / r^18 (truncation < 1e-19), then the quadrant rotation.  Max error ~2e-16.
+TM_DEV void tm_sincospi(double x, double *s, double *c)
+{
+    const double q = rint(x + x);
+    const double r = fma(q, -0.5, x), r2 = r * r;
+    const double S[9] = {3.14159265358979312e+00, -5.16771278004996937e+00, 2.55016403987734508e+00, -5.99264529320791883e-01, 8.21458866111281910e-02, -7.37043094571434784e-03, 4.66302805767612337e-04, -2.19153534478302037e-05, 7.95205400147550838e-07};
+    const double C[10] = {1.00000000000000000e+00, -4.93480220054467900e+00, 4.05871212641676760e+00, -1.33526276885458928e+00, 2.35330630358893123e-01, -2.58068913900140508e-02, 1.92957430940392206e-03, -1.04638104924845650e-04, 4.30306958703294391e-06, -1.38789524622137608e-07};
+    double ps = S[8], pc = C[9];
+#pragma unroll
+    for (int k = 7; k >= 0; k--) ps = fma(ps, r2, S[k]);
+#pragma unroll
+    for (int k = 8; k >= 0; k--) pc = fma(pc, r2, C[k]);
+    ps *= r;
+    const int iq = (int)q;                       // -2 .. 2
+    const double a = (iq & 1) ? pc : ps, b = (iq & 1) ? ps : pc;      // sin, cos before the signs
+    *s = (iq & 2) ? -a : a;
+    *c = ((iq + 1) & 2) ? -b : b;
+}
+// sqrt(x) for x >= 0 and 1/x for x > 0 from the approximate units + two Newton steps (relative error ~1e-16)
+TM_DEV double tm_sqrt_pos(double x)
+{
+    const double xs = fmax(x, 1e-300);
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(xs));
+    y = y * fma(-0.5 * xs * y, y, 1.5);
+    y = y * fma(-0.5 * xs * y, y, 1.5);
+    const double r = x * y;                       // ~ sqrt(x); one correction step on the root itself
+    return fma(0.5 * y, fma(-r, r, x), r);
+}
+TM_DEV double tm_rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    y = y * fma(-x, y, 2.0);
+    y = y * fma(-x, y, 2.0);
+    return y * fma(-x, y, 2.0);
+}
 template <typename real>
 TM_DEV void rebuild_from8(real *u, const real *p)
 {
@@ -225,12 +263,12 @@ TM_DEV void rebuild_from8(real *u, const real *p)
     real s1, c1, s2, c2;
     tm_sincospi(p[6], &s1, &c1);
     tm_sincospi(p[7], &s2, &c2);
-    const real m1 = tm_sqrt(max((real)1 - N, (real)0));
-    const real m2 = tm_sqrt(max(N - tm_fma(b1r, b1r, b1i * b1i), (real)0));
+    const real m1 = tm_sqrt_pos(max((real)1 - N, (real)0));
+    const real m2 = tm_sqrt_pos(max(N - tm_fma(b1r, b1r, b1i * b1i), (real)0));
     const real a1r = m1 * c1, a1i = m1 * s1;
     const real r2r = m2 * c2, r2i = -(m2 * s2);                               // conj(c1)
     const real r1r = -tm_fma(a1r, b1r, a1i * b1i), r1i = tm_fma(a1i, b1r, -(a1r * b1i));   // -conj(a1) b1
-    const real iN = (real)1 / N;
+    const real iN = tm_rcp(N);
     u[0] = a1r; u[1] = a1i; u[2] = a2r; u[3] = a2i; u[4] = a3r; u[5] = a3i;
     u[6] = b1r; u[7] = b1i;
     u[8] = (tm_fma(r1r, a2r, -(r1i * a2i)) - tm_fma(a3r, r2r, a3i * r2i)) * iN;
