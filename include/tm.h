@@ -108,6 +108,21 @@ int tm_field_download(const tm_field *f, tm_parity parity, double *host_full);
 int tm_field_upload_cb(tm_field *f, tm_parity parity, const double *host_cb);
 int tm_field_download_cb(const tm_field *f, tm_parity parity, double *host_cb);
 
+/* ---- host spin basis (SURVEY.md section 8f "minor": chiral <-> non-relativistic rotation in the pack kernels) ---- */
+/* The kernels work in the non-relativistic basis of PAPER.md:52 (gamma_4 diagonal; reading C5), which is also
+ * the default basis of host spinors.  With another host basis the pack / unpack kernels of tm_field_upload* /
+ * tm_field_download* rotate the spin index: psi_device = S psi_host on upload, psi_host = S^dag psi_device on download,
+ * where S is unitary with  gamma^host_mu = S^dag gamma^nonrel_mu S.  The setting belongs to the context and applies to
+ * every later upload / download; fields already on the device are not touched.
+ *   TM_BASIS_NONREL : S = 1 (default; `custom` ignored)
+ *   TM_BASIS_CHIRAL : S = (1/sqrt 2) [[1, 1], [1, -1]] in 2x2 spin blocks, i.e. the chiral basis with
+ *                     gamma_k = [[0, -i s_k], [i s_k, 0]], gamma_4 = [[0, 1], [1, 0]], gamma_5 = diag(1, 1, -1, -1)
+ *                     (reading C12; `custom` ignored)
+ *   TM_BASIS_CUSTOM : `custom` = HOST pointer to S as 32 doubles, row-major [4][4][re, im]; copied; must be unitary to
+ *                     1e-12 (else TM_ERR_ARG)                                                                       */
+typedef enum { TM_BASIS_NONREL = 0, TM_BASIS_CHIRAL = 1, TM_BASIS_CUSTOM = 2 } tm_basis;
+int tm_set_host_basis(tm_ctx *ctx, tm_basis basis, const double *custom);
+
 /* ---- gauge (a1, a4) -------------------------------------------------------------------------------- */
 /* host_links: HOST pointer, canonical gauge field; copied (may be freed on return). */
 int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_recon recon, tm_gauge **g);

@@ -27,10 +27,11 @@ TM_EVEN, TM_ODD = 0, 1
 TM_TWIST_INV_DSLASH, TM_TWIST_INV_DSLASH_XPAY, TM_DSLASH_TWIST_XPAY, TM_RECONSTRUCT = 0, 1, 2, 3
 TM_DSLASH_XPAY, TM_DSLASH_AXPY = 4, 5
 TM_MATPC_ASYM, TM_MATPC_SYM = 0, 1
+TM_BASIS_NONREL, TM_BASIS_CHIRAL, TM_BASIS_CUSTOM = 0, 1, 2
 
 EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
-    "tm_field_device_ptr", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb",
+    "tm_field_device_ptr", "tm_set_host_basis", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb",
     "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_twist_apply",
     "tm_prepare_rhs", "tm_field_axpby", "tm_field_redot", "tm_invert_cg", "tm_last_error",
     "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_set_tuning", "tm_timing_enable", "tm_timing_read",
@@ -107,6 +108,7 @@ def lib():
     L.tm_last_kernel_name.argtypes = [vp]
     L.tm_last_kernel_name.restype = ctypes.c_char_p
     L.tm_set_path.argtypes = [vp, i]
+    L.tm_set_host_basis.argtypes = [vp, i, vp]
     L.tm_set_tuning.argtypes = [vp, ctypes.c_char_p, i]
     L.tm_timing_enable.argtypes = [vp, i]
     L.tm_timing_read.argtypes = [vp, i, ctypes.POINTER(ctypes.c_char_p), ctypes.POINTER(ctypes.c_float),
@@ -239,6 +241,15 @@ def tm_launch_count(ctx):
 
 def tm_last_kernel_name(ctx):
     return lib().tm_last_kernel_name(ctx).decode()
+
+
+def tm_set_host_basis(ctx, basis, custom=None):
+    """custom: complex 4x4 (numpy) for TM_BASIS_CUSTOM."""
+    ptr = None
+    if custom is not None:
+        custom = np.ascontiguousarray(custom, dtype=np.complex128).reshape(4, 4)
+        ptr = custom.ctypes.data_as(ctypes.c_void_p)
+    _check(lib().tm_set_host_basis(ctx, int(basis), ptr))
 
 
 def tm_set_path(ctx, path):

@@ -149,6 +149,8 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->stage = -1;
     c->block_threads = 0;
     c->sm_count = 0;
+    c->basis_on = 0;
+    for (int k = 0; k < 32; k++) c->basis[k] = 0.0;
     c->staging = nullptr;
     c->staging_bytes = 0;
     c->red = nullptr;
@@ -214,6 +216,45 @@ int tm_timing_read(tm_ctx *ctx, int max_records, const char **names, float *ms, 
     }
     *n = k;
     clear_timed(ctx);
+    return TM_OK;
+}
+
+int tm_set_host_basis(tm_ctx *ctx, tm_basis basis, const double *custom)
+{
+    if (!ctx) return fail(TM_ERR_ARG, "tm_set_host_basis: NULL context");
+    double m[32];
+    for (int k = 0; k < 32; k++) m[k] = 0.0;
+    if (basis == TM_BASIS_NONREL) {
+        ctx->basis_on = 0;
+        return TM_OK;
+    } else if (basis == TM_BASIS_CHIRAL) {
+        // S = (1 / sqrt 2) [[1, 1], [1, -1]] (2x2 spin blocks): gamma^chiral = S gamma^nonrel S, gamma5^chiral = diag(1,1,-1,-1)
+        const double h = 0.70710678118654752440;
+        for (int a = 0; a < 2; a++) {
+            m[((a) * 4 + a) * 2] = h;
+            m[((a) * 4 + a + 2) * 2] = h;
+            m[((a + 2) * 4 + a) * 2] = h;
+            m[((a + 2) * 4 + a + 2) * 2] = -h;
+        }
+    } else if (basis == TM_BASIS_CUSTOM) {
+        if (!custom) return fail(TM_ERR_ARG, "tm_set_host_basis: TM_BASIS_CUSTOM needs the matrix");
+        for (int k = 0; k < 32; k++) m[k] = custom[k];
+        for (int a = 0; a < 4; a++)           // S S^dag = 1
+            for (int b = 0; b < 4; b++) {
+                double re = 0.0, im = 0.0;
+                for (int t = 0; t < 4; t++) {
+                    const double ar = m[(a * 4 + t) * 2], ai = m[(a * 4 + t) * 2 + 1], br = m[(b * 4 + t) * 2], bi = -m[(b * 4 + t) * 2 + 1];
+                    re += ar * br - ai * bi;
+                    im += ar * bi + ai * br;
+                }
+                if (std::fabs(re - (a == b ? 1.0 : 0.0)) > 1e-12 || std::fabs(im) > 1e-12)
+                    return fail(TM_ERR_ARG, "tm_set_host_basis: the matrix is not unitary (S S^dag [%d][%d] = %g%+gi)", a, b, re, im);
+            }
+    } else {
+        return fail(TM_ERR_ARG, "tm_set_host_basis: bad basis %d", (int)basis);
+    }
+    for (int k = 0; k < 32; k++) ctx->basis[k] = m[k];
+    ctx->basis_on = 1;
     return TM_OK;
 }
 

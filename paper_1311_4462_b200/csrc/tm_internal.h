@@ -37,6 +37,8 @@ struct tm_ctx {
     int stage;   // tm_set_tuning("stage_links"): -1 library default, 0 direct loads, 1 links staged through shared memory
     int block_threads;   // tm_set_tuning("block_threads"): 0 library default, else 32 / 64 / 128
     int sm_count;
+    int basis_on;         // tm_set_host_basis: host spinors are in another spin basis, psi_device = S psi_host
+    double basis[32];     // S, row-major [4][4][re, im]
     void *staging;        // device staging for upload / download
     double *red;          // reduction scratch of tm_blas.cu: [0] result, [1..] per-block partial sums
     size_t red_n;
@@ -123,6 +125,7 @@ cudaError_t tm_blas_redot(const tm_field *x, const tm_field *y, double *out);
 cudaError_t tm_blas_cg_update(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr);
 
 // pack / unpack (tm_pack.cu)
+// (both apply the context's host spin basis: S on the way in, S^dag on the way out)
 cudaError_t tm_pack_spinor(const tm_field *f, int parity, const double *dev_src, bool src_is_cb, cudaStream_t s);
 cudaError_t tm_unpack_spinor(const tm_field *f, int parity, double *dev_dst, bool dst_is_cb, cudaStream_t s);
 cudaError_t tm_pack_gauge(const tm_gauge *g, const double *dev_src, cudaStream_t s);

@@ -10,6 +10,35 @@ struct PackGeom {
     long V;
 };
 
+// host spin basis (tm_set_host_basis): w = S v (ADJ = false) or S^dag v (ADJ = true) on the spin index, color by color
+struct SpinRot {
+    int on;
+    double m[32];        // S[row][col][re, im]
+};
+template <bool ADJ>
+__device__ __forceinline__ void spin_rotate(double *v, const SpinRot &r)
+{
+    double w[24];
+#pragma unroll
+    for (int s = 0; s < 4; s++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            double re = 0.0, im = 0.0;
+#pragma unroll
+            for (int t = 0; t < 4; t++) {
+                const double mr = ADJ ? r.m[(t * 4 + s) * 2] : r.m[(s * 4 + t) * 2];
+                const double mi = ADJ ? -r.m[(t * 4 + s) * 2 + 1] : r.m[(s * 4 + t) * 2 + 1];
+                const double xr = v[(t * 3 + c) * 2], xi = v[(t * 3 + c) * 2 + 1];
+                re += mr * xr - mi * xi;
+                im += mr * xi + mi * xr;
+            }
+            w[(s * 3 + c) * 2] = re;
+            w[(s * 3 + c) * 2 + 1] = im;
+        }
+#pragma unroll
+    for (int k = 0; k < 24; k++) v[k] = w[k];
+}
+
 __device__ __forceinline__ long cb_to_lex(const PackGeom &g, int i, int parity)
 {
     int r = i / g.Xh;
@@ -21,21 +50,25 @@ __device__ __forceinline__ long cb_to_lex(const PackGeom &g, int i, int parity)
 }
 
 template <int PREC>
-__global__ void pack_spinor_kernel(char *dst, const double *src, PackGeom g, int parity, int nf, bool src_is_cb)
+__global__ void pack_spinor_kernel(char *dst, const double *src, PackGeom g, int parity, int nf, bool src_is_cb, SpinRot rot)
 {
     typedef typename PrecTraits<PREC>::real real;
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= nf * g.Vh) return;
     const int f = tid / g.Vh, i = tid % g.Vh;
     const double *s = src_is_cb ? src + ((size_t)f * g.Vh + i) * 24 : src + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
+    double d[24];
+#pragma unroll
+    for (int k = 0; k < 24; k++) d[k] = s[k];
+    if (rot.on) spin_rotate<false>(d, rot);
     real v[24];
 #pragma unroll
-    for (int k = 0; k < 24; k++) v[k] = (real)s[k];
+    for (int k = 0; k < 24; k++) v[k] = (real)d[k];
     store_spinor<PREC>(v, dst + spinor_site_off(PREC, nf, i, f), i & (TM_TILE - 1));
 }
 
 template <int PREC>
-__global__ void unpack_spinor_kernel(double *dst, const char *src, PackGeom g, int parity, int nf, bool dst_is_cb)
+__global__ void unpack_spinor_kernel(double *dst, const char *src, PackGeom g, int parity, int nf, bool dst_is_cb, SpinRot rot)
 {
     typedef typename PrecTraits<PREC>::real real;
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -44,8 +77,12 @@ __global__ void unpack_spinor_kernel(double *dst, const char *src, PackGeom g, i
     real v[24];
     load_spinor<PREC, 0>(v, src + spinor_site_off(PREC, nf, i, f), i & (TM_TILE - 1));
     double *d = dst_is_cb ? dst + ((size_t)f * g.Vh + i) * 24 : dst + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
+    double o[24];
 #pragma unroll
-    for (int k = 0; k < 24; k++) d[k] = (double)v[k];
+    for (int k = 0; k < 24; k++) o[k] = (double)v[k];
+    if (rot.on) spin_rotate<true>(o, rot);
+#pragma unroll
+    for (int k = 0; k < 24; k++) d[k] = o[k];
 }
 
 // one thread per (parity, mu, cb site): U_mu(x) for x of that parity
@@ -104,6 +141,14 @@ __global__ void pack_gauge_kernel(char *dst, const double *src, PackGeom g)
     }
 }
 
+SpinRot rot_of(const tm_ctx *c)
+{
+    SpinRot r;
+    r.on = c->basis_on;
+    for (int k = 0; k < 32; k++) r.m[k] = c->basis[k];
+    return r;
+}
+
 PackGeom geom_of(const tm_ctx *c)
 {
     PackGeom g;
@@ -122,22 +167,24 @@ PackGeom geom_of(const tm_ctx *c)
 cudaError_t tm_pack_spinor(const tm_field *f, int parity, const double *dev_src, bool src_is_cb, cudaStream_t s)
 {
     const PackGeom g = geom_of(f->ctx);
+    const SpinRot rot = rot_of(f->ctx);
     const int n = f->nf * g.Vh, threads = 128, blocks = (n + threads - 1) / threads;
     char *dst = static_cast<char *>(f->ptr);
-    if (f->prec == 8) pack_spinor_kernel<8><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb);
-    else if (f->prec == 4) pack_spinor_kernel<4><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb);
-    else pack_spinor_kernel<2><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb);
+    if (f->prec == 8) pack_spinor_kernel<8><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb, rot);
+    else if (f->prec == 4) pack_spinor_kernel<4><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb, rot);
+    else pack_spinor_kernel<2><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb, rot);
     return cudaGetLastError();
 }
 
 cudaError_t tm_unpack_spinor(const tm_field *f, int parity, double *dev_dst, bool dst_is_cb, cudaStream_t s)
 {
     const PackGeom g = geom_of(f->ctx);
+    const SpinRot rot = rot_of(f->ctx);
     const int n = f->nf * g.Vh, threads = 128, blocks = (n + threads - 1) / threads;
     const char *src = static_cast<const char *>(f->ptr);
-    if (f->prec == 8) unpack_spinor_kernel<8><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb);
-    else if (f->prec == 4) unpack_spinor_kernel<4><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb);
-    else unpack_spinor_kernel<2><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb);
+    if (f->prec == 8) unpack_spinor_kernel<8><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb, rot);
+    else if (f->prec == 4) unpack_spinor_kernel<4><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb, rot);
+    else unpack_spinor_kernel<2><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb, rot);
     return cudaGetLastError();
 }
 

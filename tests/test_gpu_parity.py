@@ -327,6 +327,59 @@ def test_t4_asym_composite_adjointness_on_gpu(kw):
         assert abs(lhs - rhs) <= tol * np.linalg.norm(phi) * np.linalg.norm(m_psi)
 
 
+# ---- T5: host spin basis (SURVEY.md section 8f "minor": chiral <-> non-relativistic rotation in the pack kernels) ----
+
+def test_t5_host_spin_basis_chiral_and_custom():
+    dims = (4, 4, 6, 8)
+    bench = bench_for(dims, "haar", 7)
+    lat, ctx = bench.lat, bench.lat.ctx
+    one = np.eye(2)
+    S = np.block([[one, one], [one, -one]]).astype(np.complex128) / np.sqrt(2.0)
+    rot = lambda M, a: np.einsum("st,fvtc->fvsc", M, a)
+    kw = dict(mu=0.15, epsilon=0.19, twist_flavor=0)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    psi_c = si.spinor_field(dims, 2, 61)                       # read as components in the chiral basis
+    x_c = si.mask_parity(si.spinor_field(dims, 2, 62), dims, 1)
+    try:
+        # 1. upload in the chiral basis, download in the kernels' basis: psi_device = S psi_host
+        tm.tm_set_host_basis(ctx, tm.TM_BASIS_CHIRAL)
+        f = lat.field(tm.TM_DOUBLE, 2).upload(0, psi_c)
+        assert rel_l2(f.download(0), si.mask_parity(psi_c, dims, 0)) <= 1e-15       # round trip S^dag S
+        tm.tm_set_host_basis(ctx, tm.TM_BASIS_NONREL)
+        assert rel_l2(f.download(0), si.mask_parity(rot(S, psi_c), dims, 0)) <= 1e-15
+        # 2. gamma5 is diagonal in the chiral basis: (1 + i a gamma5 tau3) multiplies the upper / lower spin halves of
+        #    flavor 0 by (1 +- i a) when epsilon = 0 -- a closed form that does not go through S
+        kw0 = dict(mu=0.3, epsilon=0.0, twist_flavor=0)
+        tm.tm_set_host_basis(ctx, tm.TM_BASIS_CHIRAL)
+        fin, fout = lat.field(tm.TM_DOUBLE, 2).upload(0, psi_c), lat.field(tm.TM_DOUBLE, 2)
+        tm.twist_apply(fout, fin, tm.params(KAPPA, **kw0), 0, 0)
+        got, a = fout.download(0), 2 * KAPPA * 0.3
+        want = si.mask_parity(psi_c, dims, 0)
+        want[0, :, :2] *= 1 + 1j * a
+        want[0, :, 2:] *= 1 - 1j * a
+        want[1, :, :2] *= 1 - 1j * a
+        want[1, :, 2:] *= 1 + 1j * a
+        assert rel_l2(got, want) <= 1e-14
+        # 3. every kernel type with chiral host fields = S^dag oracle(S .) in all precisions
+        inp_c = si.mask_parity(psi_c, dims, 0)
+        for kt, dagger in itertools.product((0, 1, 2, 3), (0, 1)):
+            want = rot(S.conj().T, oracle.kernel(rot(S, inp_c), rot(S, x_c), bench.U, po, 1, dagger, kt))
+            for prec in PRECS:
+                got = bench.kernel(inp_c, None if kt == 0 else x_c, pg, 1, dagger, kt, prec, tm.TM_RECON_12, 2)
+                assert rel_l2(got, want) <= TOL[prec], (PREC_NAME[prec], kt, dagger)
+        # 4. a custom unitary basis; a non-unitary matrix is refused
+        q, _ = np.linalg.qr(np.random.default_rng(5).normal(size=(4, 4)) + 1j * np.random.default_rng(6).normal(size=(4, 4)))
+        tm.tm_set_host_basis(ctx, tm.TM_BASIS_CUSTOM, q)
+        f = lat.field(tm.TM_DOUBLE, 2).upload(1, psi_c)
+        tm.tm_set_host_basis(ctx, tm.TM_BASIS_NONREL)
+        assert rel_l2(f.download(1), si.mask_parity(rot(q, psi_c), dims, 1)) <= 1e-15
+        with pytest.raises(tm.TmError) as ei:
+            tm.tm_set_host_basis(ctx, tm.TM_BASIS_CUSTOM, 1.01 * q)
+        assert ei.value.status == tm.TM_ERR_ARG
+    finally:
+        tm.tm_set_host_basis(ctx, tm.TM_BASIS_NONREL)
+
+
 # ---- T6: error paths of the boundary --------------------------------------------------------------
 
 def test_t6_error_paths():

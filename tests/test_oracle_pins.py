@@ -561,3 +561,22 @@ def test_golden_config1_file_is_what_the_oracle_computes():
             assert abs(a[0, int(s), int(sp), int(c)] - complex(float(re), float(im))) <= 1e-13
         n += 1
     assert n == 26
+
+
+def test_p15_chiral_basis_of_the_boundary_is_a_rotation_of_the_declared_basis():
+    """include/tm.h TM_BASIS_CHIRAL (reading C12): the chiral matrices written out here satisfy the Clifford
+    algebra with gamma5 = g1 g2 g3 g4 = diag(1,1,-1,-1), and S = (1/sqrt2) [[1,1],[1,-1]] maps them onto the oracle's
+    non-relativistic matrices: S gamma^chiral S^dag = gamma^nonrel."""
+    s = [np.array([[0, 1], [1, 0]], dtype=complex), np.array([[0, -1j], [1j, 0]]), np.array([[1, 0], [0, -1]], dtype=complex)]
+    z, one = np.zeros((2, 2), dtype=complex), np.eye(2, dtype=complex)
+    gc = [np.block([[z, -1j * sk], [1j * sk, z]]) for sk in s] + [np.block([[z, one], [one, z]])]
+    for a in range(4):
+        assert np.allclose(gc[a], gc[a].conj().T)
+        for b in range(4):
+            assert np.allclose(gc[a] @ gc[b] + gc[b] @ gc[a], 2.0 * (a == b) * np.eye(4))
+    assert np.allclose(gc[0] @ gc[1] @ gc[2] @ gc[3], np.diag([1, 1, -1, -1]))
+    S = np.block([[one, one], [one, -one]]) / np.sqrt(2.0)
+    assert np.allclose(S @ S.conj().T, np.eye(4))
+    for a in range(4):
+        assert np.allclose(S @ gc[a] @ S.conj().T, oracle.gamma(a), atol=1e-15)
+    assert np.allclose(S @ np.diag([1, 1, -1, -1]) @ S.conj().T, oracle.gamma(4), atol=1e-15)
