@@ -155,6 +155,8 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->staging_bytes = 0;
     c->red = nullptr;
     c->red_n = 0;
+    c->cgs = nullptr;
+    c->cgs_host = nullptr;
     c->timing = false;
     e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
     if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaDeviceGetAttribute"); }
@@ -182,6 +184,8 @@ void tm_finalize(tm_ctx *ctx)
     if (!ctx) return;
     if (ctx->staging) cudaFree(ctx->staging);
     if (ctx->red) cudaFree(ctx->red);
+    if (ctx->cgs) cudaFree(ctx->cgs);
+    if (ctx->cgs_host) cudaFreeHost(ctx->cgs_host);
     for (auto &t : ctx->timed) { cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
     delete ctx;
 }
@@ -615,6 +619,16 @@ int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, 
     tm_field *te_s = w.make(c, ps, nf), *to_s = w.make(c, ps, nf);
     if (!r_d || !t_d || !te_d || !to_d || !r_s || !p_s || !ap_s || !x_s || !te_s || !to_s) return fail(TM_ERR_NOMEM, "tm_invert_cg: work fields");
 
+    if (!c->cgs) {
+        TM_TRY_CUDA(cudaMalloc(&c->cgs, 4 * sizeof(double)), "cudaMalloc(cg scalars)");
+        TM_TRY_CUDA(cudaHostAlloc(&c->cgs_host, 6 * sizeof(double), cudaHostAllocDefault), "cudaHostAlloc(cg scalars)");
+    }
+    struct EventRing {
+        cudaEvent_t ev[2] = {nullptr, nullptr};
+        ~EventRing() { for (auto e : ev) if (e) cudaEventDestroy(e); }
+    } ring;
+    for (auto &e : ring.ev) TM_TRY_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
+
     double bnorm2 = 0.0, rnorm2 = 0.0;
     TM_TRY_CUDA(tm_blas_redot(b_e, b_e, &bnorm2), "redot");
     TM_TRY_CUDA(tm_blas_axpbyz(x_e, 0.0, b_e, 0.0, nullptr, nullptr), "zero x");        // x = 0
@@ -635,18 +649,38 @@ int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, 
         TM_TRY_CUDA(tm_blas_axpbyz(p_s, 1.0, r_s, 0.0, nullptr, nullptr), "copy p");                  // p = r_s
         rr0 = rr;
         const double target = std::max(cp->delta, 0.5 * cp->tol / relres);
-        for (;;) {
-            TM_TRY(apply_normal(ap_s, p_s, te_s, to_s, gs, p, type));                                  // Ap
-            double pap = 0.0, rr_new = 0.0;
-            TM_TRY_CUDA(tm_blas_redot(p_s, ap_s, &pap), "redot");
+        // Inner loop with DEVICE-RESIDENT scalars: alpha = |r|^2 / <p, A p> and beta = |r_new|^2 / |r|^2 are formed inside the
+        // update kernels from c->cgs, so no step waits for the host.  The scalars of every iteration are copied to a pinned
+        // ring and the host looks at them ONE ITERATION LATE (by then they have arrived): the stopping test and the
+        // breakdown test lag by one iteration, i.e. at most one update more than needed is applied to e.
+        double *sc = c->cgs, *hs = c->cgs_host;
+        hs[0] = rr;
+        TM_TRY_CUDA(cudaMemcpyAsync(sc, hs, sizeof(double), cudaMemcpyHostToDevice, c->stream), "rr -> device");
+        TM_TRY_CUDA(cudaStreamSynchronize(c->stream), "rr -> device");       // hs is reused as the ring below
+        int cur = 0, it = 0, stop = 0;
+        auto look = [&](int slot, int rr_idx) -> int {                        // the scalars of an iteration whose copy has landed
+            TM_TRY_CUDA(cudaEventSynchronize(ring.ev[slot]), "cg scalars");
+            const double pap = hs[3 * slot + 2], rr_new = hs[3 * slot + rr_idx];
             if (!(pap > 0.0)) return fail(TM_ERR_PARAM, "tm_invert_cg: <p, A p> = %g is not positive (breakdown)", pap);
-            const double alpha = rr / pap;
-            TM_TRY_CUDA(tm_blas_cg_update(x_s, r_s, p_s, ap_s, alpha, &rr_new), "cg_update");          // e += a p, r_s -= a Ap
+            if (!(rr_new >= 0.0)) return fail(TM_ERR_PARAM, "tm_invert_cg: |r|^2 = %g (breakdown)", rr_new);
+            if (std::sqrt(rr_new / rr0) <= target) stop = 1;
+            return TM_OK;
+        };
+        int prev_idx = 0;
+        for (;; it++) {
+            TM_TRY(apply_normal(ap_s, p_s, te_s, to_s, gs, p, type));                                                  // Ap
+            TM_TRY_CUDA(tm_blas_redot_dev(p_s, ap_s, nullptr, sc + 2), "redot");                                         // <p, A p>
+            TM_TRY_CUDA(tm_blas_cg_update_dev(x_s, r_s, p_s, ap_s, 0.0, nullptr, sc + cur, sc + 2, sc + (1 - cur)), "cg_update");
+            TM_TRY_CUDA(cudaMemcpyAsync(hs + 3 * (it & 1), sc, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "cg scalars");
+            TM_TRY_CUDA(cudaEventRecord(ring.ev[it & 1], c->stream), "cg scalars");
             info->iterations++;
-            if (std::sqrt(rr_new / rr0) <= target || info->iterations >= cp->max_iter) break;
-            TM_TRY_CUDA(tm_blas_axpbyz(p_s, 1.0, r_s, rr_new / rr, p_s, nullptr), "xpay");             // p = r_s + beta p
-            rr = rr_new;
+            if (it > 0) TM_TRY(look((it - 1) & 1, prev_idx));
+            prev_idx = 1 - cur;
+            if (stop || info->iterations >= cp->max_iter) break;
+            TM_TRY_CUDA(tm_blas_axpbyz_dev(p_s, 1.0, r_s, 0.0, p_s, nullptr, sc + (1 - cur), sc + cur), "xpay");        // p = r_s + beta p
+            cur = 1 - cur;
         }
+        TM_TRY(look(it & 1, prev_idx));                                        // the last iteration's scalars (breakdown test)
         TM_TRY_CUDA(tm_blas_axpbyz(x_e, rn, x_s, 1.0, x_e, nullptr), "x += |r| e");
         TM_TRY(apply_normal(t_d, x_e, te_d, to_d, g_precise, p, type));                                // true residual in double
         TM_TRY_CUDA(tm_blas_axpbyz(r_d, 1.0, b_e, -1.0, t_d, &rnorm2), "r = b - A x");

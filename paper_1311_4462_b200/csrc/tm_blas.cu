@@ -42,8 +42,10 @@ __global__ void __launch_bounds__(256) final_sum_kernel(const double *partial, i
 }
 
 template <int PZ, int PX, int PY, int NF, bool NORM>
-__global__ void __launch_bounds__(BT) axpbyz_kernel(char *z, double a, const char *x, double b, const char *y, int Vh, double *partial)
+__global__ void __launch_bounds__(BT) axpbyz_kernel(char *z, double a, const char *x, double b, const char *y, int Vh, double *partial,
+                                                    const double *bnum, const double *bden)
 {
+    if (bnum) b = *bnum / *bden;                 // device-resident scalar (inner CG: beta = |r_new|^2 / |r|^2)
     const int site = blockIdx.x * BT + threadIdx.x;
     double n2 = 0;
     if (site < Vh) {
@@ -94,9 +96,11 @@ __global__ void __launch_bounds__(BT) redot_kernel(const char *x, const char *y,
 
 // x += a p ; r -= a Ap ; partial |r|^2
 template <int P, int NF>
-__global__ void __launch_bounds__(BT) cg_update_kernel(char *x, char *r, const char *p, const char *Ap, double a, int Vh, double *partial)
+__global__ void __launch_bounds__(BT) cg_update_kernel(char *x, char *r, const char *p, const char *Ap, double a, int Vh, double *partial,
+                                                       const double *anum, const double *aden)
 {
     typedef typename PrecTraits<P>::real real;
+    if (anum) a = *anum / *aden;                 // device-resident scalar (inner CG: alpha = |r|^2 / <p, A p>)
     const int site = blockIdx.x * BT + threadIdx.x;
     double n2 = 0;
     if (site < Vh) {
@@ -136,6 +140,13 @@ cudaError_t reduce_buffers(tm_ctx *c, int blocks)
     return cudaSuccess;
 }
 
+// partials are in c->red[1..blocks]; the sum goes to *dev_out and stays on the device (no synchronisation)
+cudaError_t finish_sum_dev(tm_ctx *c, int blocks, double *dev_out)
+{
+    final_sum_kernel<<<1, 256, 0, c->stream>>>(c->red + 1, blocks, dev_out);
+    return cudaGetLastError();
+}
+
 // partials are in c->red[1..blocks]; the sum goes to c->red[0] and from there to *host (synchronises the stream)
 cudaError_t finish_sum(tm_ctx *c, int blocks, double *host)
 {
@@ -153,6 +164,13 @@ cudaError_t finish_sum(tm_ctx *c, int blocks, double *host)
 // Supported mixes: all equal; z double with x sloppy and y double; z sloppy with x double (y NULL or of z's precision).
 cudaError_t tm_blas_axpbyz(tm_field *z, double a, const tm_field *x, double b, const tm_field *y, double *norm2)
 {
+    return tm_blas_axpbyz_dev(z, a, x, b, y, norm2, nullptr, nullptr);
+}
+
+// the same with b = *bnum / *bden read on the device when bnum != NULL (DEVICE pointers)
+cudaError_t tm_blas_axpbyz_dev(tm_field *z, double a, const tm_field *x, double b, const tm_field *y, double *norm2,
+                               const double *bnum, const double *bden)
+{
     tm_ctx *c = z->ctx;
     const int Vh = c->g.Vh, blocks = (Vh + BT - 1) / BT;
     cudaError_t e = reduce_buffers(c, blocks);
@@ -164,10 +182,10 @@ cudaError_t tm_blas_axpbyz(tm_field *z, double a, const tm_field *x, double b, c
 #define TM_AX(PZ, PX, PY)                                                                                             \
     if (!done && pz == PZ && px == PX && py == PY) {                                                                  \
         done = true;                                                                                                  \
-        if (z->nf == 1) { if (norm2) axpbyz_kernel<PZ, PX, PY, 1, true><<<blocks, BT, 0, c->stream>>>(zp, a, xp, b, yp, Vh, c->red + 1);   \
-                          else axpbyz_kernel<PZ, PX, PY, 1, false><<<blocks, BT, 0, c->stream>>>(zp, a, xp, b, yp, Vh, c->red + 1); }     \
-        else            { if (norm2) axpbyz_kernel<PZ, PX, PY, 2, true><<<blocks, BT, 0, c->stream>>>(zp, a, xp, b, yp, Vh, c->red + 1);   \
-                          else axpbyz_kernel<PZ, PX, PY, 2, false><<<blocks, BT, 0, c->stream>>>(zp, a, xp, b, yp, Vh, c->red + 1); }     \
+        if (z->nf == 1) { if (norm2) axpbyz_kernel<PZ, PX, PY, 1, true><<<blocks, BT, 0, c->stream>>>(zp, a, xp, b, yp, Vh, c->red + 1, bnum, bden);   \
+                          else axpbyz_kernel<PZ, PX, PY, 1, false><<<blocks, BT, 0, c->stream>>>(zp, a, xp, b, yp, Vh, c->red + 1, bnum, bden); }     \
+        else            { if (norm2) axpbyz_kernel<PZ, PX, PY, 2, true><<<blocks, BT, 0, c->stream>>>(zp, a, xp, b, yp, Vh, c->red + 1, bnum, bden);   \
+                          else axpbyz_kernel<PZ, PX, PY, 2, false><<<blocks, BT, 0, c->stream>>>(zp, a, xp, b, yp, Vh, c->red + 1, bnum, bden); }     \
     }
     TM_AX(8, 8, 8) TM_AX(4, 4, 4) TM_AX(2, 2, 2)
     TM_AX(8, 4, 8) TM_AX(8, 2, 8)            // x_double += a * e_sloppy
@@ -181,7 +199,10 @@ cudaError_t tm_blas_axpbyz(tm_field *z, double a, const tm_field *x, double b, c
     return norm2 ? finish_sum(c, blocks, norm2) : cudaSuccess;
 }
 
-cudaError_t tm_blas_redot(const tm_field *x, const tm_field *y, double *out)
+cudaError_t tm_blas_redot(const tm_field *x, const tm_field *y, double *out) { return tm_blas_redot_dev(x, y, out, nullptr); }
+
+// dev_out != NULL: the sum is left in *dev_out (DEVICE pointer), nothing is copied back and the stream is not synchronised
+cudaError_t tm_blas_redot_dev(const tm_field *x, const tm_field *y, double *out, double *dev_out)
 {
     tm_ctx *c = x->ctx;
     const int Vh = c->g.Vh, blocks = (Vh + BT - 1) / BT;
@@ -197,10 +218,17 @@ cudaError_t tm_blas_redot(const tm_field *x, const tm_field *y, double *out)
     if (e != cudaSuccess) return e;
     c->launches++;
     c->last_kernel = "blas_redot";
-    return finish_sum(c, blocks, out);
+    return dev_out ? finish_sum_dev(c, blocks, dev_out) : finish_sum(c, blocks, out);
 }
 
 cudaError_t tm_blas_cg_update(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr)
+{
+    return tm_blas_cg_update_dev(x, r, p, Ap, a, rr, nullptr, nullptr, nullptr);
+}
+
+// anum != NULL: a = *anum / *aden on the device and |r|^2 is left in *dev_rr (DEVICE pointers), no synchronisation
+cudaError_t tm_blas_cg_update_dev(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr,
+                                  const double *anum, const double *aden, double *dev_rr)
 {
     tm_ctx *c = x->ctx;
     const int Vh = c->g.Vh, blocks = (Vh + BT - 1) / BT;
@@ -208,7 +236,7 @@ cudaError_t tm_blas_cg_update(tm_field *x, tm_field *r, const tm_field *p, const
     if (e != cudaSuccess) return e;
     char *xp = static_cast<char *>(x->ptr), *rp = static_cast<char *>(r->ptr);
     const char *pp = static_cast<const char *>(p->ptr), *ap = static_cast<const char *>(Ap->ptr);
-#define TM_UP(P, N) cg_update_kernel<P, N><<<blocks, BT, 0, c->stream>>>(xp, rp, pp, ap, a, Vh, c->red + 1)
+#define TM_UP(P, N) cg_update_kernel<P, N><<<blocks, BT, 0, c->stream>>>(xp, rp, pp, ap, a, Vh, c->red + 1, anum, aden)
     if (x->prec == 8) { if (x->nf == 1) TM_UP(8, 1); else TM_UP(8, 2); }
     else if (x->prec == 4) { if (x->nf == 1) TM_UP(4, 1); else TM_UP(4, 2); }
     else { if (x->nf == 1) TM_UP(2, 1); else TM_UP(2, 2); }
@@ -217,5 +245,5 @@ cudaError_t tm_blas_cg_update(tm_field *x, tm_field *r, const tm_field *p, const
     if (e != cudaSuccess) return e;
     c->launches++;
     c->last_kernel = "blas_cg_update";
-    return finish_sum(c, blocks, rr);
+    return dev_rr ? finish_sum_dev(c, blocks, dev_rr) : finish_sum(c, blocks, rr);
 }

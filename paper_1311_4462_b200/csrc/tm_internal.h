@@ -40,6 +40,8 @@ struct tm_ctx {
     int basis_on;         // tm_set_host_basis: host spinors are in another spin basis, psi_device = S psi_host
     double basis[32];     // S, row-major [4][4][re, im]
     void *staging;        // device staging for upload / download
+    double *cgs;          // inner CG scalars on the device: [0], [1] |r|^2 (ping-pong), [2] <p, A p>
+    double *cgs_host;     // pinned host ring the scalars are copied to: 2 x 3 doubles
     double *red;          // reduction scratch of tm_blas.cu: [0] result, [1..] per-block partial sums
     size_t red_n;
     size_t staging_bytes;
@@ -123,6 +125,12 @@ cudaError_t tm_launch_twist(const tm_field *out, const tm_field *in, double alph
 cudaError_t tm_blas_axpbyz(tm_field *z, double a, const tm_field *x, double b, const tm_field *y, double *norm2);
 cudaError_t tm_blas_redot(const tm_field *x, const tm_field *y, double *out);
 cudaError_t tm_blas_cg_update(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr);
+// the same with the scalars read from / left in DEVICE memory (no stream synchronisation): the inner CG loop
+cudaError_t tm_blas_axpbyz_dev(tm_field *z, double a, const tm_field *x, double b, const tm_field *y, double *norm2,
+                               const double *bnum, const double *bden);
+cudaError_t tm_blas_redot_dev(const tm_field *x, const tm_field *y, double *out, double *dev_out);
+cudaError_t tm_blas_cg_update_dev(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr,
+                                  const double *anum, const double *aden, double *dev_rr);
 
 // pack / unpack (tm_pack.cu)
 // (both apply the context's host spin basis: S on the way in, S^dag on the way out)
