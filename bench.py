@@ -381,6 +381,9 @@ def run_ours(args, log):
         alu_peak = SMS * LANES[k.pop("prec_bytes")] * 2 * sm_mhz * 1e-3      # GFLOPS
         k["alu_peak_gflops"] = alu_peak
         k["frac_of_alu_peak"] = k["gflops"] / alu_peak
+        # the half kernels are limited by the FP32 pipe (ncu fma pipe 63-66 % busy, math-pipe throttle the top
+        # stall, same run time with 32 % more link bytes); everything else by HBM
+        k["bound"] = "alu" if k["prec"] == "half" else "hbm"
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": "GFLOPS", "n_gpus": world, "steps": args.steps,
                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
