@@ -107,6 +107,15 @@ int tm_field_download(const tm_field *f, tm_parity parity, double *host_full);
  * (The cb order does not depend on the parity; the argument is kept for symmetry and validated.) */
 int tm_field_upload_cb(tm_field *f, tm_parity parity, const double *host_cb);
 int tm_field_download_cb(const tm_field *f, tm_parity parity, double *host_cb);
+/* Asynchronous forms (host_cb: HOST pointer to PINNED memory, same layout as above).  They return at once: the copies run on
+ * two private streams (one per direction, each with its own device staging buffer) and are ordered against the kernels of
+ * the context stream by events -- an upload's pack kernel waits for the kernels already queued (they may still read the
+ * field), kernels queued afterwards wait for it; a download unpacks after the kernels already queued, kernels queued
+ * afterwards wait for the unpack (not for the copy).  So the H2D copy of the next input, the kernels and the D2H copy of the
+ * previous result overlap.  The host buffers must stay valid, and a downloaded buffer is complete, only after tm_sync().
+ * Consecutive transfers in the same direction run in issue order.                                                        */
+int tm_field_upload_cb_async(tm_field *f, tm_parity parity, const double *host_cb);
+int tm_field_download_cb_async(const tm_field *f, tm_parity parity, double *host_cb);
 
 /* ---- host spin basis (SURVEY.md section 8f "minor": chiral <-> non-relativistic rotation in the pack kernels) ---- */
 /* The kernels work in the non-relativistic basis of PAPER.md:52 (gamma_4 diagonal; reading C5), which is also

@@ -157,6 +157,11 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->red_n = 0;
     c->cgs = nullptr;
     c->cgs_host = nullptr;
+    c->up_stream = c->down_stream = nullptr;
+    c->ev_compute = c->ev_up = c->ev_down = nullptr;
+    c->up_staging = c->down_staging = nullptr;
+    c->up_bytes = c->down_bytes = 0;
+    c->async_ready = false;
     c->timing = false;
     e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
     if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaDeviceGetAttribute"); }
@@ -176,6 +181,10 @@ int tm_sync(tm_ctx *ctx)
     if (!ctx) return fail(TM_ERR_ARG, "tm_sync: NULL context");
     cudaError_t e = cudaStreamSynchronize(ctx->stream);
     if (e != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize");
+    if (ctx->async_ready) {        // pending asynchronous uploads / downloads
+        if ((e = cudaStreamSynchronize(ctx->up_stream)) != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize(upload)");
+        if ((e = cudaStreamSynchronize(ctx->down_stream)) != cudaSuccess) return cuda_fail(e, "cudaStreamSynchronize(download)");
+    }
     return TM_OK;
 }
 
@@ -184,6 +193,17 @@ void tm_finalize(tm_ctx *ctx)
     if (!ctx) return;
     if (ctx->staging) cudaFree(ctx->staging);
     if (ctx->red) cudaFree(ctx->red);
+    if (ctx->async_ready) {
+        cudaStreamSynchronize(ctx->up_stream);
+        cudaStreamSynchronize(ctx->down_stream);
+        cudaStreamDestroy(ctx->up_stream);
+        cudaStreamDestroy(ctx->down_stream);
+        cudaEventDestroy(ctx->ev_compute);
+        cudaEventDestroy(ctx->ev_up);
+        cudaEventDestroy(ctx->ev_down);
+    }
+    if (ctx->up_staging) cudaFree(ctx->up_staging);
+    if (ctx->down_staging) cudaFree(ctx->down_staging);
     if (ctx->cgs) cudaFree(ctx->cgs);
     if (ctx->cgs_host) cudaFreeHost(ctx->cgs_host);
     for (auto &t : ctx->timed) { cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
@@ -368,6 +388,75 @@ static int field_download(const tm_field *f, int parity, double *host, bool cb)
     if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync D2H");
     e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(e, "download sync");
+    return TM_OK;
+}
+
+// ---- asynchronous forms: the copies run on their own streams and overlap the kernels of the context stream and each other ----
+static int async_setup(tm_ctx *c)
+{
+    if (c->async_ready) return TM_OK;
+    cudaError_t e;
+    if ((e = cudaStreamCreateWithFlags(&c->up_stream, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
+    if ((e = cudaStreamCreateWithFlags(&c->down_stream, cudaStreamNonBlocking)) != cudaSuccess) return cuda_fail(e, "cudaStreamCreate");
+    for (cudaEvent_t *ev : {&c->ev_compute, &c->ev_up, &c->ev_down})
+        if ((e = cudaEventCreateWithFlags(ev, cudaEventDisableTiming)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
+    c->async_ready = true;
+    return TM_OK;
+}
+
+static cudaError_t grow(void **p, size_t *have, size_t need, cudaStream_t owner)
+{
+    if (*have >= need) return cudaSuccess;
+    cudaError_t e = cudaStreamSynchronize(owner);        // the old buffer may still be in use by queued copies
+    if (e != cudaSuccess) return e;
+    if (*p) cudaFree(*p);
+    *p = nullptr;
+    *have = 0;
+    e = cudaMalloc(p, need);
+    if (e == cudaSuccess) *have = need;
+    return e;
+}
+
+int tm_field_upload_cb_async(tm_field *f, tm_parity parity, const double *host_cb)
+{
+    if (!f || !host_cb) return fail(TM_ERR_ARG, "tm_field_upload_cb_async: NULL argument");
+    if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
+    tm_ctx *c = f->ctx;
+    int rc = async_setup(c);
+    if (rc) return rc;
+    const size_t n = (size_t)f->nf * (size_t)c->g.Vh * 24 * sizeof(double);
+    cudaError_t e = grow(&c->up_staging, &c->up_bytes, n, c->up_stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
+    // H2D copy: free to run now (the staging buffer is ordered by the upload stream itself)
+    if ((e = cudaMemcpyAsync(c->up_staging, host_cb, n, cudaMemcpyHostToDevice, c->up_stream)) != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync H2D");
+    // the pack kernel overwrites f: it waits for every kernel already queued on the context stream (they may read f)
+    if ((e = cudaEventRecord(c->ev_compute, c->stream)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+    if ((e = cudaStreamWaitEvent(c->up_stream, c->ev_compute, 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
+    if ((e = tm_pack_spinor(f, (int)parity, static_cast<const double *>(c->up_staging), true, c->up_stream)) != cudaSuccess) return cuda_fail(e, "pack_spinor launch");
+    // later kernels of the context stream see the uploaded field
+    if ((e = cudaEventRecord(c->ev_up, c->up_stream)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+    if ((e = cudaStreamWaitEvent(c->stream, c->ev_up, 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
+    return TM_OK;
+}
+
+int tm_field_download_cb_async(const tm_field *f, tm_parity parity, double *host_cb)
+{
+    if (!f || !host_cb) return fail(TM_ERR_ARG, "tm_field_download_cb_async: NULL argument");
+    if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
+    tm_ctx *c = f->ctx;
+    int rc = async_setup(c);
+    if (rc) return rc;
+    const size_t n = (size_t)f->nf * (size_t)c->g.Vh * 24 * sizeof(double);
+    cudaError_t e = grow(&c->down_staging, &c->down_bytes, n, c->down_stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
+    // the unpack kernel reads f after everything queued on the context stream so far
+    if ((e = cudaEventRecord(c->ev_compute, c->stream)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+    if ((e = cudaStreamWaitEvent(c->down_stream, c->ev_compute, 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
+    if ((e = tm_unpack_spinor(f, (int)parity, static_cast<double *>(c->down_staging), true, c->down_stream)) != cudaSuccess) return cuda_fail(e, "unpack_spinor launch");
+    // later kernels of the context stream may overwrite f once it has been unpacked; the D2H copy itself overlaps them
+    if ((e = cudaEventRecord(c->ev_down, c->down_stream)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+    if ((e = cudaStreamWaitEvent(c->stream, c->ev_down, 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
+    if ((e = cudaMemcpyAsync(host_cb, c->down_staging, n, cudaMemcpyDeviceToHost, c->down_stream)) != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync D2H");
     return TM_OK;
 }
 

@@ -40,6 +40,13 @@ struct tm_ctx {
     int basis_on;         // tm_set_host_basis: host spinors are in another spin basis, psi_device = S psi_host
     double basis[32];     // S, row-major [4][4][re, im]
     void *staging;        // device staging for upload / download
+    // asynchronous upload / download (tm_field_upload_cb_async / tm_field_download_cb_async): one copy stream per direction with
+    // its own staging, ordered against the compute stream by events
+    cudaStream_t up_stream, down_stream;
+    cudaEvent_t ev_compute, ev_up, ev_down;
+    void *up_staging, *down_staging;
+    size_t up_bytes, down_bytes;
+    bool async_ready;
     double *cgs;          // inner CG scalars on the device: [0], [1] |r|^2 (ping-pong), [2] <p, A p>
     double *cgs_host;     // pinned host ring the scalars are copied to: 2 x 3 doubles
     double *red;          // reduction scratch of tm_blas.cu: [0] result, [1..] per-block partial sums
