@@ -182,8 +182,12 @@ TM_DEV void epilogue(real *acc, const real *xv, real alpha, real beta, real scal
 }
 
 
+// resident blocks of 128 threads per SM the register allocation of the fp64 degenerate kernel aims at (measured: profiles/r1_tuning.md)
+#ifndef TM_MINB_8_1
+#define TM_MINB_8_1 3
+#endif
 template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
-__global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? 3 : (PREC == 8 ? 2 : 1)) tm_dslash_generic(const DslashArgs a)
+__global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? TM_MINB_8_1 : (PREC == 8 ? 2 : 1)) tm_dslash_generic(const DslashArgs a)
 {
     typedef typename PrecTraits<PREC>::real real;
     const int Vh = a.Vh;
