@@ -191,6 +191,28 @@ typedef struct {
     double residual;               /* last true relative residual |b - A x| / |b|                                      */
     int converged;                 /* 1 if residual <= tol                                                            */
 } tm_cg_info;
+/* ---- time-direction domain decomposition --------------------------------
+ * One slab X x Y x Z x T_loc of the global lattice per context (per GPU), slabs stacked along x4 in rank order; T_loc even,
+ * so local and global site parities agree.  One distributed dslash =
+ *   tm_halo_pack(in)  ->  exchange the two face buffers with the neighbouring slabs (the caller's transport: NCCL
+ *   send / recv, peer copies; paper_1311_4462_b200.sharded does it with torch.distributed)  ->  tm_dslash_apply with
+ *   tm_set_open_time(ctx, 1) (the kernels give the time hops that leave the slab the weight 0)  ->  tm_halo_apply(out),
+ * after which `out` equals the single-lattice result on this slab (tests/test_gpu_sharded.py against the oracle on the
+ * global lattice).  The exchange can overlap the interior kernel; tm_halo_apply must follow both on the context stream.
+ * Face buffers are DEVICE memory owned by the caller, tm_halo_bytes() each: [n_flavor][XYZ/2][12 reals] of double (fp64
+ * fields) or float (fp32 and half fields); site j of a face = checkerboard index inside the time slice.
+ *   dev_to_prev  : spin-projected half-spinors of the FIRST time slice, for the previous slab's forward hops
+ *   dev_to_next  : U_4^dag times the projected half-spinors of the LAST time slice, for the next slab's backward hops
+ *   dev_from_prev = the previous slab's dev_to_next, dev_from_next = the next slab's dev_to_prev
+ *   sign_prev / sign_next : +1, or the time boundary condition (-1 antiperiodic) where that face is the global boundary
+ * `out_parity`, `dagger`, `kt` are those of the tm_dslash_apply call being completed; every kernel type is supported
+ * (the fused epilogues are affine in the hopping sum).                                                                */
+int tm_set_open_time(tm_ctx *ctx, int on);
+size_t tm_halo_bytes(const tm_ctx *ctx, tm_precision prec, int n_flavor);
+int tm_halo_pack(const tm_field *in, const tm_gauge *g, tm_parity out_parity, int dagger, void *dev_to_prev, void *dev_to_next);
+int tm_halo_apply(tm_field *out, const void *dev_from_prev, const void *dev_from_next, const tm_gauge *g, const tm_params *p,
+                  tm_parity out_parity, int dagger, tm_kernel_type kt, int sign_prev, int sign_next);
+
 /* Mixed-precision conjugate gradient on the normal equations of the even-odd preconditioned operator (the paper's
  * "double-single" / "double-half" CG, as defect correction): solves
  *     M^dag M x_e = b_e ,   M = the LHS of Eq. 2.2 (ASYM) or Eq. 2.3 (SYM),

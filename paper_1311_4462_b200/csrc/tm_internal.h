@@ -47,6 +47,7 @@ struct tm_ctx {
     void *up_staging, *down_staging;
     size_t up_bytes, down_bytes;
     bool async_ready;
+    int open_time;        // tm_set_open_time: the fused kernels drop the time hops that leave the slab (tm_halo.cu adds them)
     double *cgs;          // inner CG scalars on the device: [0], [1] |r|^2 (ping-pong), [2] <p, A p>
     double *cgs_host;     // pinned host ring the scalars are copied to: 2 x 3 doubles
     double *red;          // reduction scratch of tm_blas.cu: [0] result, [1..] per-block partial sums
@@ -138,6 +139,11 @@ cudaError_t tm_blas_axpbyz_dev(tm_field *z, double a, const tm_field *x, double 
 cudaError_t tm_blas_redot_dev(const tm_field *x, const tm_field *y, double *out, double *dev_out);
 cudaError_t tm_blas_cg_update_dev(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr,
                                   const double *anum, const double *aden, double *dev_rr);
+
+// surface kernels of the time-direction decomposition (tm_halo.cu)
+cudaError_t tm_launch_halo_pack(const tm_field *in, const tm_gauge *g, int out_parity, int dagger, void *to_prev, void *to_next, cudaStream_t s);
+cudaError_t tm_launch_halo_apply(tm_field *out, const void *from_prev, const void *from_next, const tm_gauge *g, int parity, int dagger,
+                                 double w_prev, double w_next, double alpha, double beta, double scale, double coef, int twist_on, cudaStream_t s);
 
 // pack / unpack (tm_pack.cu)
 // (both apply the context's host spin basis: S on the way in, S^dag on the way out)

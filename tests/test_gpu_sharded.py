@@ -1,0 +1,103 @@
+"""GPU parity of the time-direction decomposition (include/tm.h: tm_halo_pack / tm_halo_apply, tm_set_open_time) against the
+oracle on the GLOBAL lattice.  One GPU: the slabs of a `world`-way split are processed one after the other in this process
+(pack all, hand the face buffers over exactly as sharded.ring_exchange routes them, then interior kernel + completion per
+slab), so no kernel ever waits for another rank; the transport itself is covered by tests/test_sharded_host.py (gloo)."""
+import itertools
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1311_4462_b200 as tm
+import synth_inputs as si
+from gpu_util import TOL, PREC_NAME, rel_l2
+from paper_1311_4462_b200 import sharded
+
+pytestmark = pytest.mark.gpu
+
+KAPPA = 0.1632
+PRECS = [tm.TM_DOUBLE, tm.TM_SINGLE, tm.TM_HALF]
+
+
+class Split:
+    """`world` slabs of one global lattice on one GPU, each with its slice of the gauge field."""
+
+    def __init__(self, dims, world, U):
+        self.dims, self.world, self.U = dims, world, U
+        self.slabs = [sharded.Slab(dims, r, world) for r in range(world)]
+        self.sl = [sharded.slab_slice(dims, r, world) for r in range(world)]
+        self._g = {}
+
+    def gauge(self, r, prec, recon):
+        key = (r, prec, recon)
+        if key not in self._g:
+            self._g[key] = self.slabs[r].lat.gauge(np.ascontiguousarray(self.U[:, self.sl[r]]), prec, recon)
+        return self._g[key]
+
+    def kernel(self, inp, x, p, parity, dagger, kt, prec, recon, nf):
+        W = self.world
+        fin, fx, fout, faces = [], [], [], []
+        for r, s in enumerate(self.slabs):
+            fin.append(s.lat.field(prec, nf).upload(1 - parity, np.ascontiguousarray(inp[:, self.sl[r]])))
+            fx.append(None if x is None else s.lat.field(prec, nf).upload(parity, np.ascontiguousarray(x[:, self.sl[r]])))
+            fout.append(s.lat.field(prec, nf))
+            to_prev, to_next = s.pack(fin[r], self.gauge(r, prec, recon), parity, dagger)
+            faces.append((to_prev.clone(), to_next.clone()))
+        out = np.zeros_like(inp)
+        for r, s in enumerate(self.slabs):
+            from_prev, from_next = faces[(r - 1) % W][1], faces[(r + 1) % W][0]       # = sharded.ring_exchange
+            g = self.gauge(r, prec, recon)
+            tm.dslash_apply(fout[r], fin[r], fx[r], g, p, parity, dagger, kt)
+            s.finish(fout[r], from_prev, from_next, g, p, parity, dagger, kt)
+            s.lat.sync()
+            out[:, self.sl[r]] = fout[r].download(parity)
+        return out
+
+
+_cache = {}
+
+
+def split_for(dims, world, kind, seed):
+    key = (dims, world, kind, seed)
+    if key not in _cache:
+        _cache[key] = Split(dims, world, si.gauge_field(dims, seed, kind))
+    return _cache[key]
+
+
+@pytest.mark.parametrize("dims,world", [((4, 4, 4, 16), 2), ((4, 6, 4, 12), 3), ((6, 6, 6, 8), 1)])
+@pytest.mark.parametrize("kw", [dict(mu=0.3, epsilon=0.0, twist_flavor=-1), dict(mu=0.15, epsilon=0.19, twist_flavor=0),
+                                dict(mu=0.15, epsilon=0.19, twist_flavor=0, t_boundary=+1)], ids=["deg-", "ndeg", "ndeg-periodic"])
+def test_h1_sharded_kernels_match_the_global_oracle(dims, world, kw):
+    nf = 2 if kw["twist_flavor"] == 0 else 1
+    sp = split_for(dims, world, "haar", 21)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    full_in, full_x = si.spinor_field(dims, nf, 22), si.spinor_field(dims, nf, 23)
+    for parity, dagger, kt in itertools.product((0, 1), (0, 1), (0, 1, 2, 3, 4, 5)):
+        inp = si.mask_parity(full_in, dims, 1 - parity)
+        x = si.mask_parity(full_x, dims, parity)
+        if kt < 4:
+            want = oracle.kernel(inp, x, sp.U, po, parity, dagger, kt)
+        else:
+            want = oracle.hop_xpay(inp, x, sp.U, po, parity, dagger, -KAPPA ** 2 if kt == 4 else KAPPA)
+        for prec in PRECS:
+            recon = tm.TM_RECON_12 if prec != tm.TM_DOUBLE else tm.TM_RECON_18
+            got = sp.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, prec, recon, nf)
+            assert rel_l2(got, want) <= TOL[prec], (PREC_NAME[prec], world, parity, dagger, kt)
+
+
+def test_h2_sharded_mat_pc_world_1_and_8real():
+    """Slab.mat_pc through ring_exchange itself (world = 1: the slab is its own neighbour) and 8-real links."""
+    dims = (4, 4, 4, 8)
+    U = si.gauge_field(dims, 24, "haar")
+    kw = dict(mu=0.15, epsilon=0.19, twist_flavor=0)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    psi_e = si.mask_parity(si.spinor_field(dims, 2, 25), dims, 0)
+    s = sharded.Slab(dims, 0, 1)
+    for prec, recon in ((tm.TM_DOUBLE, tm.TM_RECON_8), (tm.TM_SINGLE, tm.TM_RECON_8), (tm.TM_HALF, tm.TM_RECON_12)):
+        g = s.lat.gauge(U, prec, recon)
+        fin, ftmp, fout = s.lat.field(prec, 2).upload(0, psi_e), s.lat.field(prec, 2), s.lat.field(prec, 2)
+        for typ, dagger in ((tm.TM_MATPC_ASYM, 0), (tm.TM_MATPC_ASYM, 1), (tm.TM_MATPC_SYM, 0)):
+            s.mat_pc(fout, fin, ftmp, g, pg, typ, dagger)
+            s.lat.sync()
+            want = oracle.matpc_adjoint(psi_e, U, po, typ) if dagger else oracle.matpc(psi_e, U, po, typ, 0)
+            assert rel_l2(fout.download(0), want) <= TOL[prec], (PREC_NAME[prec], typ, dagger)
