@@ -25,11 +25,12 @@ def slab_slice(global_dims, rank, world):
     return slice(rank * n, (rank + 1) * n)
 
 
-def ring_exchange(to_prev, to_next, rank, world, group=None):
-    """Send `to_prev` to rank-1 and `to_next` to rank+1 (periodic ring); return (from_prev, from_next) = (rank-1's to_next,
-    rank+1's to_prev).  All four are tensors of one shape and dtype.  world = 1: the slab is its own neighbour."""
-    if world == 1:
-        return to_next.clone(), to_prev.clone()
+def ring_exchange_start(to_prev, to_next, rank, world, group=None):
+    """Post the sends of `to_prev` to rank-1 and `to_next` to rank+1 and the matching receives (periodic ring); returns a
+    handle for ring_exchange_finish.  With NCCL the transfers are ordered after the work already queued on the current
+    stream (the pack kernel) and run beside whatever is queued next (the interior kernel)."""
+    if world == 1:          # the slab is its own neighbour
+        return (to_next.clone(), to_prev.clone(), [])
     import torch.distributed as dist
     prev, nxt = (rank - 1) % world, (rank + 1) % world
     from_prev, from_next = torch.empty_like(to_next), torch.empty_like(to_prev)
@@ -37,9 +38,20 @@ def ring_exchange(to_prev, to_next, rank, world, group=None):
            dist.P2POp(dist.irecv, from_next, nxt, group, tag=1), dist.P2POp(dist.irecv, from_prev, prev, group, tag=2)]
     if world == 2:          # both neighbours are the same rank: order the pairs so that sends and receives match by tag
         ops = [ops[0], ops[2], ops[1], ops[3]] if rank == 0 else [ops[2], ops[0], ops[3], ops[1]]
-    for req in dist.batch_isend_irecv(ops):
+    return (from_prev, from_next, dist.batch_isend_irecv(ops))
+
+
+def ring_exchange_finish(handle):
+    """(from_prev, from_next) = (rank-1's to_next, rank+1's to_prev); later work on the current stream sees them."""
+    from_prev, from_next, reqs = handle
+    for req in reqs:
         req.wait()
     return from_prev, from_next
+
+
+def ring_exchange(to_prev, to_next, rank, world, group=None):
+    """Blocking form: all four tensors have one shape and dtype."""
+    return ring_exchange_finish(ring_exchange_start(to_prev, to_next, rank, world, group))
 
 
 class Slab:
@@ -77,9 +89,9 @@ class Slab:
     def dslash_apply(self, out, inp, x, gauge, p, parity, dagger, kernel_type):
         """The distributed form of tm.dslash_apply: faces out, interior kernel while they travel, boundary sites completed."""
         to_prev, to_next = self.pack(inp, gauge, parity, dagger)
-        torch.cuda.current_stream(self.device).synchronize() if self.world > 1 else None
-        from_prev, from_next = ring_exchange(to_prev, to_next, self.rank, self.world, self.group)
-        tm.dslash_apply(out, inp, x, gauge, p, parity, dagger, kernel_type)
+        handle = ring_exchange_start(to_prev, to_next, self.rank, self.world, self.group)
+        tm.dslash_apply(out, inp, x, gauge, p, parity, dagger, kernel_type)            # overlaps the transfer
+        from_prev, from_next = ring_exchange_finish(handle)
         self.finish(out, from_prev, from_next, gauge, p, parity, dagger, kernel_type)
 
     def mat_pc(self, out_e, in_e, tmp_o, gauge, p, matpc_type, dagger=0):

@@ -101,3 +101,21 @@ def test_h2_sharded_mat_pc_world_1_and_8real():
             s.lat.sync()
             want = oracle.matpc_adjoint(psi_e, U, po, typ) if dagger else oracle.matpc(psi_e, U, po, typ, 0)
             assert rel_l2(fout.download(0), want) <= TOL[prec], (PREC_NAME[prec], typ, dagger)
+
+
+def test_h3_torchrun_script_world_1():
+    """tests/run_sharded_torchrun.py (the multi-GPU check, NCCL) launched the way the driver launches bench.py, with one rank."""
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "1", "--master-addr", "127.0.0.1",
+                        "--master-port", str(port), os.path.join(root, "tests", "run_sharded_torchrun.py")],
+                       capture_output=True, text=True, timeout=600, cwd=root)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    assert "sharded ok: world 1" in r.stdout
