@@ -60,3 +60,13 @@ def test_product_path_does_not_import_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in src.replace("no CPU fallback", ""), f
                 assert "_work/" not in src, f
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/tm.h is a C boundary: it compiles as C99 with no C++ or CUDA types in the signatures."""
+    import subprocess
+    src = tmp_path / "hdr.c"
+    src.write_text('#include "tm.h"\nint main(void) { return TM_OK + TM_RECON_8 + TM_BASIS_CHIRAL; }\n')
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(ROOT, "include"),
+                        "-c", str(src), "-o", str(tmp_path / "hdr.o")], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
