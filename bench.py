@@ -166,12 +166,15 @@ def ncu_traffic(name):
 class Workload:
     """Device-resident inputs of one step (seeded synthetic stand-ins for the paper's ensembles)."""
 
-    def __init__(self, device, log):
+    def __init__(self, device, log, slab=None):
         import torch
         import paper_1311_4462_b200 as tm
         import synth_inputs as si
         self.tm, self.si, self.torch = tm, si, torch
-        self.lat = tm.Lattice(DIMS, device)
+        # --sharded: this rank's 32^3x64 slab of a 32^3 x (64 N) lattice (the same seeded fields on every slab: N copies stacked
+        # along x4 are a valid gauge field), kernels with open time hops + face exchange (paper_1311_4462_b200/sharded.py)
+        self.slab = slab
+        self.lat = slab.lat if slab is not None else tm.Lattice(DIMS, device)
         self.vh = self.lat.Vh
         t = time.time()
         self.host_gauge = {1: si.gauge_field(DIMS, SEED_DEG, "haar"), 2: si.gauge_field(DIMS, SEED_NDEG, "near_identity")}
@@ -189,11 +192,15 @@ class Workload:
             self.ftmp[key], self.fout[key] = self.lat.field(prec, nf), self.lat.field(prec, nf)
         self.lat.sync()
 
+    def mat_pc(self, key, nf, typ, dagger):
+        if self.slab is not None:
+            self.slab.mat_pc(self.fout[key], self.fin[key], self.ftmp[key], self.gauge[key], self.params[nf], typ, dagger)
+        else:
+            self.tm.mat_pc(self.fout[key], self.fin[key], self.ftmp[key], self.gauge[key], self.params[nf], typ, dagger)
+
     def step(self):
-        tm = self.tm
         for nf, prec, typ, dagger in step_ops():
-            key = (nf, prec)
-            tm.mat_pc(self.fout[key], self.fin[key], self.ftmp[key], self.gauge[key], self.params[nf], typ, dagger)
+            self.mat_pc((nf, prec), nf, typ, dagger)
 
     def make_pinned(self):
         torch = self.torch
@@ -214,7 +221,7 @@ class Workload:
         for nf, prec, typ, dagger in step_ops():
             key = (nf, prec)
             tm.tm_field_upload_cb_async(self.fin[key].h, 0, self.pin_in[nf].data_ptr())
-            tm.mat_pc(self.fout[key], self.fin[key], self.ftmp[key], self.gauge[key], self.params[nf], typ, dagger)
+            self.mat_pc(key, nf, typ, dagger)
             tm.tm_field_download_cb_async(self.fout[key].h, 0, self.pin_out[nf].data_ptr())
             h2d += self.pin_in[nf].numel() * 8
             d2h += self.pin_out[nf].numel() * 8
@@ -281,7 +288,11 @@ def run_ours(args, log):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     import paper_1311_4462_b200 as tm
-    w = Workload(local, log)
+    slab = None
+    if args.sharded:
+        from paper_1311_4462_b200 import sharded
+        slab = sharded.Slab((DIMS[0], DIMS[1], DIMS[2], DIMS[3] * world), rank, world, local)
+    w = Workload(local, log, slab)
     lat, vh = w.lat, w.vh
     tm.tm_set_path(lat.ctx, args.path)
     ops = step_ops()
@@ -393,7 +404,8 @@ def run_ours(args, log):
                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                "vs_baseline": None, "dtype": "f64+f32+i16/f32", "data": "synthetic",
                "config": {"workload": WORKLOAD % (RECON, RECON), "lattice": list(DIMS), "recon": RECON, "kappa": KAPPA,
-                          "parallelism": "replicas only (path does not shard)" if world > 1 else "single GPU",
+                          "parallelism": ("time-direction slabs of a 32^3 x %d lattice, one per GPU, face exchange per dslash (--sharded)" % (DIMS[3] * world))
+                          if args.sharded else ("replicas only (north_star: no sharding)" if world > 1 else "single GPU"),
                           "l2": "inputs larger than L2 (gauge fields 201-805 MB each, 2.3 GB touched per step)"},
                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                "step_flops": step_flops, "step_alg_bytes": step_bytes, "kernels": kernels,
@@ -414,6 +426,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--path", type=int, default=0, help="tm_set_path: 0 = default kernel selection, 1 = scalar kernels only")
+    ap.add_argument("--sharded", action="store_true",
+                    help="each rank holds a 32^3x64 slab of a 32^3 x (64 N) lattice: kernels with open time hops, face exchange over "
+                         "torch.distributed, boundary completion (DESIGN.md section 9); default: N independent replicas")
     ap.add_argument("--recon", type=int, default=12, choices=[18, 12, 8],
                     help="reals stored per link (BASELINE.json configs[2], configs[3]: 12); 18 and 8 are the other rows of the paper's Table 1")
     args = ap.parse_args()
