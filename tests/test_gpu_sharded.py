@@ -119,3 +119,42 @@ def test_h3_torchrun_script_world_1():
                        capture_output=True, text=True, timeout=600, cwd=root)
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
     assert "sharded ok: world 1" in r.stdout
+
+
+def test_h4_halo_api_sizes_and_error_paths():
+    import torch
+    dims = (4, 6, 4, 8)
+    s = sharded.Slab(dims, 0, 1)
+    lat, ctx = s.lat, s.lat.ctx
+    vs2 = 4 * 6 * 4 // 2
+    assert tm.tm_halo_bytes(ctx, tm.TM_DOUBLE, 1) == vs2 * 12 * 8
+    assert tm.tm_halo_bytes(ctx, tm.TM_SINGLE, 2) == 2 * vs2 * 12 * 4
+    assert tm.tm_halo_bytes(ctx, tm.TM_HALF, 2) == 2 * vs2 * 12 * 4          # half fields travel as float
+    assert tm.tm_halo_bytes(ctx, 3, 1) == 0 and tm.tm_halo_bytes(ctx, tm.TM_DOUBLE, 3) == 0
+    U = si.gauge_field(dims, 26, "haar")
+    g64, g32 = lat.gauge(U, tm.TM_DOUBLE, tm.TM_RECON_12), lat.gauge(U, tm.TM_SINGLE, tm.TM_RECON_12)
+    f = lat.field(tm.TM_DOUBLE, 1)
+    a, b = s.faces(tm.TM_DOUBLE, 1)
+    p = tm.params(KAPPA, mu=0.1)
+    for bad in (lambda: tm.tm_halo_pack(f.h, g32.h, 0, 0, a.data_ptr(), b.data_ptr()),                      # precision mismatch
+                lambda: tm.tm_halo_pack(f.h, g64.h, 2, 0, a.data_ptr(), b.data_ptr()),                      # parity
+                lambda: tm.tm_halo_pack(f.h, g64.h, 0, 0, 0, b.data_ptr()),                                 # NULL buffer
+                lambda: tm.tm_halo_apply(f.h, a.data_ptr(), b.data_ptr(), g64.h, p, 0, 0, 7, 1, 1),         # kernel type
+                lambda: tm.tm_halo_apply(f.h, a.data_ptr(), b.data_ptr(), g64.h, p, 0, 0, 0, 0, 1)):        # boundary sign
+        with pytest.raises(tm.TmError):
+            bad()
+    # open time hops off again: the context is an ordinary periodic / antiperiodic lattice
+    psi = si.mask_parity(si.spinor_field(dims, 1, 27), dims, 0)
+    po = oracle.params(dims, KAPPA, mu=0.1)
+    fin, fout = lat.field(tm.TM_DOUBLE, 1).upload(0, psi), lat.field(tm.TM_DOUBLE, 1)
+    tm.dslash_apply(fout, fin, None, g64, p, 1, 0, 0)
+    lat.sync()
+    open_result = fout.download(1)
+    tm.tm_set_open_time(ctx, 0)
+    tm.dslash_apply(fout, fin, None, g64, p, 1, 0, 0)
+    lat.sync()
+    want = oracle.kernel(psi, np.zeros_like(psi), U, po, 1, 0, 0)
+    assert rel_l2(fout.download(1), want) <= 1e-12
+    # with open time hops only the two boundary time slices differ from the closed lattice
+    diff = np.abs(open_result - want).reshape(1, dims[3], -1).max(axis=2)[0]
+    assert (diff[1:-1] < 1e-12).all() and diff[0] > 1e-3 and diff[-1] > 1e-3
