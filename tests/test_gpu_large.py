@@ -7,8 +7,9 @@ and the antiperiodic time sign act, and the GPU result is compared there element
 tolerances (relative L2 over the sampled sites).  Properties that hold at any size are checked on the whole field:
 the other parity stays untouched and finite, and repeated application is bit-for-bit reproducible.
 
-configs[4] (48^3x96, "applied 100 times back to back") is `test_config5_...`: host inputs for it need ~20 GB of RAM
-and minutes of generation, so it runs only when TM_TEST_HUGE=1; the same kernels are covered at 32^3x64.
+configs[4] (48^3x96, "applied 100 times back to back") is `test_config5_...` (~25 GB of host memory, about a minute on the
+B200 box); `test_64c64_...` is the maximum-size case of the addressing (gauge parity blocks beyond 4 GiB, ~35 GB of host
+memory, half a minute).  Both run by default and are skipped only when the host is short of memory or TM_TEST_HUGE=0.
 """
 import os
 
@@ -183,3 +184,33 @@ def test_config5_48c96_nondegenerate_fp64_sym_100_applications():
         tm.mat_pc(fout, fin, ftmp, g, pg, tm.TM_MATPC_SYM, 0)
     c.lat.sync()
     assert bool((first == fout.storage).all())
+
+
+@pytest.mark.skipif(os.environ.get("TM_TEST_HUGE", "1") == "0" or _host_gb() < 60,
+                    reason="64^4 host inputs need ~35 GB of host memory (or TM_TEST_HUGE=0)")
+def test_64c64_fp64_gauge_blocks_beyond_4_gib():
+    """Maximum-size case for the addressing: at 64^4 one parity block of the fp64 18-real gauge field is 4.8 GB, so link
+    offsets pass 2^32 bytes (no BASELINE.json config does: 48^3x96 stops at 3.1 GB per block).  Kernels A (odd output) and
+    B (even output) against the oracle at sampled sites, which include the last sites of both parities.  The gauge field is
+    a 64^3 x 8 Haar block repeated along x4 (a valid SU(3) field; generating 67 M independent links would take minutes)."""
+    dims, small = (64, 64, 64, 64), (64, 64, 64, 8)
+    U = np.ascontiguousarray(np.tile(si.gauge_field(small, 6, "haar"), (1, 8, 1, 1)))
+    lat = tm.Lattice(dims)
+    g = lat.gauge(U, tm.TM_DOUBLE, tm.TM_RECON_18)
+    assert 4 * lat.Vh * 18 * 8 > 2 ** 32
+    kw = dict(mu=0.004, epsilon=0.0, twist_flavor=1)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    psi = si.spinor_field(dims, 1, 6)
+    for parity, kt in ((1, 0), (0, 2)):
+        inp = si.mask_parity(psi, dims, 1 - parity)
+        x = si.mask_parity(psi, dims, parity)
+        fin = lat.field(tm.TM_DOUBLE, 1).upload(1 - parity, inp)
+        fx = lat.field(tm.TM_DOUBLE, 1).upload(parity, x)
+        fout = lat.field(tm.TM_DOUBLE, 1)
+        tm.dslash_apply(fout, fin, None if kt == 0 else fx, g, pg, parity, 0, kt)
+        lat.sync()
+        sites = sample_sites(dims, parity, 60 + parity, n=1024)
+        want = oracle.kernel_sites(sites, inp, x, U, po, 0, kt)
+        err = rel_l2_sites(fout.download(parity), want, sites)
+        assert err <= TOL[tm.TM_DOUBLE], (parity, kt, err)
+        del fin, fx, fout
