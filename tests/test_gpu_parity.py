@@ -413,6 +413,45 @@ def test_t4_asym_composite_adjointness_on_gpu(kw):
         assert abs(lhs - rhs) <= tol * np.linalg.norm(phi) * np.linalg.norm(m_psi)
 
 
+# ---- T4b: degenerate inputs -----------------------------------------------------------------------------------------
+
+def test_t4b_zero_fields_zero_sites_and_unit_links():
+    """The degenerate cases of the method: an all-zero input (half: site norm 0, q 0 -- reading C9), an input that is zero on
+    most sites, and the free field (unit links, 18- and 12-real; 8-real refuses them, T2c).  No NaN / inf, exact zeros stay
+    zero, and the sparse / free-field results match the oracle."""
+    dims = (4, 4, 6, 8)
+    lat = tm.Lattice(dims)
+    unit = np.zeros((4, lat.V, 3, 3), dtype=np.complex128)
+    unit[:, :, [0, 1, 2], [0, 1, 2]] = 1.0
+    kw = dict(mu=0.15, epsilon=0.19, twist_flavor=0)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    sparse = si.mask_parity(si.spinor_field(dims, 2, 81), dims, 0)
+    keep = si.parity_sites(dims, 0)[::37]
+    mask = np.zeros(lat.V, dtype=bool)
+    mask[keep] = True
+    sparse[:, ~mask] = 0.0                                   # nonzero on 1 site in 37
+    x = si.mask_parity(si.spinor_field(dims, 2, 82), dims, 1)
+    for prec, recon in itertools.product(PRECS, RECONS):
+        g = lat.gauge(unit, prec, recon)
+        zero = lat.field(prec, 2).upload(0, np.zeros_like(sparse))
+        fx, fout = lat.field(prec, 2).upload(1, x), lat.field(prec, 2)
+        tm.dslash_apply(fout, zero, None, g, pg, 1, 0, 0)                       # A on a zero field
+        lat.sync()
+        assert np.abs(fout.download(1)).max() == 0.0
+        tm.dslash_apply(fout, zero, fx, g, pg, 1, 0, 1)                         # A-xpay: out = x exactly (up to the format)
+        lat.sync()
+        got = fout.download(1)
+        assert np.isfinite(got.view(np.float64)).all()
+        assert rel_l2(got, fx.download(1)) <= (0.0 if prec != tm.TM_HALF else 1e-4)
+        fin = lat.field(prec, 2).upload(0, sparse)
+        for kt in (0, 2):
+            tm.dslash_apply(fout, fin, fx, g, pg, 1, 0, kt)
+            lat.sync()
+            got = fout.download(1)
+            assert np.isfinite(got.view(np.float64)).all()
+            assert rel_l2(got, oracle.kernel(sparse, x, unit, po, 1, 0, kt)) <= TOL[prec], (PREC_NAME[prec], recon, kt)
+
+
 # ---- T5: host spin basis (SURVEY.md section 8f "minor": chiral <-> non-relativistic rotation in the pack kernels) ----
 
 def test_t5_host_spin_basis_chiral_and_custom():
