@@ -56,6 +56,18 @@ int cuda_fail(cudaError_t e, const char *what)
     return fail(TM_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
+// Every entry point that allocates, copies or launches selects the context's device first (the caller's current
+// device may be another one: two contexts on two GPUs in one thread).
+int use_device(const tm_ctx *c)
+{
+    int cur = -1;
+    if (cudaGetDevice(&cur) == cudaSuccess && cur == c->device) return TM_OK;
+    cudaError_t e = cudaSetDevice(c->device);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaSetDevice");
+    return TM_OK;
+}
+#define TM_USE_DEVICE(c) do { int rc_ = use_device(c); if (rc_) return rc_; } while (0)
+
 bool valid_prec(int p) { return p == TM_DOUBLE || p == TM_SINGLE || p == TM_HALF; }
 
 size_t field_bytes(const TmGeom &g, int prec, int nf)
@@ -326,6 +338,7 @@ int tm_field_alloc(tm_ctx *ctx, tm_precision prec, int n_flavor, void *ext_dev_p
     *f = nullptr;
     if (!valid_prec(prec)) return fail(TM_ERR_ARG, "bad precision %d", (int)prec);
     if (n_flavor < 1 || n_flavor > 2) return fail(TM_ERR_ARG, "n_flavor must be 1 or 2");
+    TM_USE_DEVICE(ctx);
     const size_t bytes = field_bytes(ctx->g, prec, n_flavor);
     tm_field *fl = new (std::nothrow) tm_field();
     if (!fl) return fail(TM_ERR_NOMEM, "out of host memory");
@@ -357,6 +370,7 @@ static int field_upload(tm_field *f, int parity, const double *host, bool cb)
     if (!f || !host) return fail(TM_ERR_ARG, "tm_field_upload: NULL argument");
     if (parity != 0 && parity != 1) return fail(TM_ERR_ARG, "bad parity %d", parity);
     tm_ctx *c = f->ctx;
+    TM_USE_DEVICE(c);
     const size_t n = (size_t)f->nf * (cb ? (size_t)c->g.Vh : (size_t)c->g.V) * 24 * sizeof(double);
     Staging st(c);
     cudaError_t e = st.alloc(n);
@@ -375,6 +389,7 @@ static int field_download(const tm_field *f, int parity, double *host, bool cb)
     if (!f || !host) return fail(TM_ERR_ARG, "tm_field_download: NULL argument");
     if (parity != 0 && parity != 1) return fail(TM_ERR_ARG, "bad parity %d", parity);
     tm_ctx *c = f->ctx;
+    TM_USE_DEVICE(c);
     const size_t n = (size_t)f->nf * (cb ? (size_t)c->g.Vh : (size_t)c->g.V) * 24 * sizeof(double);
     Staging st(c);
     cudaError_t e = st.alloc(n);
@@ -423,6 +438,7 @@ int tm_field_upload_cb_async(tm_field *f, tm_parity parity, const double *host_c
     if (!f || !host_cb) return fail(TM_ERR_ARG, "tm_field_upload_cb_async: NULL argument");
     if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
     tm_ctx *c = f->ctx;
+    TM_USE_DEVICE(c);
     int rc = async_setup(c);
     if (rc) return rc;
     const size_t n = (size_t)f->nf * (size_t)c->g.Vh * 24 * sizeof(double);
@@ -445,6 +461,7 @@ int tm_field_download_cb_async(const tm_field *f, tm_parity parity, double *host
     if (!f || !host_cb) return fail(TM_ERR_ARG, "tm_field_download_cb_async: NULL argument");
     if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
     tm_ctx *c = f->ctx;
+    TM_USE_DEVICE(c);
     int rc = async_setup(c);
     if (rc) return rc;
     const size_t n = (size_t)f->nf * (size_t)c->g.Vh * 24 * sizeof(double);
@@ -484,6 +501,7 @@ int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_r
         if (!(nmin >= 1e-10))
             return fail(TM_ERR_PARAM, "8-real links: a link has |U01|^2 + |U02|^2 = %.3g, at the chart's singular point (use 12- or 18-real)", nmin);
     }
+    TM_USE_DEVICE(ctx);
     tm_gauge *gg = new (std::nothrow) tm_gauge();
     if (!gg) return fail(TM_ERR_NOMEM, "out of host memory");
     gg->ctx = ctx; gg->prec = prec; gg->recon = recon;
@@ -524,6 +542,8 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
         return fail(TM_ERR_MISMATCH, "precision mismatch (call %d, out %d, in %d, gauge %d)", (int)prec, out->prec, in->prec, g->prec);
     if (in->nf != out->nf || (x && x->nf != out->nf)) return fail(TM_ERR_MISMATCH, "flavor count mismatch");
     if (overlap(out, in)) return fail(TM_ERR_ALIAS, "out aliases in");
+    if (x && overlap(out, x) && out->ptr != x->ptr) return fail(TM_ERR_ALIAS, "out partially overlaps x (only out == x is allowed)");
+    TM_USE_DEVICE(c);
     Coeffs co;
     int rc = make_coeffs(p, out->nf, dagger ? 1 : 0, (int)kt, &co);
     if (rc) return rc;
@@ -600,6 +620,7 @@ int tm_twist_apply(tm_field *out, const tm_field *in, const tm_params *p, int in
     if (in->ctx != c) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
     if (in->prec != out->prec || in->nf != out->nf) return fail(TM_ERR_MISMATCH, "precision or flavor count mismatch");
     if (overlap(out, in) && out->ptr != in->ptr) return fail(TM_ERR_ALIAS, "out partially overlaps in");
+    TM_USE_DEVICE(c);
     Coeffs co;
     int rc = make_coeffs(p, out->nf, dagger ? 1 : 0, inverse ? (int)TM_TWIST_INV_DSLASH : (int)TM_DSLASH_TWIST_XPAY, &co);
     if (rc) return rc;
@@ -615,7 +636,7 @@ int tm_prepare_rhs(tm_field *rhs_e, const tm_field *b_e, const tm_field *b_o, tm
 {
     if (!rhs_e || !b_e || !b_o || !tmp_o || !g || !p) return fail(TM_ERR_ARG, "tm_prepare_rhs: NULL argument");
     if (type != TM_MATPC_ASYM && type != TM_MATPC_SYM) return fail(TM_ERR_ARG, "bad matpc type %d", (int)type);
-    if (overlap(tmp_o, b_e) || overlap(tmp_o, rhs_e)) return fail(TM_ERR_ALIAS, "tmp_o aliases b_e or rhs_e");
+    if (overlap(tmp_o, b_e) || overlap(tmp_o, rhs_e) || overlap(tmp_o, b_o)) return fail(TM_ERR_ALIAS, "tmp_o aliases b_e, b_o or rhs_e");
     const tm_precision prec = (tm_precision)rhs_e->prec;
     int rc = tm_twist_apply(tmp_o, b_o, p, 1, 0);                                     // tmp_o = R_oo^-1 b_o
     if (rc) return rc;
@@ -756,6 +777,7 @@ int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, 
         return fail(TM_ERR_ARG, "need tol > 0, max_iter >= 1, 0 < delta < 1");
     if (type != TM_MATPC_ASYM && type != TM_MATPC_SYM) return fail(TM_ERR_ARG, "bad matpc type %d", (int)type);
     const int nf = x_e->nf;
+    TM_USE_DEVICE(c);
 
     WorkFields w;
     tm_field *r_d = w.make(c, TM_DOUBLE, nf), *t_d = w.make(c, TM_DOUBLE, nf), *te_d = w.make(c, TM_DOUBLE, nf), *to_d = w.make(c, TM_DOUBLE, nf);
@@ -763,10 +785,8 @@ int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, 
     tm_field *te_s = w.make(c, ps, nf), *to_s = w.make(c, ps, nf);
     if (!r_d || !t_d || !te_d || !to_d || !r_s || !p_s || !ap_s || !x_s || !te_s || !to_s) return fail(TM_ERR_NOMEM, "tm_invert_cg: work fields");
 
-    if (!c->cgs) {
-        TM_TRY_CUDA(cudaMalloc(&c->cgs, 4 * sizeof(double)), "cudaMalloc(cg scalars)");
-        TM_TRY_CUDA(cudaHostAlloc(&c->cgs_host, 6 * sizeof(double), cudaHostAllocDefault), "cudaHostAlloc(cg scalars)");
-    }
+    if (!c->cgs) TM_TRY_CUDA(cudaMalloc(&c->cgs, 4 * sizeof(double)), "cudaMalloc(cg scalars)");
+    if (!c->cgs_host) TM_TRY_CUDA(cudaHostAlloc(&c->cgs_host, 6 * sizeof(double), cudaHostAllocDefault), "cudaHostAlloc(cg scalars)");
     struct EventRing {
         cudaEvent_t ev[2] = {nullptr, nullptr};
         ~EventRing() { for (auto e : ev) if (e) cudaEventDestroy(e); }

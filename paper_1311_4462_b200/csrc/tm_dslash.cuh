@@ -1,7 +1,7 @@
 // tm_dslash.cuh -- the generic fused twisted-mass dslash kernel (rows a2-a9 of DESIGN.md).
 // One thread per output site (both flavors of a doublet); direct 128-bit read-only loads, neighbour reuse through L1/L2.
-// Works for every even lattice with extents >= 4; the tiled TMA path (tm_dslash_tma.cuh) takes over on
-// conforming lattices.
+// Works for every even lattice with extents >= 4.  The production path for fp64; fp32 and half run the packed
+// kernels of tm_dslash_f2.cuh and fall back to this one only for combinations those do not cover.
 //
 // gamma basis (C5):  gamma_k = [[0, i s_k], [-i s_k, 0]],  gamma_4 = diag(1,1,-1,-1),  gamma_5 swaps
 // the upper and lower two spin components.  With sgn = +1 for (1 - gamma_mu), -1 for (1 + gamma_mu):
@@ -266,13 +266,9 @@ cudaError_t tm_launch_generic(const DslashArgs &a, cudaStream_t s)
     const int blocks = (a.Vh + threads - 1) / threads;
     const size_t smem = STG ? (size_t)8 * RECON * PREC * threads : 0;
     if (smem > 48 * 1024) {
-        static bool raised = false;      // per instantiation
-        if (!raised) {
-            cudaError_t e = cudaFuncSetAttribute(tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG>,
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-            if (e != cudaSuccess) return e;
-            raised = true;
-        }
+        static std::atomic<unsigned long long> raised{0};      // per instantiation, one bit per device
+        cudaError_t e = tm_raise_smem(tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG>, raised);
+        if (e != cudaSuccess) return e;
     }
     tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG><<<blocks, threads, smem, s>>>(a);
     return cudaGetLastError();

@@ -557,13 +557,9 @@ cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
     const int blocks = (a.Vh + threads - 1) / threads;
     const size_t smem = STG ? (size_t)8 * RECON * PREC * threads : 0;
     if (smem > 48 * 1024) {
-        static bool raised = false;      // per instantiation
-        if (!raised) {
-            cudaError_t e = cudaFuncSetAttribute(tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG>,
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-            if (e != cudaSuccess) return e;
-            raised = true;
-        }
+        static std::atomic<unsigned long long> raised{0};      // per instantiation, one bit per device
+        cudaError_t e = tm_raise_smem(tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG>, raised);
+        if (e != cudaSuccess) return e;
     }
     tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG><<<blocks, threads, smem, s>>>(a);
     return cudaGetLastError();
@@ -575,15 +571,6 @@ cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
     {tm_launch_f2<P, N, R, K, false, true>, "f2_staged<" #P "," #N "," #R "," #K ",plain>"},       \
     {tm_launch_f2<P, N, R, K, true, false>, "f2<" #P "," #N "," #R "," #K ",dagger>"},             \
     {tm_launch_f2<P, N, R, K, true, true>, "f2_staged<" #P "," #N "," #R "," #K ",dagger>"}
-#ifdef TM_F2_SWEEP   /* working builds: only recon 12, kernel types A and B, plain */
-#define TM_F2_NONE {nullptr, "absent"}
-#define TM_F2_ROW0 TM_F2_NONE, TM_F2_NONE, TM_F2_NONE, TM_F2_NONE
-#define TM_F2_ROWS(P, N, R, K) {tm_launch_f2<P, N, R, K, false, false>, "f2<" #P "," #N "," #R "," #K ",plain>"}, {tm_launch_f2<P, N, R, K, false, true>, "f2_staged<" #P "," #N "," #R "," #K ",plain>"}, TM_F2_NONE, TM_F2_NONE
-#define TM_F2_TABLE(P, N)                                                                    \
-    static const TmKernelEntry f2table_##P##_##N[48] = {                                    \
-        TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROW0, TM_F2_ROWS(P, N, 12, 0), TM_F2_ROW0, TM_F2_ROWS(P, N, 12, 2), TM_F2_ROW0}; \
-    const TmKernelEntry *tm_f2_table_##P##_##N() { return f2table_##P##_##N; }
-#else
 // 8-real links: fp32 only, direct loads only (both staging slots hold the direct kernel); half has no entry (nullptr ->
 // tm_dslash_apply takes the scalar kernel)
 #define TM_F2_ROW8(N, K)                                                                           \
@@ -599,4 +586,3 @@ cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
         TM_F2_ROW(P, N, 18, 3), TM_F2_ROW(P, N, 12, 0), TM_F2_ROW(P, N, 12, 1),             \
         TM_F2_ROW(P, N, 12, 2), TM_F2_ROW(P, N, 12, 3) TM_F2_ROWS8_##P(N)};                 \
     const TmKernelEntry *tm_f2_table_##P##_##N() { return f2table_##P##_##N; }
-#endif

@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 #include <stddef.h>
 
+#include <atomic>
 #include <vector>
 
 #include "../../include/tm.h"
@@ -116,6 +117,21 @@ struct DslashArgs {
     int block_threads;   // threads per block (= sites per block)
     int pf_dist;         // L2 prefetch distance in thread blocks (0 = off): block b prefetches the tile of block b + pf_dist
 };
+
+// Kernels that stage more than 48 KB of shared memory need cudaFuncAttributeMaxDynamicSharedMemorySize raised; the
+// attribute is per DEVICE, so it is remembered per (instantiation, device id) in a bit mask, not per process.
+template <class K>
+inline cudaError_t tm_raise_smem(K kernel, std::atomic<unsigned long long> &done)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const unsigned long long bit = 1ULL << (dev & 63);
+    if (dev < 64 && (done.load(std::memory_order_relaxed) & bit)) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (e == cudaSuccess && dev < 64) done.fetch_or(bit, std::memory_order_relaxed);
+    return e;
+}
 
 // kernel launchers (one translation unit per precision x flavor count)
 typedef cudaError_t (*tm_launch_fn)(const DslashArgs &, cudaStream_t);
