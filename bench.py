@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the fused twisted-mass dslash hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--profile-brief]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--recon 18|12|8] [--sharded] [--no-extra]
+    python bench.py --sass-mix | --import-ncu FILE.csv      (host only: refresh profiles/sass_mix.csv / profiles/traffic.csv)
 
 One STEP = one pass of the whole hot path over the 32^3x64 lattice (BASELINE.json configs[2] and configs[3]):
   degenerate doublet (Haar links, 12-real, kappa=0.1632, mu=0.0015):   for fp64, fp32, half:  LHS of Eq. 2.2 (ASYM)
@@ -15,7 +16,9 @@ gauge fields (201-805 MB each) and the sweep's working set are far larger than t
 Multi-GPU: the path does not shard (BASELINE.json: one GPU, no halo exchange) -> replicas only; with --gpus N every
 rank runs the same step on its own GPU, value = N x units / max-over-ranks time, scaling "weak".
 
---impl reference times the CPU oracle (oracle/, fp64, as it stands) on the host cores on a bounded sample.
+--impl reference times the CPU oracle (oracle/, fp64, as it stands) on the host cores on the same full-lattice step.
+The JSON line also carries `kernels` (every launch of the step, timed inside the loop) and `kernels_extra` (every kernel type x
+precision x flavors x link compression of the library + the Wilson limit, each timed alone in the same run).
 """
 import argparse
 import json
@@ -149,19 +152,141 @@ def reduce_over_ranks(ms_local, world):
     return float(t.item())
 
 
-def ncu_traffic(name):
-    """DRAM read+write bytes per launch of kernel `name` from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.csv")
+def source_hash():
+    """sha256 (12 hex digits) over the kernel sources: ties the stored ncu traffic / SASS mix to the build being timed."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1311_4462_b200", "csrc")
+    for f in sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh")) + glob.glob(os.path.join(csrc, "*.h"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:12]
+
+
+def read_profile_table(fname):
+    """profiles/<fname>: '# source_hash=<h> ...' header, then 'kernel;v1;v2...' rows -> (hash or None, {kernel: [floats]})."""
+    path = os.path.join(ROOT, "profiles", fname)
+    rows, h = {}, None
     if not os.path.exists(path):
-        return None
+        return None, rows
     for line in open(path):
+        if line.startswith("#"):
+            for tok in line[1:].split():
+                if tok.startswith("source_hash="):
+                    h = tok.split("=", 1)[1]
+            continue
         f = [c.strip() for c in line.split(";")]
-        if len(f) >= 2 and f[0] == name:
+        try:
+            rows[f[0]] = [float(v) for v in f[1:]]
+        except ValueError:
+            continue
+    return h, rows
+
+
+def ncu_traffic(name):
+    """DRAM read+write bytes per launch of kernel `name` from the committed ncu summary (profiles/traffic.csv, written by
+    `bench.py --import-ncu`), or None when the kernel sources have changed since that capture (hash mismatch)."""
+    h, rows = read_profile_table("traffic.csv")
+    if h != source_hash() or name not in rows:
+        return None
+    return rows[name][0]
+
+
+def sass_mix(name):
+    """(packed FP32, integer-pipe, scalar FP32, all) instructions per thread of kernel `name` from profiles/sass_mix.csv
+    (written by `bench.py --sass-mix` from cuobjdump -sass of the built objects), or None on a hash mismatch."""
+    h, rows = read_profile_table("sass_mix.csv")
+    if h != source_hash() or name not in rows:
+        return None
+    return rows[name]
+
+
+PACKED_OPS = ("FFMA2", "FMUL2", "FADD2")
+INT_OPS = ("PRMT", "IADD3", "IMAD", "SHF", "LOP3", "ISETP", "LEA", "SEL", "MOV", "VIADDMNMX", "IABS", "FMNMX3", "FMNMX", "FSEL", "FSETP", "PLOP3")
+FP32_OPS = ("FFMA", "FMUL", "FADD")
+FP64_OPS = ("DFMA", "DMUL", "DADD")
+
+
+def write_sass_mix():
+    """--sass-mix: opcode histogram of every fused-dslash kernel in the built objects -> profiles/sass_mix.csv (one row per
+    kernel: packed FP32; integer pipe; scalar FP32; FP64; all) and profiles/r2_sass_histogram.md (the full histograms)."""
+    import glob
+    import re
+    build = os.path.join(ROOT, "paper_1311_4462_b200", "csrc", "build")
+    rows, md = [], []
+    for obj in sorted(glob.glob(os.path.join(build, "tm_f2_*.o")) + glob.glob(os.path.join(build, "tm_generic_*.o"))):
+        txt = subprocess.run(["cuobjdump", "-sass", obj], capture_output=True, text=True).stdout
+        for blk in txt.split("Function : ")[1:]:
+            mangled = blk.split("\n", 1)[0].strip()
+            m = re.match(r"_Z\d+tm_dslash_(f2|generic)ILi(\d)ELi(\d)ELi(\d+)ELi(\d)ELb([01])ELb([01])E", mangled)
+            if not m:
+                continue
+            fam, prec, nf, recon, kt, dag, stg = m.groups()
+            name = "%s%s<%s,%s,%s,%s,%s>" % (fam, "_staged" if stg == "1" else "", prec, nf, recon, kt, "dagger" if dag == "1" else "plain")
+            hist = {}
+            for line in blk.splitlines():
+                mm = re.match(r"\s+/\*[0-9a-f]{4,}\*/\s+(?:@!?U?P\w+\s+)?([A-Z][A-Z0-9_]*)", line)
+                if mm:
+                    hist[mm.group(1)] = hist.get(mm.group(1), 0) + 1
+            for k in ("NOP", "BRA", "EXIT"):
+                hist.pop(k, None)
+            tot = sum(hist.values())
+            cnt = lambda ops: sum(hist.get(o, 0) for o in ops)
+            rows.append((name, cnt(PACKED_OPS), cnt(INT_OPS), cnt(FP32_OPS), cnt(FP64_OPS), tot))
+            md.append("| `%s` | %d | %s |" % (name, tot, " ".join("%s:%d" % kv for kv in sorted(hist.items(), key=lambda kv: -kv[1])[:18])))
+    hsh = source_hash()
+    commit = subprocess.run(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip()
+    with open(os.path.join(ROOT, "profiles", "sass_mix.csv"), "w") as f:
+        f.write("# source_hash=%s parent_commit=%s  kernel ; packed FP32 (FFMA2/FMUL2/FADD2) ; integer pipe ; scalar FP32 ; FP64 ; all  "
+                "(static instruction counts per thread, both sides of the few branches; written by `python bench.py --sass-mix`)\n" % (hsh, commit))
+        for r in rows:
+            f.write(";".join(str(v) for v in r) + "\n")
+    with open(os.path.join(ROOT, "profiles", "r2_sass_histogram.md"), "w") as f:
+        f.write("# r2: SASS opcode histogram of every fused dslash kernel\n\nCommand: `python -m paper_1311_4462_b200.build && python bench.py --sass-mix` "
+                "(cuobjdump -sass of `paper_1311_4462_b200/csrc/build/*.o`; source_hash=%s, parent commit %s).\n"
+                "Static counts per thread (NOP / BRA / EXIT dropped); the kernels are straight-line code, so static = executed up to the prefetch prologue.\n\n"
+                "| kernel | instructions | top opcodes |\n|---|---|---|\n" % (hsh, commit))
+        f.write("\n".join(md) + "\n")
+    print("wrote profiles/sass_mix.csv (%d kernels), profiles/r2_sass_histogram.md" % len(rows))
+
+
+def import_ncu(csv_path):
+    """--import-ncu FILE: an `ncu --csv --page raw` export (metrics dram__bytes_read.sum, dram__bytes_write.sum) of THIS build
+    -> profiles/traffic.csv with the source hash, mean per launch and kernel."""
+    import csv
+    import re
+    acc = {}
+    with open(csv_path, newline="") as f:
+        rd = csv.reader(f)
+        hdr = None
+        for row in rd:
+            if hdr is None:
+                if "Kernel Name" in row:
+                    hdr = row
+                continue
+            if len(row) != len(hdr) or not row[0].isdigit():
+                continue
+            d = dict(zip(hdr, row))
+            m = re.search(r"tm_dslash_(f2|generic)<\(?int\)?(\d), \(?int\)?(\d), \(?int\)?(\d+), \(?int\)?(\d), \(?bool\)?(\w+), \(?bool\)?(\w+)>", d["Kernel Name"].replace("(int)", "").replace("(bool)", ""))
+            if not m:
+                continue
+            fam, prec, nf, recon, kt, dag, stg = m.groups()
+            name = "%s%s<%s,%s,%s,%s,%s>" % (fam, "_staged" if stg in ("1", "true") else "", prec, nf, recon, kt, "dagger" if dag in ("1", "true") else "plain")
             try:
-                return float(f[1])
-            except ValueError:
-                return None
-    return None
+                b = float(d["dram__bytes_read.sum"].replace(",", "")) + float(d["dram__bytes_write.sum"].replace(",", ""))
+            except (KeyError, ValueError):
+                continue
+            a = acc.setdefault(name, [0.0, 0])
+            a[0] += b
+            a[1] += 1
+    commit = subprocess.run(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip()
+    with open(os.path.join(ROOT, "profiles", "traffic.csv"), "w") as f:
+        f.write("# source_hash=%s parent_commit=%s  kernel ; DRAM bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean over "
+                "the captured launches; written by `python bench.py --import-ncu %s`)\n" % (source_hash(), commit, os.path.basename(csv_path)))
+        for name, (tot, n) in sorted(acc.items()):
+            f.write("%s;%d\n" % (name, round(tot / n)))
+    print("wrote profiles/traffic.csv (%d kernels)" % len(acc))
 
 
 class Workload:
@@ -244,26 +369,33 @@ def oracle_step(ora, si, dims, gauge, inp, sample_desc):
 
 
 def run_reference(args, log):
-    """--impl reference: the oracle as it stands on the host cores, bounded sample = a 32^3 x 8 time slab."""
+    """--impl reference: the oracle as it stands on the host cores, the SAME workload as our arm's step: one fp64 pass of the
+    step's 4 distinct operators on the full 32^3x64 lattice per step (~1.6 s on 16 cores).  Steps are capped by --ref-steps
+    (default 5) and warm-up by 1 so that the run ends within a few minutes; the caps are reported."""
     import oracle as ora
     import synth_inputs as si
-    dims = (32, 32, 32, 8)
+    dims = DIMS
+    t = time.time()
     gauge = {1: si.gauge_field(dims, SEED_DEG, "haar"), 2: si.gauge_field(dims, SEED_NDEG, "near_identity")}
     inp = {nf: si.mask_parity(si.spinor_field(dims, nf, s), dims, 0) for nf, s in ((1, SEED_DEG), (2, SEED_NDEG))}
-    sample = "32^3x8 time slab (1/8 of the 32^3x64 lattice), the step's 4 distinct operators (deg ASYM, SYM; ndeg ASYM, ASYM-dagger) once each in fp64"
-    for _ in range(args.warmup):
+    log("host inputs generated in %.1f s" % (time.time() - t))
+    sample = ("full 32^3x64 lattice: the step's 4 distinct operators (deg ASYM, SYM; ndeg ASYM, ASYM-dagger) once each in fp64 per step "
+              "(the oracle has one precision; our arm runs them in fp64 / fp32 / half)")
+    steps, warm = max(1, min(args.steps, args.ref_steps)), min(args.warmup, 1)
+    for _ in range(warm):
         oracle_step(ora, si, dims, gauge, inp, sample)
     tot_s, tot_f = 0.0, 0
-    for _ in range(args.steps):
+    for _ in range(steps):
         s, f = oracle_step(ora, si, dims, gauge, inp, sample)
         tot_s += s
         tot_f += f
     val = tot_f / tot_s / 1e9
     cores = ora.num_threads()
-    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": "GFLOPS", "n_gpus": args.gpus, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps, "higher_is_better": True, "scaling": "weak",
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": "GFLOPS", "n_gpus": args.gpus, "steps": steps,
+           "warmup": warm, "steps_requested": args.steps, "warmup_requested": args.warmup, "ms_per_step": 1e3 * tot_s / steps,
+           "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": WORKLOAD % (RECON, RECON), "sample": sample},
+           "config": {"workload": WORKLOAD % (RECON, RECON), "lattice": list(dims), "sample": sample},
            "cpu_baseline": {"value": val, "unit": "GFLOPS", "cores": cores, "kind": "oracle", "sample": sample},
            "e2e": {"value": val, "unit": "GFLOPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
@@ -275,6 +407,86 @@ WORKLOAD = ("32^3x64: configs[2] degenerate (Haar links, %d-real, mu=0.0015) ASY
             "non-degenerate (exp(i0.3H) links, %d-real, mu=0.15, eps=0.19) ASYM plain+dagger in fp32/half")
 # plain-ALU peak: 128 FP32 / 64 FP64 FMA lanes per SM, 148 SMs, 2 flop per FMA, at the SM clock under load
 SMS, LANES = 148, {8: 64, 4: 128, 2: 128}
+
+
+SMSPS = 148 * 4
+CYC = {"packed": 2.0, "int": 1.0, "fp32": 1.0, "fp64": 2.0}
+
+
+def annotate_bound(k, vh, sm_mhz):
+    """Adds the plain-ALU flop fraction and the datapath fraction (see run_ours) to a kernel record; names the bound."""
+    pb = k.pop("prec_bytes")
+    alu_peak = SMS * LANES[pb] * 2 * sm_mhz * 1e-3      # GFLOPS
+    k["alu_peak_gflops"] = alu_peak
+    k["frac_of_alu_peak"] = k["gflops"] / alu_peak
+    mix = sass_mix(k["kernel"])
+    k["frac_of_datapath"] = None
+    if mix:
+        packed, integer, fp32, fp64 = mix[0], mix[1], mix[2], mix[3]
+        cyc = CYC["packed"] * packed + CYC["int"] * integer + CYC["fp32"] * fp32 + CYC["fp64"] * fp64
+        floor_us = cyc * (vh / 32.0) / SMSPS / sm_mhz
+        k["datapath_cycles_per_warp"] = cyc
+        k["frac_of_datapath"] = floor_us / k["us"]
+    k["bound"] = "alu" if (k["frac_of_datapath"] or 0.0) > k["frac_of_measured_peak"] else "hbm"
+
+
+def time_alone(fn, sync, launches=20, reps=3):
+    """Mean microseconds per launch of fn(), `launches` back to back between two CUDA events, best of `reps`."""
+    import torch
+    for _ in range(10):
+        fn()
+    sync()
+    best = None
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(launches):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        t = e0.elapsed_time(e1) / launches * 1e3
+        best = t if best is None else min(best, t)
+    return best
+
+
+def kernels_extra(w, args, sm_mhz, peak):
+    """Every (kernel type x precision x flavors x link compression) of the library, each timed ALONE in this run (20 launches
+    between two CUDA events, best of 3) at 32^3x64 through tm_dslash_apply -- outside `value`, whose step stays BASELINE.json's.
+    Rows: 12- / 18- / 8-real x fp64 / fp32 / half x degenerate / doublet x A / A-xpay / B / REC, and the Wilson limit
+    (mu = eps = 0: the paper's Table 1 Wilson column) of kernel A."""
+    tm, lat, vh = w.tm, w.lat, w.vh
+    out = []
+    host_u = w.host_gauge[1]
+    for _ in range(20):          # the GPU idled during the CPU baseline: bring the clocks back up before timing anything
+        w.step()
+    lat.sync()
+    fields = {}
+    for prec in (8, 4, 2):
+        for nf in (1, 2):
+            fin = w.fin.get((nf, prec)) or lat.field(prec, nf).upload_cb(0, w.host_in[nf])
+            fx = lat.field(prec, nf).upload_cb(0, w.host_in[nf])
+            fields[(prec, nf)] = (fin, fx, w.fout.get((nf, prec)) or lat.field(prec, nf))
+    wilson = tm.params(KAPPA, mu=0.0, epsilon=0.0, twist_flavor=1)
+    for recon in (12, 18, 8):
+        for prec in (8, 4, 2):
+            g = w.gauge.get((1, prec)) if recon == RECON else None
+            g = g or lat.gauge(host_u, prec, recon)
+            for nf in (1, 2):
+                fin, fx, fout = fields[(prec, nf)]
+                for kt, label in ((0, "A"), (1, "A-xpay"), (2, "B"), (3, "REC"), (0, "A wilson")):
+                    if label == "A wilson" and (nf == 2 or recon != 12):
+                        continue
+                    p = wilson if label == "A wilson" else w.params[nf]
+                    us = time_alone(lambda: tm.dslash_apply(fout, fin, None if kt == 0 else fx, g, p, 1, 0, kt), lat.sync)
+                    b = bytes_per_site(nf, prec, recon, kt) * vh
+                    f = flops_per_site(nf, kt) * vh
+                    k = {"kernel": tm.tm_last_kernel_name(lat.ctx), "flavors": nf, "prec": PREC_NAME[prec], "type": label, "recon": recon,
+                         "us": us, "gflops": f / us / 1e3, "alg_gbs": b / us / 1e3, "frac_of_measured_peak": b / us / 1e3 / peak,
+                         "bytes_per_site": bytes_per_site(nf, prec, recon, kt), "prec_bytes": prec}
+                    annotate_bound(k, vh, sm_mhz)
+                    out.append(k)
+            del g
+    return out
 
 
 def run_ours(args, log):
@@ -359,6 +571,8 @@ def run_ours(args, log):
     if dom:
         roofline = {"bound": "hbm", "kernel": dom["kernel"], "achieved": dom["alg_gbs"], "peak": peak, "unit": "GB/s",
                     "frac": dom["alg_gbs"] / peak, "traffic": ncu_traffic(dom["kernel"]), "peak_source": peak_src,
+                    "traffic_source": "committed ncu --set full summary of this build (profiles/traffic.csv, source hash %s); null when the "
+                                      "kernel sources have changed since the capture" % source_hash(),
                     "bytes_per_launch": dom["bytes_per_site"] * vh, "us_per_launch": dom["us"],
                     "step_alg_gbs": step_bytes / (ms_per_step * 1e-3) / 1e9,
                     "step_frac": step_bytes / (ms_per_step * 1e-3) / 1e9 / peak}
@@ -391,15 +605,15 @@ def run_ours(args, log):
         cpu = {"value": f / s / 1e9, "unit": "GFLOPS", "cores": ora.num_threads(), "kind": "oracle", "sample": sample,
                "seconds": s}
 
-    # second roofline per kernel: useful flops against the plain-ALU peak at the clock seen under load
+    # second roofline per kernel (profiles/r2_pipes.md): the FP32 / integer datapath.  Executed instructions
+    # per thread by class (profiles/sass_mix.csv, from cuobjdump of this build) x the LEAST each can cost per warp and sub-partition
+    # (packed FP32 and FP64: 2 cycles of the 32- / 16-lane pipe; integer-pipe and scalar FP32: their issue slot, 1 cycle -- measured
+    # 2.08 alone and 1.07-2.6 next to FFMA2) = cycles the datapath needs per warp; x warps per sub-partition / SM clock = a time below
+    # which the kernel cannot run.  A conservative floor: bound = "alu" only when even this fraction exceeds the HBM fraction.
     sm_mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0
     for k in kernels:
-        alu_peak = SMS * LANES[k.pop("prec_bytes")] * 2 * sm_mhz * 1e-3      # GFLOPS
-        k["alu_peak_gflops"] = alu_peak
-        k["frac_of_alu_peak"] = k["gflops"] / alu_peak
-        # the half kernels are limited by the FP32 pipe (ncu fma pipe 63-66 % busy, math-pipe throttle the top
-        # stall, same run time with 32 % more link bytes); everything else by HBM
-        k["bound"] = "alu" if k["prec"] == "half" else "hbm"
+        annotate_bound(k, vh, sm_mhz)
+    extra = kernels_extra(w, args, sm_mhz, peak) if (rank == 0 and world == 1 and not args.no_extra) else None
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": "GFLOPS", "n_gpus": world, "steps": args.steps,
                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -409,7 +623,7 @@ def run_ours(args, log):
                           if args.sharded else ("replicas only (north_star: no sharding)" if world > 1 else "single GPU"),
                           "l2": "inputs larger than L2 (gauge fields 201-805 MB each, 2.3 GB touched per step)"},
                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-               "step_flops": step_flops, "step_alg_bytes": step_bytes, "kernels": kernels,
+               "step_flops": step_flops, "step_alg_bytes": step_bytes, "kernels": kernels, "kernels_extra": extra,
                "paper_table1_gflops_12real": {"%s/%s" % ("deg" if k[0] == 1 else "ndeg", PREC_NAME[k[1]]): v
                                               for k, v in PAPER_GFLOPS.items()},
                "paper_table1_gflops_8real": {"%s/%s" % ("deg" if k[0] == 1 else "ndeg", PREC_NAME[k[1]]): v
@@ -427,7 +641,11 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--ref-steps", type=int, default=5, help="--impl reference: cap on the timed full-lattice oracle steps (1.6 s each)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the kernels_extra table (every kernel type x precision x compression, timed alone)")
+    ap.add_argument("--sass-mix", action="store_true", help="host only: write profiles/sass_mix.csv + profiles/r2_sass_histogram.md from the built objects")
+    ap.add_argument("--import-ncu", metavar="CSV", help="host only: turn an `ncu --csv --page raw` export of this build into profiles/traffic.csv")
     ap.add_argument("--path", type=int, default=0, help="tm_set_path: 0 = default kernel selection, 1 = scalar kernels only")
     ap.add_argument("--sharded", action="store_true",
                     help="each rank holds a 32^3x64 slab of a 32^3 x (64 N) lattice: kernels with open time hops, face exchange over "
@@ -437,6 +655,24 @@ def main():
     args = ap.parse_args()
     global RECON
     RECON = args.recon
+    if args.sass_mix:
+        return write_sass_mix()
+    if args.import_ncu:
+        return import_ncu(args.import_ncu)
+    # --gpus N: one process per GPU.  Under torch.distributed.run (WORLD_SIZE set) the count must agree; a plain
+    # `python bench.py --gpus N` starts the N ranks itself by re-executing under torch.distributed.run on this node.
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is not None and int(world_env) != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%s" % (args.gpus, world_env))
+    if world_env is None and args.gpus > 1:
+        import socket
+        s = socket.socket()
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+        s.close()
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     rank = int(os.environ.get("RANK", "0"))
 
     def log(msg):
