@@ -159,6 +159,7 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->path = 0;
     c->pf_dist = -1;
     c->stage = -1;
+    c->z_chunks = -1;
     c->block_threads = 0;
     c->sm_count = 0;
     c->basis_on = 0;
@@ -313,6 +314,11 @@ int tm_set_tuning(tm_ctx *ctx, const char *key, int value)
     if (!strcmp(key, "stage_links")) {
         if (value < -1 || value > 1) return fail(TM_ERR_ARG, "stage_links must be -1 (default), 0 or 1");
         ctx->stage = value;
+        return TM_OK;
+    }
+    if (!strcmp(key, "z_chunks")) {
+        if (value < -1 || value == 0) return fail(TM_ERR_ARG, "z_chunks must be -1 (default) or >= 1");
+        ctx->z_chunks = value;
         return TM_OK;
     }
     if (!strcmp(key, "block_threads")) {
@@ -563,6 +569,21 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.block_threads = c->block_threads ? c->block_threads : 128;
     if (g->recon == 8) stage = 0;        // 8-real links: direct loads
     while (stage && (size_t)8 * g->recon * (int)prec * a.block_threads > 96 * 1024 && a.block_threads > 32) a.block_threads /= 2;
+
+    // z-chunked traversal: the input spinor is re-read over a window of three time slices; when those (next to the streaming
+    // links and the output) do not fit the L2, the lattice is walked in chunks of Z / nzc z-planes (profiles/r2_tuning.md)
+    {
+        const size_t slice = (size_t)c->g.Xh * c->g.X[1] * c->g.X[2];                          // sites of one parity per time slice
+        const size_t window = 3 * slice * (size_t)out->nf * 24 * (int)prec;
+        int nzc = c->z_chunks >= 1 ? c->z_chunks : 1;
+        if (c->z_chunks < 0)
+            while (window / nzc > (size_t)40 << 20 && nzc < c->g.X[2]) nzc *= 2;
+        while (nzc > 1 && (c->g.X[2] % nzc != 0 || (slice / nzc) % a.block_threads != 0 || slice / nzc / a.block_threads < 2)) nzc--;
+        a.nzc = nzc;
+        a.bpz = (int)(slice / nzc / a.block_threads);
+        if (nzc > 1) { a.dbpc = tm_fastdiv(a.bpz * c->g.X[3]); a.dbpz = tm_fastdiv(a.bpz); }
+        else { a.dbpc = tm_fastdiv(2); a.dbpz = tm_fastdiv(2); }
+    }
 
     // path 0: fp32 / half run the packed-FP32 kernels, fp64 the scalar kernel; path 1 forces the scalar kernel
     // (8-real links: packed kernels exist for fp32 only; half takes the scalar kernel)

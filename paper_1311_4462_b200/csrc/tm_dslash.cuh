@@ -191,8 +191,9 @@ __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? TM_MINB_
 {
     typedef typename PrecTraits<PREC>::real real;
     const int Vh = a.Vh;
-    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, blockIdx.x);
-    const int site = blockIdx.x * blockDim.x + threadIdx.x;        // one thread per output site, all flavors
+    const int vblock = tm_virtual_block(a, blockIdx.x);
+    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, vblock);
+    const int site = vblock * blockDim.x + threadIdx.x;        // one thread per output site, all flavors
     if (site >= Vh) return;
 
     // a2: site decode and neighbours

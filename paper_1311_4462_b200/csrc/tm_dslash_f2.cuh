@@ -94,9 +94,10 @@ TM_DEV unsigned ldg_nc_u1(const void *p)
     asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(p));
     return v;
 }
-template <bool SM> TM_DEV uint4 ld_u4(const void *p) { if constexpr (SM) return *reinterpret_cast<const uint4 *>(p); else return ldg_nc_u4(p); }
-template <bool SM> TM_DEV uint2 ld_u2(const void *p) { if constexpr (SM) return *reinterpret_cast<const uint2 *>(p); else return ldg_nc_u2(p); }
-template <bool SM> TM_DEV unsigned ld_u1(const void *p) { if constexpr (SM) return *reinterpret_cast<const unsigned *>(p); else return ldg_nc_u1(p); }
+// link words: from the staged shared-memory copy (SM) or streaming from global memory (L2 evict-first, tm_layout.cuh)
+template <bool SM> TM_DEV uint4 ld_u4(const void *p) { if constexpr (SM) return *reinterpret_cast<const uint4 *>(p); else return ldg_stream_u4(p); }
+template <bool SM> TM_DEV uint2 ld_u2(const void *p) { if constexpr (SM) return *reinterpret_cast<const uint2 *>(p); else return ldg_stream_u2(p); }
+template <bool SM> TM_DEV unsigned ld_u1(const void *p) { if constexpr (SM) return *reinterpret_cast<const unsigned *>(p); else return ldg_stream_u1(p); }
 
 // a4 (fetch): the stored words of one link; `lp` = the link's site pointer in global memory or in the staged copy
 template <int PREC, int NF, int RECON, bool SM>
@@ -120,11 +121,11 @@ TM_DEV void issue_spinor(HopRaw<PREC, NF, RECON> &r, const char *sp, int lane)
         if constexpr (PREC == 4) {
             constexpr int lo = (PART == 2) ? 3 : 0, hi = (PART == 1) ? 3 : 6;
 #pragma unroll
-            for (int k = lo; k < hi; k++) r.s[f][k] = ld_u4<false>(p + k * TM_PLANE);
+            for (int k = lo; k < hi; k++) r.s[f][k] = ldg_nc_u4(p + k * TM_PLANE);
         } else {
-            if constexpr (PART != 2) r.s[f][0] = ld_u4<false>(p);
-            r.s[f][1] = ld_u4<false>(p + TM_PLANE);
-            if constexpr (PART != 1) r.s[f][2] = ld_u4<false>(p + 2 * TM_PLANE);
+            if constexpr (PART != 2) r.s[f][0] = ldg_nc_u4(p);
+            r.s[f][1] = ldg_nc_u4(p + TM_PLANE);
+            if constexpr (PART != 1) r.s[f][2] = ldg_nc_u4(p + 2 * TM_PLANE);
             r.n[f] = __uint_as_float(ldg_nc_u1(p + tail_off(3, 4, lane)));
         }
     }
@@ -503,8 +504,9 @@ __global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(c
 {
     constexpr int PD = f2_pipeline_depth<PREC, NF>();
     const int Vh = a.Vh;
-    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, blockIdx.x);
-    const int site = blockIdx.x * blockDim.x + threadIdx.x;
+    const int vblock = tm_virtual_block(a, blockIdx.x);
+    prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, vblock);
+    const int site = vblock * blockDim.x + threadIdx.x;
     if (site >= Vh) return;
 
     HopPtrs p;

@@ -37,6 +37,7 @@ struct tm_ctx {
     int pf_dist; // tm_set_tuning("prefetch_blocks")
     int stage;   // tm_set_tuning("stage_links"): -1 library default, 0 direct loads, 1 links staged through shared memory
     int block_threads;   // tm_set_tuning("block_threads"): 0 library default, else 32 / 64 / 128
+    int z_chunks;        // tm_set_tuning("z_chunks"): -1 library default (from the L2 working set), else the number of z-chunks
     int sm_count;
     int basis_on;         // tm_set_host_basis: host spinors are in another spin basis, psi_device = S psi_host
     double basis[32];     // S, row-major [4][4][re, im]
@@ -116,7 +117,25 @@ struct DslashArgs {
     double tbound;       // +-1, multiplies the time hop that wraps
     int block_threads;   // threads per block (= sites per block)
     int pf_dist;         // L2 prefetch distance in thread blocks (0 = off): block b prefetches the tile of block b + pf_dist
+    // z-chunked traversal (tm_virtual_block): thread blocks walk the lattice chunk by chunk of Z / nzc z-planes, all time slices
+    // of a chunk before the next chunk, so that the three time slices of input spinor a block range re-reads fit the L2
+    int nzc;             // number of z-chunks (1 = plain index order)
+    int bpz;             // thread blocks per (time slice, chunk)
+    TmFastDiv dbpc, dbpz;   // division by bpz * T and by bpz
 };
+#ifdef __CUDACC__
+// The block of sites that thread block b works on.  nzc == 1: b itself.  Otherwise b counts (chunk, t, block within the chunk's
+// part of slice t), while site order is (t, z, y, x): the virtual block is (t * nzc + chunk) * bpz + w.
+__device__ __forceinline__ int tm_virtual_block(const DslashArgs &a, int b)
+{
+    if (a.nzc <= 1) return b;
+    const int c = tm_div(b, a.dbpc);
+    const int r = b - c * a.dbpc.d;
+    const int t = tm_div(r, a.dbpz);
+    const int w = r - t * a.bpz;
+    return (t * a.nzc + c) * a.bpz + w;
+}
+#endif
 
 // Kernels that stage more than 48 KB of shared memory need cudaFuncAttributeMaxDynamicSharedMemorySize raised; the
 // attribute is per DEVICE, so it is remembered per (instantiation, device id) in a bit mask, not per process.

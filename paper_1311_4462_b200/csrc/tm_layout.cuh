@@ -54,13 +54,83 @@ TM_DEV int4 ldg_i4(const void *p) { return __ldg(reinterpret_cast<const int4 *>(
 TM_DEV int2 ldg_i2(const void *p) { return __ldg(reinterpret_cast<const int2 *>(p)); }
 TM_DEV int ldg_i1(const void *p) { return __ldg(reinterpret_cast<const int *>(p)); }
 TM_DEV float ldg_f1(const void *p) { return __ldg(reinterpret_cast<const float *>(p)); }
-// SM = true: the pointer is shared memory (staged links, tm_stream.cuh) -> plain loads
-template <bool SM> TM_DEV double2 ld_d2(const void *p) { if constexpr (SM) return *reinterpret_cast<const double2 *>(p); else return ldg_d2(p); }
-template <bool SM> TM_DEV float4 ld_f4(const void *p) { if constexpr (SM) return *reinterpret_cast<const float4 *>(p); else return ldg_f4(p); }
-template <bool SM> TM_DEV float2 ld_f2(const void *p) { if constexpr (SM) return *reinterpret_cast<const float2 *>(p); else return ldg_f2(p); }
-template <bool SM> TM_DEV int4 ld_i4(const void *p) { if constexpr (SM) return *reinterpret_cast<const int4 *>(p); else return ldg_i4(p); }
-template <bool SM> TM_DEV int2 ld_i2(const void *p) { if constexpr (SM) return *reinterpret_cast<const int2 *>(p); else return ldg_i2(p); }
-template <bool SM> TM_DEV int ld_i1(const void *p) { if constexpr (SM) return *reinterpret_cast<const int *>(p); else return ldg_i1(p); }
+// The gauge field is read exactly once per launch and is most of the traffic; the input spinor is read 8 times (once per
+// neighbouring output site) over a window of two time slices.  On lattices whose time slice (both gauge parities + spinor) does
+// not fit the 126 MB L2 next to the streaming links (48^3 x 96: ~85 MB of links per slice), the links evict the spinor before
+// its reuse and DRAM traffic rises above the algorithmic bytes.  Link loads therefore carry an L2 evict-first policy
+// (createpolicy + ld.global.nc.L2::cache_hint): they leave the L2 first, the spinor stays.
+#ifndef TM_LINK_HINT
+#define TM_LINK_HINT 1
+#endif
+TM_DEV unsigned long long tm_policy_stream()
+{
+    unsigned long long p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+TM_DEV double2 ldg_stream_d2(const void *p)
+{
+#if TM_LINK_HINT
+    double2 v;
+    asm("ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(tm_policy_stream()));
+    return v;
+#else
+    return ldg_d2(p);
+#endif
+}
+TM_DEV uint4 ldg_stream_u4(const void *p)
+{
+    uint4 v;
+#if TM_LINK_HINT
+    asm("ld.global.nc.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(tm_policy_stream()));
+#else
+    asm("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+#endif
+    return v;
+}
+TM_DEV uint2 ldg_stream_u2(const void *p)
+{
+    uint2 v;
+#if TM_LINK_HINT
+    asm("ld.global.nc.L2::cache_hint.v2.u32 {%0, %1}, [%2], %3;" : "=r"(v.x), "=r"(v.y) : "l"(p), "l"(tm_policy_stream()));
+#else
+    asm("ld.global.nc.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+#endif
+    return v;
+}
+TM_DEV unsigned ldg_stream_u1(const void *p)
+{
+    unsigned v;
+#if TM_LINK_HINT
+    asm("ld.global.nc.L2::cache_hint.u32 %0, [%1], %2;" : "=r"(v) : "l"(p), "l"(tm_policy_stream()));
+#else
+    asm("ld.global.nc.u32 %0, [%1];" : "=r"(v) : "l"(p));
+#endif
+    return v;
+}
+// link loads.  SM = true: the pointer is shared memory (staged links, tm_stream.cuh) -> plain loads; else streaming global loads
+template <bool SM> TM_DEV double2 ld_d2(const void *p) { if constexpr (SM) return *reinterpret_cast<const double2 *>(p); else return ldg_stream_d2(p); }
+template <bool SM> TM_DEV float4 ld_f4(const void *p)
+{
+    if constexpr (SM) return *reinterpret_cast<const float4 *>(p);
+    else { const uint4 v = ldg_stream_u4(p); return make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w)); }
+}
+template <bool SM> TM_DEV float2 ld_f2(const void *p)
+{
+    if constexpr (SM) return *reinterpret_cast<const float2 *>(p);
+    else { const uint2 v = ldg_stream_u2(p); return make_float2(__uint_as_float(v.x), __uint_as_float(v.y)); }
+}
+template <bool SM> TM_DEV int4 ld_i4(const void *p)
+{
+    if constexpr (SM) return *reinterpret_cast<const int4 *>(p);
+    else { const uint4 v = ldg_stream_u4(p); return make_int4((int)v.x, (int)v.y, (int)v.z, (int)v.w); }
+}
+template <bool SM> TM_DEV int2 ld_i2(const void *p)
+{
+    if constexpr (SM) return *reinterpret_cast<const int2 *>(p);
+    else { const uint2 v = ldg_stream_u2(p); return make_int2((int)v.x, (int)v.y); }
+}
+template <bool SM> TM_DEV int ld_i1(const void *p) { if constexpr (SM) return *reinterpret_cast<const int *>(p); else return (int)ldg_stream_u1(p); }
 
 // Stored int16 are OFFSET BINARY (u = q + 32768, see tm_f2.cuh): two per 32-bit word -> two floats (exact), times s
 TM_DEV void unpack2(int w, float s, float &lo, float &hi)

@@ -52,6 +52,7 @@ def bench_for(dims, kind, seed):
     tm.tm_set_tuning(ctx, "stage_links", -1)
     tm.tm_set_tuning(ctx, "block_threads", 0)
     tm.tm_set_tuning(ctx, "prefetch_blocks", -1)
+    tm.tm_set_tuning(ctx, "z_chunks", -1)
     return _cache[key]
 
 
@@ -149,6 +150,32 @@ def test_t2_every_kernel_variant_matches_oracle(dims, kind, kw, variant):
             assert err <= TOL[prec], (PREC_NAME[prec], recon, parity, dagger, kt, err)
             assert np.abs(si.mask_parity(got, dims, 1 - parity)).max() == 0
     print("worst rel L2:", {PREC_NAME[k]: v for k, v in worst.items()})
+
+
+@pytest.mark.parametrize("kw", [FLAVORS[0], FLAVORS[2]], ids=["deg", "ndeg"])
+@pytest.mark.parametrize("chunks,threads", [(2, 128), (4, 64), (8, 32)])
+def test_t2e_z_chunked_traversal_matches_oracle(kw, chunks, threads):
+    """tm_set_tuning("z_chunks"): the thread blocks walk the lattice chunk by chunk of Z / n z-planes (the library turns this on
+    by itself when three time slices of the input do not fit the L2, e.g. 48^3 x 96 fp64 doublet).  A permutation of the block
+    order only: every kernel type must still match the oracle.  16 x 8 x 16 x 6: 1024 sites per slice and parity."""
+    dims, nf = (16, 8, 16, 6), nf_of(kw)
+    bench = bench_for(dims, "haar", 6)
+    tm.tm_set_tuning(bench.lat.ctx, "z_chunks", chunks)
+    tm.tm_set_tuning(bench.lat.ctx, "block_threads", threads)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    full_in, full_x = si.spinor_field(dims, nf, 2), si.spinor_field(dims, nf, 3)
+    for parity, dagger, kt in ((0, 0, 0), (1, 1, 1), (0, 1, 2), (1, 0, 3)):
+        inp, x = si.mask_parity(full_in, dims, 1 - parity), si.mask_parity(full_x, dims, parity)
+        want = oracle.kernel(inp, x, bench.U, po, parity, dagger, kt)
+        for prec in PRECS:
+            got = bench.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, prec, tm.TM_RECON_12, nf)
+            assert rel_l2(got, want) <= TOL[prec], (PREC_NAME[prec], parity, dagger, kt, rel_l2(got, want))
+    for path in (0, 1):                      # packed and scalar kernels
+        tm.tm_set_path(bench.lat.ctx, path)
+        inp = si.mask_parity(full_in, dims, 0)
+        want = oracle.matpc(inp, bench.U, po, oracle.SYM, 0)
+        got = bench.matpc(inp, pg, tm.TM_MATPC_SYM, 0, tm.TM_SINGLE, tm.TM_RECON_18, nf)
+        assert rel_l2(got, want) <= TOL[tm.TM_SINGLE]
 
 
 def test_t2b_periodic_time_and_wilson_limit():
