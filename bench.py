@@ -504,7 +504,8 @@ def run_ours(args, log):
     slab = None
     if args.sharded:
         from paper_1311_4462_b200 import sharded
-        slab = sharded.Slab((DIMS[0], DIMS[1], DIMS[2], DIMS[3] * world), rank, world, local)
+        grid = tuple(int(v) for v in args.grid.split(",")) if args.grid else (1, 1, world)
+        slab = sharded.Slab((DIMS[0], DIMS[1] * grid[0], DIMS[2] * grid[1], DIMS[3] * grid[2]), rank, world, local, grid=grid, peer=args.peer)
     w = Workload(local, log, slab)
     lat, vh = w.lat, w.vh
     tm.tm_set_path(lat.ctx, args.path)
@@ -619,7 +620,8 @@ def run_ours(args, log):
                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                "vs_baseline": None, "dtype": "f64+f32+i16/f32", "data": "synthetic",
                "config": {"workload": WORKLOAD % (RECON, RECON), "lattice": list(DIMS), "recon": RECON, "kappa": KAPPA,
-                          "parallelism": ("time-direction slabs of a 32^3 x %d lattice, one per GPU, face exchange per dslash (--sharded)" % (DIMS[3] * world))
+                          "parallelism": ("sub-lattices of 32^3 x 64 on a (y, z, t) process grid %s, one per GPU, face exchange per dslash through %s (--sharded)"
+                                          % (args.grid or "1,1,%d" % world, "peer-mapped buffers + flag words" if args.peer else "torch.distributed send / recv"))
                           if args.sharded else ("replicas only (north_star: no sharding)" if world > 1 else "single GPU"),
                           "l2": "inputs larger than L2 (gauge fields 201-805 MB each, 2.3 GB touched per step)"},
                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
@@ -650,6 +652,8 @@ def main():
     ap.add_argument("--sharded", action="store_true",
                     help="each rank holds a 32^3x64 slab of a 32^3 x (64 N) lattice: kernels with open time hops, face exchange over "
                          "torch.distributed, boundary completion (DESIGN.md section 9); default: N independent replicas")
+    ap.add_argument("--grid", default="", help="--sharded: process grid PY,PZ,PT over the y, z, t directions (default 1,1,N: time slabs)")
+    ap.add_argument("--peer", action="store_true", help="--sharded: faces through peer-mapped buffers and flag words (CUDA IPC) instead of NCCL send / recv")
     ap.add_argument("--recon", type=int, default=12, choices=[18, 12, 8],
                     help="reals stored per link (BASELINE.json configs[2], configs[3]: 12); 18 and 8 are the other rows of the paper's Table 1")
     args = ap.parse_args()

@@ -191,27 +191,47 @@ typedef struct {
     double residual;               /* last true relative residual |b - A x| / |b|                                      */
     int converged;                 /* 1 if residual <= tol                                                            */
 } tm_cg_info;
-/* ---- time-direction domain decomposition --------------------------------
- * One slab X x Y x Z x T_loc of the global lattice per context (per GPU), slabs stacked along x4 in rank order; T_loc even,
- * so local and global site parities agree.  One distributed dslash =
- *   tm_halo_pack(in)  ->  exchange the two face buffers with the neighbouring slabs (the caller's transport: NCCL
- *   send / recv, peer copies; paper_1311_4462_b200.sharded does it with torch.distributed)  ->  tm_dslash_apply with
- *   tm_set_open_time(ctx, 1) (the kernels give the time hops that leave the slab the weight 0)  ->  tm_halo_apply(out),
- * after which `out` equals the single-lattice result on this slab (tests/test_gpu_sharded.py against the oracle on the
- * global lattice).  The exchange can overlap the interior kernel; tm_halo_apply must follow both on the context stream.
- * Face buffers are DEVICE memory owned by the caller, tm_halo_bytes() each: [n_flavor][XYZ/2][12 reals] of double (fp64
- * fields) or float (fp32 and half fields); site j of a face = checkerboard index inside the time slice.
- *   dev_to_prev  : spin-projected half-spinors of the FIRST time slice, for the previous slab's forward hops
- *   dev_to_next  : U_4^dag times the projected half-spinors of the LAST time slice, for the next slab's backward hops
- *   dev_from_prev = the previous slab's dev_to_next, dev_from_next = the next slab's dev_to_prev
- *   sign_prev / sign_next : +1, or the time boundary condition (-1 antiperiodic) where that face is the global boundary
+/* ---- domain decomposition in y, z and t ---------------------------------
+ * One sub-lattice X x Y_loc x Z_loc x T_loc of the global lattice per context (per GPU), a process grid over the directions
+ * mu = 1 (y), 2 (z), 3 (t) in any combination; the local extents even, so local and global site parities agree.  x is never
+ * cut (the checkerboard index lives on it).  PAPER.md:72: the packing routines "take into account the fifth flavor dimension
+ * when gathering boundary-spinor sites in non-temporal lattice directions": a face of a non-temporal direction is a STRIDED
+ * set of sites of the tiled layout, gathered per flavor.  One distributed dslash =
+ *   for every cut direction: tm_halo_pack(in, dir)  ->  the two face buffers reach the neighbouring sub-lattices (either the
+ *   buffers ARE the neighbours' receive buffers, mapped with CUDA IPC / peer access, and the pack kernel's stores are the
+ *   transfer, signalled by the flags below; or the caller moves them: NCCL send / recv, paper_1311_4462_b200.sharded)
+ *   ->  tm_dslash_apply with tm_set_open_dirs(ctx, mask) (the kernels give the hops that leave the sub-lattice in a cut
+ *   direction the weight 0)  ->  for every cut direction: tm_halo_apply(out, dir),
+ * after which `out` equals the single-lattice result on this sub-lattice (tests/test_gpu_sharded.py against the oracle on
+ * the global lattice).  The exchange can overlap the interior kernel; tm_halo_apply follows both on the context stream.
+ * Face buffers are DEVICE memory owned by the caller, tm_halo_bytes(dir) each: [n_flavor][V_loc / (2 L_dir)][12 reals] of
+ * double (fp64 fields) or float (fp32 and half fields); site j of a face = checkerboard order of the face's sites
+ * (x fastest, then the uncut coordinates in increasing order), the same on both sides of the cut.
+ *   dev_to_prev  : spin-projected half-spinors ((1 -+ gamma_dir) psi, 12 reals per site AND FLAVOR) of the FIRST slice
+ *                  x_dir = 0, for the previous sub-lattice's forward hops
+ *   dev_to_next  : U_dir^dag times the projected half-spinors of the LAST slice, for the next one's backward hops (the link
+ *                  lives with the sender)
+ *   dev_from_prev = the previous sub-lattice's dev_to_next, dev_from_next = the next one's dev_to_prev
+ *   sign_prev / sign_next : +1, or for dir = 3 the time boundary condition (-1 antiperiodic) where that face is the global
+ *                  boundary (TM_ERR_ARG for -1 in a spatial direction: space is periodic)
+ *   flags (all may be NULL = no signalling): DEVICE pointers to 32-bit unsigned words.  tm_halo_pack stores `epoch` to
+ *   *dev_flag_prev and *dev_flag_next (system-scope release) after every face element has been written; tm_halo_apply
+ *   spins until *dev_wait_prev >= epoch and *dev_wait_next >= epoch (system-scope acquire) before it reads the faces.  With
+ *   peer-mapped receive buffers the sender's flag_prev / flag_next are words in the NEIGHBOURS' memory next to the buffers.
+ *   Epochs must increase by one per exchange and direction; two receive-buffer sets used alternately (epoch & 1) make the
+ *   scheme race-free for nearest-neighbour exchanges (paper_1311_4462_b200/sharded.py: PeerRing).
  * `out_parity`, `dagger`, `kt` are those of the tm_dslash_apply call being completed; every kernel type is supported
- * (the fused epilogues are affine in the hopping sum).                                                                */
+ * (the fused epilogues are affine in the hopping sum), and the directions' completions commute.
+ * tm_set_open_dirs: mask bit mu (1 << mu) for mu = 1, 2, 3; TM_ERR_ARG for other bits.  tm_set_open_time(ctx, on) =
+ * tm_set_open_dirs(ctx, on ? 8 : 0).                                                                                  */
+int tm_set_open_dirs(tm_ctx *ctx, int mask);
 int tm_set_open_time(tm_ctx *ctx, int on);
-size_t tm_halo_bytes(const tm_ctx *ctx, tm_precision prec, int n_flavor);
-int tm_halo_pack(const tm_field *in, const tm_gauge *g, tm_parity out_parity, int dagger, void *dev_to_prev, void *dev_to_next);
+size_t tm_halo_bytes(const tm_ctx *ctx, tm_precision prec, int n_flavor, int dir);
+int tm_halo_pack(const tm_field *in, const tm_gauge *g, tm_parity out_parity, int dagger, int dir, void *dev_to_prev, void *dev_to_next,
+                 unsigned *dev_flag_prev, unsigned *dev_flag_next, unsigned epoch);
 int tm_halo_apply(tm_field *out, const void *dev_from_prev, const void *dev_from_next, const tm_gauge *g, const tm_params *p,
-                  tm_parity out_parity, int dagger, tm_kernel_type kt, int sign_prev, int sign_next);
+                  tm_parity out_parity, int dagger, tm_kernel_type kt, int dir, int sign_prev, int sign_next,
+                  const unsigned *dev_wait_prev, const unsigned *dev_wait_next, unsigned epoch);
 
 /* Mixed-precision conjugate gradient on the normal equations of the even-odd preconditioned operator (the paper's
  * "double-single" / "double-half" CG, as defect correction): solves
@@ -240,7 +260,9 @@ int tm_set_path(tm_ctx *ctx, int path);
  *   "prefetch_blocks": L2 prefetch distance of the dslash kernels in thread blocks, 0 = off, -1 = library
  *   default (chosen per precision and flavor count);
  *   "stage_links": 1 = the 8 links of a site are copied to shared memory with cp.async before the hops, 0 = direct
- *   loads, -1 = library default;   "block_threads": 32 / 64 / 128 sites per thread block, 0 = library default.
+ *   loads, -1 = library default;   "block_threads": 32 / 64 / 128 sites per thread block, 0 = library default;
+ *   "z_chunks": the thread blocks walk the lattice in n chunks of Z / n z-planes (all time slices of a chunk first) so that
+ *   the input spinor's reuse window fits the L2; -1 = library default (from the size of three time slices).
  *   Unknown key or bad value -> TM_ERR_ARG. */
 int tm_set_tuning(tm_ctx *ctx, const char *key, int value);
 

@@ -33,7 +33,7 @@ EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
     "tm_field_device_ptr", "tm_set_host_basis", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb", "tm_field_upload_cb_async", "tm_field_download_cb_async",
     "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_twist_apply",
-    "tm_prepare_rhs", "tm_set_open_time", "tm_halo_bytes", "tm_halo_pack", "tm_halo_apply", "tm_field_axpby", "tm_field_redot", "tm_invert_cg", "tm_last_error",
+    "tm_prepare_rhs", "tm_set_open_time", "tm_set_open_dirs", "tm_halo_bytes", "tm_halo_pack", "tm_halo_apply", "tm_field_axpby", "tm_field_redot", "tm_invert_cg", "tm_last_error",
     "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_set_tuning", "tm_timing_enable", "tm_timing_read",
 ]
 
@@ -101,10 +101,11 @@ def lib():
     L.tm_twist_apply.argtypes = [vp, vp, pp, i, i]
     L.tm_prepare_rhs.argtypes = [vp, vp, vp, vp, vp, pp, i]
     L.tm_set_open_time.argtypes = [vp, i]
-    L.tm_halo_bytes.argtypes = [vp, i, i]
+    L.tm_set_open_dirs.argtypes = [vp, i]
+    L.tm_halo_bytes.argtypes = [vp, i, i, i]
     L.tm_halo_bytes.restype = ctypes.c_size_t
-    L.tm_halo_pack.argtypes = [vp, vp, i, i, vp, vp]
-    L.tm_halo_apply.argtypes = [vp, vp, vp, vp, pp, i, i, i, i, i]
+    L.tm_halo_pack.argtypes = [vp, vp, i, i, i, vp, vp, vp, vp, ctypes.c_uint]
+    L.tm_halo_apply.argtypes = [vp, vp, vp, vp, pp, i, i, i, i, i, i, vp, vp, ctypes.c_uint]
     L.tm_field_axpby.argtypes = [vp, d, vp, d, vp]
     L.tm_field_redot.argtypes = [vp, vp, ctypes.POINTER(d)]
     L.tm_invert_cg.argtypes = [vp, vp, vp, vp, pp, i, ctypes.POINTER(tm_cg_params), ctypes.POINTER(tm_cg_info)]
@@ -237,18 +238,24 @@ def tm_set_open_time(ctx, on):
     _check(lib().tm_set_open_time(ctx, int(on)))
 
 
-def tm_halo_bytes(ctx, prec, n_flavor):
-    return int(lib().tm_halo_bytes(ctx, int(prec), int(n_flavor)))
+def tm_set_open_dirs(ctx, mask):
+    _check(lib().tm_set_open_dirs(ctx, int(mask)))
 
 
-def tm_halo_pack(inp, gauge, out_parity, dagger, dev_to_prev, dev_to_next):
-    """dev_*: device addresses (int) of face buffers of tm_halo_bytes each."""
-    _check(lib().tm_halo_pack(inp, gauge, int(out_parity), int(dagger), ctypes.c_void_p(dev_to_prev), ctypes.c_void_p(dev_to_next)))
+def tm_halo_bytes(ctx, prec, n_flavor, direction=3):
+    return lib().tm_halo_bytes(ctx, int(prec), int(n_flavor), int(direction))
 
 
-def tm_halo_apply(out, dev_from_prev, dev_from_next, gauge, p, out_parity, dagger, kernel_type, sign_prev, sign_next):
+def tm_halo_pack(inp, gauge, out_parity, dagger, dev_to_prev, dev_to_next, direction=3, flag_prev=None, flag_next=None, epoch=0):
+    _check(lib().tm_halo_pack(inp, gauge, int(out_parity), int(dagger), int(direction), ctypes.c_void_p(dev_to_prev),
+                              ctypes.c_void_p(dev_to_next), ctypes.c_void_p(flag_prev), ctypes.c_void_p(flag_next), int(epoch)))
+
+
+def tm_halo_apply(out, dev_from_prev, dev_from_next, gauge, p, out_parity, dagger, kernel_type, sign_prev, sign_next, direction=3,
+                  wait_prev=None, wait_next=None, epoch=0):
     _check(lib().tm_halo_apply(out, ctypes.c_void_p(dev_from_prev), ctypes.c_void_p(dev_from_next), gauge, ctypes.byref(p),
-                               int(out_parity), int(dagger), int(kernel_type), int(sign_prev), int(sign_next)))
+                               int(out_parity), int(dagger), int(kernel_type), int(direction), int(sign_prev), int(sign_next),
+                               ctypes.c_void_p(wait_prev), ctypes.c_void_p(wait_next), int(epoch)))
 
 
 def tm_field_axpby(z, a, x, b, y):

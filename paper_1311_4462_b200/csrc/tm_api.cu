@@ -175,7 +175,8 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->up_staging = c->down_staging = nullptr;
     c->up_bytes = c->down_bytes = 0;
     c->async_ready = false;
-    c->open_time = 0;
+    c->open_mask = 0;
+    c->halo_counter = nullptr;
     c->timing = false;
     e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
     if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaDeviceGetAttribute"); }
@@ -219,6 +220,7 @@ void tm_finalize(tm_ctx *ctx)
     if (ctx->up_staging) cudaFree(ctx->up_staging);
     if (ctx->down_staging) cudaFree(ctx->down_staging);
     if (ctx->cgs) cudaFree(ctx->cgs);
+    if (ctx->halo_counter) cudaFree(ctx->halo_counter);
     if (ctx->cgs_host) cudaFreeHost(ctx->cgs_host);
     for (auto &t : ctx->timed) { cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
     delete ctx;
@@ -561,7 +563,9 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.parity = (int)parity;
     a.alpha = co.alpha; a.beta = co.beta; a.scale = co.scale;
     a.kappa = p->kappa; a.kappa2 = p->kappa * p->kappa;
-    a.tbound = c->open_time ? 0.0 : (double)p->t_boundary;      // open time: the wrapped hops come from tm_halo_apply
+    a.tbound = (c->open_mask & 8) ? 0.0 : (double)p->t_boundary;      // cut directions: the wrapped hops come from tm_halo_apply
+    a.wrap_y = (c->open_mask & 2) ? 0.f : 1.f;
+    a.wrap_z = (c->open_mask & 4) ? 0.f : 1.f;
     // measured defaults (profiles/): the fp64 doublet kernels with 12-real links gain from an L2 prefetch 8 tiles ahead, the half
     // kernels from staging the link stream through shared memory; everything else runs plain
     a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_DOUBLE && out->nf == 2 && g->recon == 12 ? 8 : 0);
@@ -665,28 +669,40 @@ int tm_prepare_rhs(tm_field *rhs_e, const tm_field *b_e, const tm_field *b_o, tm
     return tm_dslash_apply(rhs_e, tmp_o, b_e, g, p, TM_EVEN, 0, type == TM_MATPC_ASYM ? TM_DSLASH_AXPY : TM_RECONSTRUCT, prec);
 }
 
-// ---- time-direction domain decomposition -------------------------------------------------------
-int tm_set_open_time(tm_ctx *ctx, int on)
+// ---- domain decomposition in y, z, t ---------------------------------------------------------
+int tm_set_open_dirs(tm_ctx *ctx, int mask)
 {
-    if (!ctx) return fail(TM_ERR_ARG, "tm_set_open_time: NULL context");
-    ctx->open_time = on ? 1 : 0;
+    if (!ctx) return fail(TM_ERR_ARG, "tm_set_open_dirs: NULL context");
+    if (mask & ~14) return fail(TM_ERR_ARG, "tm_set_open_dirs: mask %d has bits other than 2 (y), 4 (z), 8 (t)", mask);
+    ctx->open_mask = mask;
     return TM_OK;
 }
 
-size_t tm_halo_bytes(const tm_ctx *ctx, tm_precision prec, int n_flavor)
+int tm_set_open_time(tm_ctx *ctx, int on) { return tm_set_open_dirs(ctx, on ? 8 : 0); }
+
+size_t tm_halo_bytes(const tm_ctx *ctx, tm_precision prec, int n_flavor, int dir)
 {
-    if (!ctx || !valid_prec(prec) || (n_flavor != 1 && n_flavor != 2)) return 0;
-    return (size_t)n_flavor * (size_t)(ctx->g.Vh / ctx->g.X[3]) * 12 * ((int)prec == TM_DOUBLE ? sizeof(double) : sizeof(float));
+    if (!ctx || !valid_prec(prec) || (n_flavor != 1 && n_flavor != 2) || dir < 1 || dir > 3) return 0;
+    return (size_t)n_flavor * (size_t)(ctx->g.Vh / ctx->g.X[dir]) * 12 * ((int)prec == TM_DOUBLE ? sizeof(double) : sizeof(float));
 }
 
-int tm_halo_pack(const tm_field *in, const tm_gauge *g, tm_parity out_parity, int dagger, void *dev_to_prev, void *dev_to_next)
+int tm_halo_pack(const tm_field *in, const tm_gauge *g, tm_parity out_parity, int dagger, int dir, void *dev_to_prev, void *dev_to_next,
+                 unsigned *dev_flag_prev, unsigned *dev_flag_next, unsigned epoch)
 {
     if (!in || !g || !dev_to_prev || !dev_to_next) return fail(TM_ERR_ARG, "tm_halo_pack: NULL argument");
     if (out_parity != TM_EVEN && out_parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)out_parity);
+    if (dir < 1 || dir > 3) return fail(TM_ERR_ARG, "tm_halo_pack: dir %d is not 1 (y), 2 (z) or 3 (t)", dir);
     tm_ctx *c = in->ctx;
     if (g->ctx != c) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
     if (g->prec != in->prec) return fail(TM_ERR_MISMATCH, "precision mismatch (field %d, gauge %d)", in->prec, g->prec);
-    cudaError_t e = tm_launch_halo_pack(in, g, (int)out_parity, dagger ? 1 : 0, dev_to_prev, dev_to_next, c->stream);
+    TM_USE_DEVICE(c);
+    if ((dev_flag_prev || dev_flag_next) && !c->halo_counter) {
+        cudaError_t e = cudaMalloc(&c->halo_counter, sizeof(unsigned));
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->halo_counter, 0, sizeof(unsigned), c->stream);
+        if (e != cudaSuccess) return cuda_fail(e, "halo counter");
+    }
+    cudaError_t e = tm_launch_halo_pack(in, g, (int)out_parity, dagger ? 1 : 0, dir, dev_to_prev, dev_to_next, dev_flag_prev, dev_flag_next,
+                                        epoch, c->halo_counter, c->stream);
     if (e != cudaSuccess) return cuda_fail(e, "halo_pack launch");
     c->launches++;
     c->last_kernel = "halo_pack";
@@ -694,15 +710,19 @@ int tm_halo_pack(const tm_field *in, const tm_gauge *g, tm_parity out_parity, in
 }
 
 int tm_halo_apply(tm_field *out, const void *dev_from_prev, const void *dev_from_next, const tm_gauge *g, const tm_params *p,
-                  tm_parity out_parity, int dagger, tm_kernel_type kt, int sign_prev, int sign_next)
+                  tm_parity out_parity, int dagger, tm_kernel_type kt, int dir, int sign_prev, int sign_next,
+                  const unsigned *dev_wait_prev, const unsigned *dev_wait_next, unsigned epoch)
 {
     if (!out || !dev_from_prev || !dev_from_next || !g || !p) return fail(TM_ERR_ARG, "tm_halo_apply: NULL argument");
     if (out_parity != TM_EVEN && out_parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)out_parity);
     if ((int)kt < 0 || (int)kt > 5) return fail(TM_ERR_ARG, "bad kernel type %d", (int)kt);
+    if (dir < 1 || dir > 3) return fail(TM_ERR_ARG, "tm_halo_apply: dir %d is not 1 (y), 2 (z) or 3 (t)", dir);
     if ((sign_prev != 1 && sign_prev != -1) || (sign_next != 1 && sign_next != -1)) return fail(TM_ERR_ARG, "boundary signs must be +1 or -1");
+    if (dir != 3 && (sign_prev != 1 || sign_next != 1)) return fail(TM_ERR_ARG, "space is periodic: boundary signs must be +1 for dir %d", dir);
     tm_ctx *c = out->ctx;
     if (g->ctx != c) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
     if (g->prec != out->prec) return fail(TM_ERR_MISMATCH, "precision mismatch (field %d, gauge %d)", out->prec, g->prec);
+    TM_USE_DEVICE(c);
     Coeffs co;
     int rc = make_coeffs(p, out->nf, dagger ? 1 : 0, (int)kt, &co);
     if (rc) return rc;
@@ -711,8 +731,10 @@ int tm_halo_apply(tm_field *out, const void *dev_from_prev, const void *dev_from
     const int kcode = kt == TM_DSLASH_XPAY ? (int)TM_DSLASH_TWIST_XPAY : kt == TM_DSLASH_AXPY ? (int)TM_RECONSTRUCT : (int)kt;
     const double k2 = p->kappa * p->kappa;
     const double coef = kcode == 0 ? 1.0 : kcode == 3 ? p->kappa : -k2;
-    cudaError_t e = tm_launch_halo_apply(out, dev_from_prev, dev_from_next, g, (int)out_parity, dagger ? 1 : 0, 2.0 * sign_prev, 2.0 * sign_next,
-                                         co.alpha, co.beta, co.scale, coef, kcode != 2, c->stream);
+    const double hopw = dir == 3 ? 2.0 : 1.0;                      // (1 -+ gamma_4) keeps half the spinor with weight 2
+    cudaError_t e = tm_launch_halo_apply(out, dev_from_prev, dev_from_next, g, (int)out_parity, dagger ? 1 : 0, dir, hopw * sign_prev,
+                                         hopw * sign_next, co.alpha, co.beta, co.scale, coef, kcode != 2, dev_wait_prev, dev_wait_next,
+                                         epoch, c->stream);
     if (e != cudaSuccess) return cuda_fail(e, "halo_apply launch");
     c->launches++;
     c->last_kernel = "halo_apply";

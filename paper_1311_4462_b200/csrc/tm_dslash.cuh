@@ -79,26 +79,27 @@ TM_DEV void reconstruct_acc(real *acc, const real *g, real w)
 #pragma unroll
         for (int i = 0; i < 12; i++) dst[i] += w * g[i];
     } else {
+        const real sw = (real)SGN * w;          // w = 1, or 0 for a hop that leaves a sub-lattice (tm_set_open_dirs)
 #pragma unroll
-        for (int i = 0; i < 12; i++) au[i] += g[i];
+        for (int i = 0; i < 12; i++) au[i] += w * g[i];
 #pragma unroll
         for (int c = 0; c < 3; c++) {
             const int a = 2 * c, b = 6 + 2 * c;
             if constexpr (MU == 0) {
-                al[a] -= SGN * g[b + 1];
-                al[a + 1] += SGN * g[b];
-                al[b] -= SGN * g[a + 1];
-                al[b + 1] += SGN * g[a];
+                al[a] -= sw * g[b + 1];
+                al[a + 1] += sw * g[b];
+                al[b] -= sw * g[a + 1];
+                al[b + 1] += sw * g[a];
             } else if constexpr (MU == 1) {
-                al[a] += SGN * g[b];
-                al[a + 1] += SGN * g[b + 1];
-                al[b] -= SGN * g[a];
-                al[b + 1] -= SGN * g[a + 1];
+                al[a] += sw * g[b];
+                al[a + 1] += sw * g[b + 1];
+                al[b] -= sw * g[a];
+                al[b + 1] -= sw * g[a + 1];
             } else {
-                al[a] -= SGN * g[a + 1];
-                al[a + 1] += SGN * g[a];
-                al[b] += SGN * g[b + 1];
-                al[b + 1] -= SGN * g[b];
+                al[a] -= sw * g[a + 1];
+                al[a + 1] += sw * g[a];
+                al[b] += sw * g[b + 1];
+                al[b + 1] -= sw * g[b];
             }
         }
     }
@@ -216,6 +217,9 @@ __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? TM_MINB_
     const int tm = (t == 0) ? site + (a.T - 1) * st : site - st;
     const real wtp = (real)2 * ((t == a.T - 1) ? (real)a.tbound : (real)1);
     const real wtm = (real)2 * ((t == 0) ? (real)a.tbound : (real)1);
+    // y / z hops that wrap: weight 1, or 0 when that direction is cut between GPUs (tm_halo.cu supplies the hop)
+    const real wyp = (y == a.Y - 1) ? (real)a.wrap_y : (real)1, wym = (y == 0) ? (real)a.wrap_y : (real)1;
+    const real wzp = (z == a.Z - 1) ? (real)a.wrap_z : (real)1, wzm = (z == 0) ? (real)a.wrap_z : (real)1;
 
     const int nbr[8] = {xp, xm, yp, ym, zp, zm, tp, tm};
     const char *in = static_cast<const char *>(a.in);
@@ -241,8 +245,8 @@ __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? TM_MINB_
                                         ((H) & 1) ? gb + link_site_off(PREC, RECON, nbr[(H)], (H) >> 1)             \
                                                   : lf + ((H) >> 1) * link_tile_bytes(PREC, RECON),                 \
                                         ((H) & 1) ? (nbr[(H)] & (TM_TILE - 1)) : lane, (W))
-    TM_HOP(0, (real)1); TM_HOP(1, (real)1); TM_HOP(2, (real)1); TM_HOP(3, (real)1);
-    TM_HOP(4, (real)1); TM_HOP(5, (real)1); TM_HOP(6, wtp); TM_HOP(7, wtm);
+    TM_HOP(0, (real)1); TM_HOP(1, (real)1); TM_HOP(2, wyp); TM_HOP(3, wym);
+    TM_HOP(4, wzp); TM_HOP(5, wzm); TM_HOP(6, wtp); TM_HOP(7, wtm);
 #undef TM_HOP
 
     // a7: fused local epilogue

@@ -327,7 +327,8 @@ struct HopPtrs {
 struct HopCtx {
     int site;
     int nbr[8];              // +x -x +y -y +z -z +t -t
-    float wt[2];             // weight of the +t / -t hop (2 x boundary sign)
+    float wt[2];             // weight of the +t / -t hop (2 x boundary sign; 0 when the hop leaves a sub-lattice cut in t)
+    float ws[4];             // weight of the +y -y +z -z hop (1; 0 when the hop leaves a sub-lattice cut in that direction)
 };
 
 TM_DEV void site_ctx(HopCtx &c, const DslashArgs &a, int site)
@@ -352,6 +353,10 @@ TM_DEV void site_ctx(HopCtx &c, const DslashArgs &a, int site)
     c.nbr[7] = (t == 0) ? site + (a.T - 1) * st : site - st;
     c.wt[0] = 2.f * ((t == a.T - 1) ? (float)a.tbound : 1.f);
     c.wt[1] = 2.f * ((t == 0) ? (float)a.tbound : 1.f);
+    c.ws[0] = (y == a.Y - 1) ? a.wrap_y : 1.f;
+    c.ws[1] = (y == 0) ? a.wrap_y : 1.f;
+    c.ws[2] = (z == a.Z - 1) ? a.wrap_z : 1.f;
+    c.ws[3] = (z == 0) ? a.wrap_z : 1.f;
 }
 
 // Pipeline slot H of a site: 0..7 = the hops in the order of HopCtx::nbr, 8 = the xpay input of the site, > 8 nothing.
@@ -389,7 +394,7 @@ TM_DEV void consume_hop(f2 *A, HopRaw<PREC, NF, RECON> &r, const HopCtx &c)
     }
     f2 W[9];
     raw_to_link<PREC, NF, RECON>(W, r);
-    const float w = (MU == 3) ? c.wt[H & 1] : 1.f;
+    const float w = (MU == 3) ? c.wt[H & 1] : (MU == 0) ? 1.f : c.ws[H - 2];
 #pragma unroll
     for (int f = 0; f < NF; f++) {
         f2 S[12], H6[6], G[6];

@@ -49,7 +49,8 @@ struct tm_ctx {
     void *up_staging, *down_staging;
     size_t up_bytes, down_bytes;
     bool async_ready;
-    int open_time;        // tm_set_open_time: the fused kernels drop the time hops that leave the slab (tm_halo.cu adds them)
+    int open_mask;        // tm_set_open_dirs: bit mu set = the fused kernels drop the mu hops that leave the sub-lattice (tm_halo.cu adds them)
+    unsigned *halo_counter;   // device word: blocks of the running halo_pack kernel that have finished (flag signalling)
     double *cgs;          // inner CG scalars on the device: [0], [1] |r|^2 (ping-pong), [2] <p, A p>
     double *cgs_host;     // pinned host ring the scalars are copied to: 2 x 3 doubles
     double *red;          // reduction scratch of tm_blas.cu: [0] result, [1..] per-block partial sums
@@ -114,7 +115,8 @@ struct DslashArgs {
     double scale;
     double kappa;        // REC
     double kappa2;       // A-xpay, B
-    double tbound;       // +-1, multiplies the time hop that wraps
+    double tbound;       // +-1 (0 when the time direction is decomposed), multiplies the time hop that wraps
+    float wrap_y, wrap_z;   // weight of the y / z hop that wraps: 1, or 0 when that direction is decomposed (tm_set_open_dirs)
     int block_threads;   // threads per block (= sites per block)
     int pf_dist;         // L2 prefetch distance in thread blocks (0 = off): block b prefetches the tile of block b + pf_dist
     // z-chunked traversal (tm_virtual_block): thread blocks walk the lattice chunk by chunk of Z / nzc z-planes, all time slices
@@ -175,10 +177,12 @@ cudaError_t tm_blas_redot_dev(const tm_field *x, const tm_field *y, double *out,
 cudaError_t tm_blas_cg_update_dev(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr,
                                   const double *anum, const double *aden, double *dev_rr);
 
-// surface kernels of the time-direction decomposition (tm_halo.cu)
-cudaError_t tm_launch_halo_pack(const tm_field *in, const tm_gauge *g, int out_parity, int dagger, void *to_prev, void *to_next, cudaStream_t s);
-cudaError_t tm_launch_halo_apply(tm_field *out, const void *from_prev, const void *from_next, const tm_gauge *g, int parity, int dagger,
-                                 double w_prev, double w_next, double alpha, double beta, double scale, double coef, int twist_on, cudaStream_t s);
+// surface kernels of the domain decomposition (tm_halo.cu); dir = 1 (y), 2 (z), 3 (t)
+cudaError_t tm_launch_halo_pack(const tm_field *in, const tm_gauge *g, int out_parity, int dagger, int dir, void *to_prev, void *to_next,
+                                unsigned *flag_prev, unsigned *flag_next, unsigned epoch, unsigned *counter, cudaStream_t s);
+cudaError_t tm_launch_halo_apply(tm_field *out, const void *from_prev, const void *from_next, const tm_gauge *g, int parity, int dagger, int dir,
+                                 double w_prev, double w_next, double alpha, double beta, double scale, double coef, int twist_on,
+                                 const unsigned *wait_prev, const unsigned *wait_next, unsigned epoch, cudaStream_t s);
 
 // pack / unpack (tm_pack.cu)
 // (both apply the context's host spin basis: S on the way in, S^dag on the way out)

@@ -1,4 +1,4 @@
-"""GPU parity of the time-direction decomposition (include/tm.h: tm_halo_pack / tm_halo_apply, tm_set_open_time) against the
+"""GPU parity of the domain decomposition in y, z, t (include/tm.h: tm_halo_pack / tm_halo_apply, tm_set_open_dirs) against the
 oracle on the GLOBAL lattice.  One GPU: the slabs of a `world`-way split are processed one after the other in this process
 (pack all, hand the face buffers over exactly as sharded.ring_exchange routes them, then interior kernel + completion per
 slab), so no kernel ever waits for another rank; the transport itself is covered by tests/test_sharded_host.py (gloo)."""
@@ -20,12 +20,12 @@ PRECS = [tm.TM_DOUBLE, tm.TM_SINGLE, tm.TM_HALF]
 
 
 class Split:
-    """`world` slabs of one global lattice on one GPU, each with its slice of the gauge field."""
+    """The sub-lattices of one global lattice on a (py, pz, pt) process grid, all on one GPU, each with its part of the gauge field."""
 
-    def __init__(self, dims, world, U):
+    def __init__(self, dims, world, U, grid=None):
         self.dims, self.world, self.U = dims, world, U
-        self.slabs = [sharded.Slab(dims, r, world) for r in range(world)]
-        self.sl = [sharded.slab_slice(dims, r, world) for r in range(world)]
+        self.slabs = [sharded.Slab(dims, r, world, grid=grid) for r in range(world)]
+        self.sl = [s.sites() for s in self.slabs]
         self._g = {}
 
     def gauge(self, r, prec, recon):
@@ -35,20 +35,22 @@ class Split:
         return self._g[key]
 
     def kernel(self, inp, x, p, parity, dagger, kt, prec, recon, nf):
-        W = self.world
         fin, fx, fout, faces = [], [], [], []
         for r, s in enumerate(self.slabs):
             fin.append(s.lat.field(prec, nf).upload(1 - parity, np.ascontiguousarray(inp[:, self.sl[r]])))
             fx.append(None if x is None else s.lat.field(prec, nf).upload(parity, np.ascontiguousarray(x[:, self.sl[r]])))
             fout.append(s.lat.field(prec, nf))
-            to_prev, to_next = s.pack(fin[r], self.gauge(r, prec, recon), parity, dagger)
-            faces.append((to_prev.clone(), to_next.clone()))
+            faces.append({})
+            for d in s.cut:
+                to_prev, to_next = s.pack(fin[r], self.gauge(r, prec, recon), parity, dagger, d)
+                faces[r][d] = (to_prev.clone(), to_next.clone())
         out = np.zeros_like(inp)
         for r, s in enumerate(self.slabs):
-            from_prev, from_next = faces[(r - 1) % W][1], faces[(r + 1) % W][0]       # = sharded.ring_exchange
             g = self.gauge(r, prec, recon)
             tm.dslash_apply(fout[r], fin[r], fx[r], g, p, parity, dagger, kt)
-            s.finish(fout[r], from_prev, from_next, g, p, parity, dagger, kt)
+            for d in s.cut:
+                prev, nxt = s.neighbors(d)
+                s.finish(fout[r], faces[prev][d][1], faces[nxt][d][0], g, p, parity, dagger, kt, d)      # = the exchange's routing
             s.lat.sync()
             out[:, self.sl[r]] = fout[r].download(parity)
         return out
@@ -57,10 +59,10 @@ class Split:
 _cache = {}
 
 
-def split_for(dims, world, kind, seed):
-    key = (dims, world, kind, seed)
+def split_for(dims, world, kind, seed, grid=None):
+    key = (dims, world, kind, seed, grid)
     if key not in _cache:
-        _cache[key] = Split(dims, world, si.gauge_field(dims, seed, kind))
+        _cache[key] = Split(dims, world, si.gauge_field(dims, seed, kind), grid)
     return _cache[key]
 
 
@@ -85,6 +87,58 @@ def test_h1_sharded_kernels_match_the_global_oracle(dims, world, kw):
             assert rel_l2(got, want) <= TOL[prec], (PREC_NAME[prec], world, parity, dagger, kt)
 
 
+@pytest.mark.parametrize("dims,grid", [((4, 4, 8, 8), (1, 2, 1)), ((4, 8, 4, 8), (2, 1, 1)), ((4, 4, 8, 8), (1, 2, 2)), ((6, 8, 8, 4), (2, 2, 1)),
+                                       ((4, 12, 4, 8), (3, 1, 2))],
+                         ids=["z2", "y2", "z2t2", "y2z2", "y3t2"])
+@pytest.mark.parametrize("kw", [dict(mu=0.3, epsilon=0.0, twist_flavor=-1), dict(mu=0.15, epsilon=0.19, twist_flavor=0)], ids=["deg-", "ndeg"])
+def test_h1b_spatial_and_mixed_splits_match_the_global_oracle(dims, grid, kw):
+    """Cuts in non-temporal directions (the face gather is strided and flavor-aware) and in two directions at once:
+    every kernel type, parity, dagger and precision against the oracle on the GLOBAL lattice, sub-lattices processed in turn."""
+    nf = 2 if kw["twist_flavor"] == 0 else 1
+    world = grid[0] * grid[1] * grid[2]
+    sp = split_for(dims, world, "haar", 31, grid)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    full_in, full_x = si.spinor_field(dims, nf, 32), si.spinor_field(dims, nf, 33)
+    for parity, dagger, kt in itertools.product((0, 1), (0, 1), (0, 1, 2, 3, 4, 5)):
+        inp = si.mask_parity(full_in, dims, 1 - parity)
+        x = si.mask_parity(full_x, dims, parity)
+        if kt < 4:
+            want = oracle.kernel(inp, x, sp.U, po, parity, dagger, kt)
+        else:
+            want = oracle.hop_xpay(inp, x, sp.U, po, parity, dagger, -KAPPA ** 2 if kt == 4 else KAPPA)
+        for prec in PRECS:
+            recon = tm.TM_RECON_12 if prec != tm.TM_DOUBLE else tm.TM_RECON_18
+            got = sp.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, prec, recon, nf)
+            assert rel_l2(got, want) <= TOL[prec], (PREC_NAME[prec], grid, parity, dagger, kt, rel_l2(got, want))
+
+
+@pytest.mark.parametrize("cut", [(3,), (2,), (1, 2, 3)], ids=["t", "z", "yzt"])
+def test_h5_peer_ring_flags_and_sym_dagger_world_1(cut):
+    """The peer-buffer transport (PeerRing: the pack kernel stores into the receiver's buffer and publishes the epoch, the
+    completion kernel waits on the flag word) with one rank, which is its own neighbour in every cut direction, so that both
+    kernels run through the flag code in stream order; and Slab.mat_pc for every operator including the exact SYM adjoint."""
+    dims = (4, 4, 4, 8)
+    U = si.gauge_field(dims, 34, "haar")
+    kw = dict(mu=0.15, epsilon=0.19, twist_flavor=0)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    psi_e = si.mask_parity(si.spinor_field(dims, 2, 35), dims, 0)
+    for peer in (True, False):
+        s = sharded.Slab(dims, 0, 1, cut=cut, peer=peer)
+        for prec in PRECS:
+            g = s.lat.gauge(U, prec, tm.TM_RECON_12)
+            fin, ftmp, fout = s.lat.field(prec, 2).upload(0, psi_e), s.lat.field(prec, 2), s.lat.field(prec, 2)
+            for rep in range(3):                  # epochs 1..: both buffer slots are used
+                for typ, dagger in ((tm.TM_MATPC_ASYM, 0), (tm.TM_MATPC_ASYM, 1), (tm.TM_MATPC_SYM, 0), (tm.TM_MATPC_SYM, 1)):
+                    s.mat_pc(fout, fin, ftmp, g, pg, typ, dagger)
+                    s.lat.sync()
+                    want = oracle.matpc_adjoint(psi_e, U, po, typ) if dagger else oracle.matpc(psi_e, U, po, typ, 0)
+                    assert rel_l2(fout.download(0), want) <= TOL[prec], (PREC_NAME[prec], peer, typ, dagger, rep)
+        if peer:
+            ring = s.ring(tm.TM_HALF, 2, cut[0])
+            assert ring.epoch == 3 * (2 + 2 + 2 + 2)          # two hopping terms per operator
+            assert int(ring.flag.max().item()) == ring.epoch
+
+
 def test_h2_sharded_mat_pc_world_1_and_8real():
     """Slab.mat_pc through ring_exchange itself (world = 1: the slab is its own neighbour) and 8-real links."""
     dims = (4, 4, 4, 8)
@@ -103,7 +157,8 @@ def test_h2_sharded_mat_pc_world_1_and_8real():
             assert rel_l2(fout.download(0), want) <= TOL[prec], (PREC_NAME[prec], typ, dagger)
 
 
-def test_h3_torchrun_script_world_1():
+@pytest.mark.parametrize("extra", [[], ["--peer"]], ids=["sendrecv", "peer"])
+def test_h3_torchrun_script_world_1(extra):
     """tests/run_sharded_torchrun.py (the multi-GPU check, NCCL) launched the way the driver launches bench.py, with one rank."""
     import os
     import socket
@@ -115,7 +170,7 @@ def test_h3_torchrun_script_world_1():
     port = s.getsockname()[1]
     s.close()
     r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "1", "--master-addr", "127.0.0.1",
-                        "--master-port", str(port), os.path.join(root, "tests", "run_sharded_torchrun.py")],
+                        "--master-port", str(port), os.path.join(root, "tests", "run_sharded_torchrun.py")] + extra,
                        capture_output=True, text=True, timeout=600, cwd=root)
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
     assert "sharded ok: world 1" in r.stdout
@@ -131,6 +186,8 @@ def test_h4_halo_api_sizes_and_error_paths():
     assert tm.tm_halo_bytes(ctx, tm.TM_SINGLE, 2) == 2 * vs2 * 12 * 4
     assert tm.tm_halo_bytes(ctx, tm.TM_HALF, 2) == 2 * vs2 * 12 * 4          # half fields travel as float
     assert tm.tm_halo_bytes(ctx, 3, 1) == 0 and tm.tm_halo_bytes(ctx, tm.TM_DOUBLE, 3) == 0
+    assert tm.tm_halo_bytes(ctx, tm.TM_DOUBLE, 1, 2) == (4 * 6 * 8 // 2) * 12 * 8 and tm.tm_halo_bytes(ctx, tm.TM_DOUBLE, 2, 1) == 2 * (4 * 4 * 8 // 2) * 12 * 8
+    assert tm.tm_halo_bytes(ctx, tm.TM_DOUBLE, 1, 0) == 0 and tm.tm_halo_bytes(ctx, tm.TM_DOUBLE, 1, 4) == 0       # x is never cut
     U = si.gauge_field(dims, 26, "haar")
     g64, g32 = lat.gauge(U, tm.TM_DOUBLE, tm.TM_RECON_12), lat.gauge(U, tm.TM_SINGLE, tm.TM_RECON_12)
     f = lat.field(tm.TM_DOUBLE, 1)
@@ -140,7 +197,10 @@ def test_h4_halo_api_sizes_and_error_paths():
                 lambda: tm.tm_halo_pack(f.h, g64.h, 2, 0, a.data_ptr(), b.data_ptr()),                      # parity
                 lambda: tm.tm_halo_pack(f.h, g64.h, 0, 0, 0, b.data_ptr()),                                 # NULL buffer
                 lambda: tm.tm_halo_apply(f.h, a.data_ptr(), b.data_ptr(), g64.h, p, 0, 0, 7, 1, 1),         # kernel type
-                lambda: tm.tm_halo_apply(f.h, a.data_ptr(), b.data_ptr(), g64.h, p, 0, 0, 0, 0, 1)):        # boundary sign
+                lambda: tm.tm_halo_apply(f.h, a.data_ptr(), b.data_ptr(), g64.h, p, 0, 0, 0, 0, 1),         # boundary sign
+                lambda: tm.tm_halo_apply(f.h, a.data_ptr(), b.data_ptr(), g64.h, p, 0, 0, 0, -1, 1, 2),     # antiperiodic in space
+                lambda: tm.tm_halo_pack(f.h, g64.h, 0, 0, a.data_ptr(), b.data_ptr(), 0),                   # direction x
+                lambda: tm.tm_set_open_dirs(ctx, 1)):                                                       # mask bit of x
         with pytest.raises(tm.TmError):
             bad()
     # open time hops off again: the context is an ordinary periodic / antiperiodic lattice
