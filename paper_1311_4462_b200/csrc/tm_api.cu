@@ -498,7 +498,12 @@ int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_r
     if (!valid_prec(prec)) return fail(TM_ERR_ARG, "bad precision %d", (int)prec);
     if (recon != TM_RECON_18 && recon != TM_RECON_12 && recon != TM_RECON_8) return fail(TM_ERR_ARG, "bad recon %d", (int)recon);
     if (recon == TM_RECON_8) {
-        // the 8-real chart divides by N = |U01|^2 + |U02|^2 (tm_layout.cuh: rebuild_from8); its error grows like eps / N
+        // The 8-real chart divides by N = |U01|^2 + |U02|^2 (tm_layout.cuh: rebuild_from8): a rounding / storage error eps of the
+        // stored reals comes back as eps / N in the rebuilt row 1.  eps: 1e-16 (fp64), ~5e-7 (fp32: the packed kernels rebuild with
+        // the fast sin / cos / rcp units), 3e-5 (half: int16 storage).  The bound keeps the worst single link's error below
+        // 1e-8 / 5e-2 / 3 (x its magnitude): links closer to the chart's singular point are refused, not silently degraded
+        // further.  (Haar links: P(N < d) = d^2, so 32^3 x 64 has ~0.3 links below 1e-4 and none below 1e-5 in expectation.)
+        const double nmin_ok = (int)prec == TM_DOUBLE ? 1e-8 : 1e-5;
         const size_t nl = (size_t)4 * ctx->g.V;
         double nmin = 1.0;
         for (size_t l = 0; l < nl; l++) {
@@ -506,8 +511,9 @@ int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_r
             const double N = u[2] * u[2] + u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
             if (N < nmin) nmin = N;
         }
-        if (!(nmin >= 1e-10))
-            return fail(TM_ERR_PARAM, "8-real links: a link has |U01|^2 + |U02|^2 = %.3g, at the chart's singular point (use 12- or 18-real)", nmin);
+        if (!(nmin >= nmin_ok))
+            return fail(TM_ERR_PARAM, "8-real links: a link has |U01|^2 + |U02|^2 = %.3g < %.0e, too close to the chart's singular point for "
+                                      "this precision (use 12- or 18-real)", nmin, nmin_ok);
     }
     TM_USE_DEVICE(ctx);
     tm_gauge *gg = new (std::nothrow) tm_gauge();

@@ -165,14 +165,24 @@ TM_DEV void rows01_from8_fast(f2 *W, const float *p)
 {
     const float a2r = p[0], a2i = p[1], a3r = p[2], a3i = p[3], b1r = p[4], b1i = p[5];
     const float N = fmaf(a2r, a2r, fmaf(a2i, a2i, fmaf(a3r, a3r, a3i * a3i)));
+#ifndef TM_RECON8_ACCURATE      /* IEEE sincospi / division: 20-30 % slower (profiles/r2_tuning.md), no faster than 12-real links */
     const float t1 = p[6] * 3.14159265358979f, t2 = p[7] * 3.14159265358979f;
     const float s1 = __sinf(t1), c1 = __cosf(t1), s2 = __sinf(t2), c2 = __cosf(t2);
+#else
+    float s1, c1, s2, c2;
+    sincospif(p[6], &s1, &c1);
+    sincospif(p[7], &s2, &c2);
+#endif
     const float q1 = fmaxf(1.f - N, 0.f), q2 = fmaxf(N - fmaf(b1r, b1r, b1i * b1i), 0.f);
     const float m1 = q1 * rsqrtf(fmaxf(q1, 1e-30f)), m2 = q2 * rsqrtf(fmaxf(q2, 1e-30f));
     const float a1r = m1 * c1, a1i = m1 * s1;
     const float r2r = m2 * c2, r2i = -(m2 * s2);                                        // conj(c1)
     const float r1r = -fmaf(a1r, b1r, a1i * b1i), r1i = fmaf(a1i, b1r, -(a1r * b1i));   // -conj(a1) b1
+#ifndef TM_RECON8_ACCURATE      /* IEEE sincospi / division: 20-30 % slower (profiles/r2_tuning.md), no faster than 12-real links */
     const float iN = __fdividef(1.f, N);
+#else
+    const float iN = 1.f / N;
+#endif
     W[0] = mk2(a1r, a1i);
     W[1] = mk2(a2r, a2i);
     W[2] = mk2(a3r, a3i);

@@ -290,6 +290,74 @@ def test_t2c_recon8_composites_and_singular_chart():
     with pytest.raises(tm.TmError) as ei:
         bench.lat.gauge(unit, tm.TM_DOUBLE, tm.TM_RECON_8)
     assert ei.value.status == tm.TM_ERR_PARAM
+    # near the singular point the rebuild's error grows like eps / N: the bound is per precision (tm_gauge_load).  A field with one
+    # link at N = |U01|^2 + |U02|^2 ~ 1e-6: fp64 takes it (and stays accurate SITE BY SITE, not only in the L2 norm), fp32 / half refuse
+    U = np.array(bench.U, copy=True)
+    c, s_ = np.cos(7e-4), np.sin(7e-4)
+    near = np.array([[c, s_ * 0.6, s_ * 0.8j], [-s_ * 0.6, c, 0], [s_ * 0.8j, 0, c]], dtype=np.complex128)
+    near, _ = np.linalg.qr(near)
+    near = near * (np.linalg.det(near) ** (-1.0 / 3.0))
+    near = near @ np.diag(np.exp(1j * np.array([0.3, -0.1, -0.2])))                 # generic phases, det = 1
+    U[2, 37] = near
+    n_near = float((np.abs(near[0, 1:]) ** 2).sum())
+    assert 1e-8 < n_near < 1e-5
+    for prec in (tm.TM_SINGLE, tm.TM_HALF):
+        with pytest.raises(tm.TmError) as ei:
+            bench.lat.gauge(U, prec, tm.TM_RECON_8)
+        assert ei.value.status == tm.TM_ERR_PARAM
+    g8 = bench.lat.gauge(U, tm.TM_DOUBLE, tm.TM_RECON_8)
+    fin, ftmp, fout = bench.lat.field(tm.TM_DOUBLE, 2).upload(0, psi_e), bench.lat.field(tm.TM_DOUBLE, 2), bench.lat.field(tm.TM_DOUBLE, 2)
+    tm.mat_pc(fout, fin, ftmp, g8, pg, tm.TM_MATPC_ASYM, 0)
+    bench.lat.sync()
+    got, want = fout.download(0), oracle.matpc(psi_e, U, po, oracle.ASYM, 0)
+    ev = si.parity_sites(dims, 0)
+    site_err = np.abs((got - want)[:, ev]).max(axis=(0, 2, 3)) / np.sqrt((np.abs(want[:, ev]) ** 2).sum(axis=(0, 2, 3)))
+    assert site_err.max() <= 1e-9, site_err.max()                                  # eps / N = 1e-16 / 1e-6, with margin
+
+
+# ---- T7: out-of-bounds stores and races, without compute-sanitizer (closed on this pool: profiles/r2_sanitizer.md) ------------
+
+@pytest.mark.parametrize("variant", VARIANTS, ids=[v[0] for v in VARIANTS])
+def test_t7_guard_bands_and_run_to_run_identity(variant):
+    """Every kernel type / precision / flavor count of every code path writes into an output field that sits between two 64 KB
+    guard bands of a canary pattern (external storage, tm_field_alloc); afterwards the bands are intact (no store outside the
+    field, ragged last tile included: 6^4 has 20.25 tiles per parity) and the field is bit-identical to a second and third run
+    (the staged kernels read shared memory without a block barrier: a race would show up as a difference between runs)."""
+    import torch
+    dims = (6, 6, 6, 6)
+    bench = bench_for(dims, "haar", 1)
+    lat = bench.lat
+    tm.tm_set_path(lat.ctx, variant[1])
+    for key, val in variant[2].items():
+        tm.tm_set_tuning(lat.ctx, key, val)
+    GUARD = 64 * 1024
+    for kw in (FLAVORS[0], FLAVORS[2]):
+        nf = nf_of(kw)
+        pg = tm.params(KAPPA, **kw)
+        inp, x = si.spinor_field(dims, nf, 2), si.spinor_field(dims, nf, 3)
+        for prec in PRECS:
+            nbytes = tm.tm_field_bytes(lat.ctx, prec, nf)
+            pad = (-nbytes) % 256
+            buf = torch.full((GUARD + nbytes + pad + GUARD,), 0xA5, dtype=torch.uint8, device="cuda")
+            assert buf.data_ptr() % 256 == 0
+            body = buf[GUARD:GUARD + nbytes]
+            h = tm.tm_field_alloc(lat.ctx, prec, nf, body.data_ptr(), nbytes)
+            try:
+                for recon in RECONS + [tm.TM_RECON_8]:
+                    g = bench.gauge(prec, recon)
+                    for parity, dagger, kt in ((0, 0, 0), (1, 1, 1), (0, 1, 2), (1, 0, 3), (0, 0, 4), (1, 1, 5)):
+                        fin = lat.field(prec, nf).upload(1 - parity, si.mask_parity(inp, dims, 1 - parity))
+                        fx = lat.field(prec, nf).upload(parity, si.mask_parity(x, dims, parity))
+                        runs = []
+                        for rep in range(3):
+                            body.fill_(0x5A)
+                            tm.tm_dslash_apply(h, fin.h, None if kt == 0 else fx.h, g.h, pg, parity, dagger, kt, prec)
+                            lat.sync()
+                            runs.append(body.clone())
+                        assert bool((buf[:GUARD] == 0xA5).all()) and bool((buf[GUARD + nbytes:] == 0xA5).all()), (prec, recon, kt)
+                        assert bool((runs[0] == runs[1]).all()) and bool((runs[0] == runs[2]).all()), (prec, recon, kt)
+            finally:
+                tm.tm_field_free(h)
 
 
 # ---- T3: composites; BASELINE.json config 1 -------------------------------------------------------

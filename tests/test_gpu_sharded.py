@@ -218,3 +218,31 @@ def test_h4_halo_api_sizes_and_error_paths():
     # with open time hops only the two boundary time slices differ from the closed lattice
     diff = np.abs(open_result - want).reshape(1, dims[3], -1).max(axis=2)[0]
     assert (diff[1:-1] < 1e-12).all() and diff[0] > 1e-3 and diff[-1] > 1e-3
+
+
+@pytest.mark.parametrize("dims,grid", [((4, 4, 4, 16), (1, 1, 2)), ((4, 4, 8, 8), (1, 2, 2))], ids=["t2", "z2t2"])
+def test_h6_sharded_half_tight_against_the_oracle_on_the_quantised_inputs(dims, grid):
+    """T2d on the sharded path: the oracle is fed the inputs as stored (int16 + norms), which leaves the fp32 arithmetic and the
+    output quantisation.  The completion kernel re-quantises the boundary sites (load, add the missing hops, store: a second
+    rounding of at most 1/2 LSB of the new site norm), so boundary components may be off by up to ~2.5 LSB instead of 1.75."""
+    from test_gpu_parity import _quantise_links, _quantise_spinor
+    world = grid[0] * grid[1] * grid[2]
+    sp = split_for(dims, world, "haar", 41, grid)
+    Uq = _quantise_links(sp.U)
+    kw = dict(mu=0.15, epsilon=0.19, twist_flavor=0)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    full_in, full_x = si.spinor_field(dims, 2, 42), si.spinor_field(dims, 2, 43)
+    worst_l2 = worst_lsb = 0.0
+    for parity, dagger, kt in itertools.product((0, 1), (0, 1), (0, 1, 2, 3)):
+        inp, x = si.mask_parity(full_in, dims, 1 - parity), si.mask_parity(full_x, dims, parity)
+        want = oracle.kernel(_quantise_spinor(inp), _quantise_spinor(x), Uq, po, parity, dagger, kt)
+        got = sp.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, tm.TM_HALF, tm.TM_RECON_18, 2)
+        err = rel_l2(got, want)
+        idx = si.parity_sites(dims, parity)
+        w = want[:, idx].view(np.float64).reshape(2, len(idx), 24)
+        g = got[:, idx].view(np.float64).reshape(2, len(idx), 24)
+        lsb = np.abs(g - w) / (np.abs(w).max(axis=2, keepdims=True) / 32767.0 + 1e-300)
+        worst_l2, worst_lsb = max(worst_l2, err), max(worst_lsb, float(lsb.max()))
+        assert err <= 6e-5, (parity, dagger, kt, err)
+        assert lsb.max() <= 2.75, (parity, dagger, kt, lsb.max())
+    print("sharded half, quantised inputs: worst rel L2 %.2e, worst component %.2f LSB" % (worst_l2, worst_lsb))

@@ -357,6 +357,18 @@ def test_p14_rhs_preparation_against_the_full_operator(kw):
     x = si.mask_parity(si.spinor_field(dims, nf, 73), dims, 0)
     got = oracle.hop_xpay(psi_o, x, U, p, 0, 0, -KAPPA * KAPPA)
     assert rel(got, x - KAPPA * KAPPA * si.mask_parity(oracle.dhop(psi_o, U, p), dims, 0)) < 1e-14
+    # ... and pinned through the full operator (P2, P5 pin `mat`), not through their own formula:  M = R - kappa D_hop, so
+    #   (M psi)_e = hop_xpay(psi_o, R psi_e; even, -kappa)   and, with b = M psi,   R psi_o = hop_xpay(psi_e, b_o; odd, +kappa)
+    r_e = oracle.twist(psi_e, p, 0, 0)
+    assert rel(oracle.hop_xpay(psi_o, r_e, U, p, 0, 0, -KAPPA), si.mask_parity(b, dims, 0)) < 1e-13
+    r_o = oracle.twist(psi_o, p, 0, 0)
+    assert rel(oracle.hop_xpay(psi_e, si.mask_parity(b, dims, 1), U, p, 1, 0, +KAPPA), r_o) < 1e-13
+    # the daggered form is the adjoint of the plain one between the two parities: <phi_e, D_eo psi_o> = <D^dag_oe phi_e, psi_o>
+    phi_e = si.mask_parity(si.spinor_field(dims, nf, 74), dims, 0)
+    zero = np.zeros_like(psi)
+    lhs = np.vdot(phi_e, oracle.hop_xpay(psi_o, zero, U, p, 0, 0, 1.0))
+    rhs_ = np.vdot(oracle.hop_xpay(phi_e, zero, U, p, 1, 1, 1.0), psi_o)
+    assert abs(lhs - rhs_) <= 1e-12 * abs(lhs)
 
 
 # ---- P7 / P8: special cases -----------------------------------------------------------------------
