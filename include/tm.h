@@ -65,7 +65,15 @@ typedef enum {                       /* the fused kernels of PAPER.md:68 (sectio
     TM_RECONSTRUCT = 3,              /* REC    : out_p = R^-1 (x_p + kappa D_hop in)     (Eq. 2.4)       */
     /* the same hopping kernels with no twist (R = 1): the pieces of M^_sym^dag and of the right-hand sides */
     TM_DSLASH_XPAY = 4,              /*          out_p = x_p - kappa^2 D_hop in                          */
-    TM_DSLASH_AXPY = 5               /*          out_p = x_p + kappa D_hop in                            */
+    TM_DSLASH_AXPY = 5,              /*          out_p = x_p + kappa D_hop in                            */
+    /* the fused "D R^-1" forms: the inverse twist is applied to the 8 neighbour INPUT sites in registers before the spin
+     * projection ("all local operators ... merged into dslash kernels"; the right-hand sides
+     * b_e + kappa D_eo R_oo^-1 b_o, and the exact adjoint of Eq. 2.3's operator).  gamma5 mixes the spin halves and tau1 the
+     * flavors, so these kernels read the whole neighbour site on the time hops too (one spinor of traffic more per site
+     * than kernel A, two fewer than a separate twist pass).                                                          */
+    TM_TWIST_INV_DSLASH_TWIST_INV = 6, /*        out_p = R^-1 D_hop R^-1 in                                */
+    TM_RECONSTRUCT_TWIST_INV = 7,    /*          out_p = R^-1 (x_p + kappa D_hop R^-1 in)                  */
+    TM_DSLASH_TWIST_INV_AXPY = 8     /*          out_p = x_p + kappa D_hop R^-1 in                         */
 } tm_kernel_type;
 /* dagger != 0: D_hop -> D_hop^dag (projectors swapped) and R -> R^dag (a -> -a), order kept.            */
 
@@ -148,9 +156,10 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
 /* LHS of Eq. 2.2 (ASYM: out_e = (R_ee - kappa^2 D_eo R_oo^-1 D_oe) in_e) or Eq. 2.3 (SYM:
  * out_e = (1 - kappa^2 R_ee^-1 D_eo R_oo^-1 D_oe) in_e): two launches, tmp_o is the odd
  * intermediate R_oo^-1 D_oe in_e.  dagger: the exact adjoint.  ASYM: the same two launches with the daggered
- * kernels.  SYM: M^_sym^dag = 1 - kappa^2 D^dag_eo R^dag^-1_oo D^dag_oe R^dag^-1_ee (C7) = the local twist
- * R^dag^-1 (into out_e, used as scratch: out_e must not alias in_e, TM_ERR_ALIAS), kernel A^dag, and the plain
- * xpay kernel: three launches.  Asynchronous. */
+ * kernels.  SYM: M^_sym^dag = 1 - kappa^2 D^dag_eo R^dag^-1_oo D^dag_oe R^dag^-1_ee (C7) = the fused
+ * TM_TWIST_INV_DSLASH_TWIST_INV^dag kernel (R^dag^-1 D^dag R^dag^-1) and the plain xpay kernel: two launches as well
+ * (half-precision doublets: the local twist into out_e first, three launches; out_e must not alias in_e, TM_ERR_ALIAS).
+ * Asynchronous. */
 int tm_mat_pc(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p,
               tm_matpc type, int dagger);
 
@@ -160,8 +169,10 @@ int tm_mat_pc(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_g
 int tm_twist_apply(tm_field *out, const tm_field *in, const tm_params *p, int inverse, int dagger);
 
 /* Right-hand side of Eq. 2.2 (ASYM: rhs_e = b_e + kappa D_eo R_oo^-1 b_o) or Eq. 2.3 (SYM: rhs_e = R_ee^-1 (b_e +
- * kappa D_eo R_oo^-1 b_o)), PAPER.md:60-64 in the reading C4 of DESIGN.md.  tmp_o receives R_oo^-1 b_o; it must not
- * alias b_e or rhs_e (TM_ERR_ALIAS); rhs_e may alias b_e.  Two launches.  Asynchronous. */
+ * kappa D_eo R_oo^-1 b_o)), PAPER.md:60-64 in the reading C4 of DESIGN.md.  One launch of the fused D R^-1 kernel
+ * (TM_DSLASH_TWIST_INV_AXPY / TM_RECONSTRUCT_TWIST_INV); half-precision doublets, whose kernels are bound by arithmetic,
+ * take the local twist into tmp_o and the plain kernel instead (two launches).  tmp_o is scratch: a valid field that does
+ * not alias b_e, b_o or rhs_e (TM_ERR_ALIAS); rhs_e may alias b_e.  Asynchronous. */
 int tm_prepare_rhs(tm_field *rhs_e, const tm_field *b_e, const tm_field *b_o, tm_field *tmp_o, const tm_gauge *g,
                    const tm_params *p, tm_matpc type);
 

@@ -213,6 +213,20 @@ def hop_xpay(inp, x, gauge, p, parity, dagger, coeff):
     return _mask(x, p, parity) + coeff * _mask(dhop(inp, gauge, p, dagger), p, parity)
 
 
+def kernel_twist_in(inp, x, gauge, p, parity, dagger, form):
+    """The fused "D R^-1" forms (the inverse twist acts on the INPUT field, then the hopping term):
+    form "A": R^-1 D_hop R^-1 in;  "REC": R^-1 (x + kappa D_hop R^-1 in);  "AXPY": x + kappa D_hop R^-1 in,
+    restricted to `parity`; dagger: R -> R^dag, D_hop -> D_hop^dag.  Compositions of twist, kernel and hop_xpay."""
+    t = twist(_mask(inp, p, 1 - parity), p, 1, dagger)
+    if form == "A":
+        return kernel(t, None, gauge, p, parity, dagger, A)
+    if form == "REC":
+        return kernel(t, x, gauge, p, parity, dagger, REC)
+    if form == "AXPY":
+        return hop_xpay(t, x, gauge, p, parity, dagger, p.kappa)
+    raise ValueError(form)
+
+
 def matpc_adjoint(inp, gauge, p, matpc_type):
     """The adjoint of the even-even operators written out from D_hop^dag and R^dag (C7):
     ASYM: (R_ee^dag - kappa^2 D_eo^dag R_oo^dag^-1 D_oe^dag) in_e

@@ -26,6 +26,7 @@ TM_RECON_18, TM_RECON_12, TM_RECON_8 = 18, 12, 8
 TM_EVEN, TM_ODD = 0, 1
 TM_TWIST_INV_DSLASH, TM_TWIST_INV_DSLASH_XPAY, TM_DSLASH_TWIST_XPAY, TM_RECONSTRUCT = 0, 1, 2, 3
 TM_DSLASH_XPAY, TM_DSLASH_AXPY = 4, 5
+TM_TWIST_INV_DSLASH_TWIST_INV, TM_RECONSTRUCT_TWIST_INV, TM_DSLASH_TWIST_INV_AXPY = 6, 7, 8
 TM_MATPC_ASYM, TM_MATPC_SYM = 0, 1
 TM_BASIS_NONREL, TM_BASIS_CHIRAL, TM_BASIS_CUSTOM = 0, 1, 2
 

@@ -18,6 +18,25 @@ const TmKernelEntry *tm_generic_table_4_2();
 const TmKernelEntry *tm_generic_table_2_1();
 const TmKernelEntry *tm_generic_table_2_2();
 
+const TmKernelEntry *tm_generic_twin_table_8_1();
+const TmKernelEntry *tm_generic_twin_table_8_2();
+const TmKernelEntry *tm_generic_twin_table_4_1();
+const TmKernelEntry *tm_generic_twin_table_4_2();
+const TmKernelEntry *tm_generic_twin_table_2_1();
+const TmKernelEntry *tm_generic_twin_table_2_2();
+const TmKernelEntry *tm_f2_twin_table_4_1();
+const TmKernelEntry *tm_f2_twin_table_4_2();
+const TmKernelEntry *tm_f2_twin_table_2_1();
+const TmKernelEntry *tm_f2_twin_table_2_2();
+
+// input-twist (D R^-1) kernels: packed for fp32 / half unless the scalar path is forced
+const TmKernelEntry *tm_twin_table(int prec, int nf, bool packed)
+{
+    if (prec == 8) return nf == 1 ? tm_generic_twin_table_8_1() : tm_generic_twin_table_8_2();
+    if (prec == 4) return packed ? (nf == 1 ? tm_f2_twin_table_4_1() : tm_f2_twin_table_4_2()) : (nf == 1 ? tm_generic_twin_table_4_1() : tm_generic_twin_table_4_2());
+    return packed ? (nf == 1 ? tm_f2_twin_table_2_1() : tm_f2_twin_table_2_2()) : (nf == 1 ? tm_generic_twin_table_2_1() : tm_generic_twin_table_2_2());
+}
+
 const TmKernelEntry *tm_generic_table(int prec, int nf)
 {
     if (prec == 8) return nf == 1 ? tm_generic_table_8_1() : tm_generic_table_8_2();
@@ -75,6 +94,11 @@ size_t field_bytes(const TmGeom &g, int prec, int nf)
     return (size_t)nf * tm_tiles(g.Vh) * spinor_tile_bytes(prec);      // tiled SoA, the last tile padded (tm_layout.cuh)
 }
 
+// The fused D R^-1 kernels (TWIN) replace a separate local pass (read + write of one field) by 8 register twists and full-site
+// time hops.  That pays wherever the kernel is bandwidth-bound; the half-precision doublet kernel is bound by the FP32 datapath
+// (profiles/r2_pipes.md) and runs 170 us fused against 111 + ~35 us in two launches at 32^3 x 64, so it keeps the local pass.
+bool fused_twist_in_pays(const tm_field *f) { return !(f->prec == TM_HALF && f->nf == 2); }
+
 bool overlap(const tm_field *a, const tm_field *b)
 {
     const char *pa = static_cast<const char *>(a->ptr), *pb = static_cast<const char *>(b->ptr);
@@ -118,7 +142,7 @@ int make_coeffs(const tm_params *p, int nf, int dagger, int kt, Coeffs *c)
     double a = 2.0 * p->kappa * p->mu, b = 2.0 * p->kappa * p->epsilon;
     if (dagger) a = -a;
     if (nf == 1) { a *= (double)p->twist_flavor; b = 0.0; }
-    if (kt == TM_DSLASH_XPAY || kt == TM_DSLASH_AXPY) {       // no twist: the B / REC kernels with R = 1
+    if (kt == TM_DSLASH_XPAY || kt == TM_DSLASH_AXPY || kt == TM_DSLASH_TWIST_INV_AXPY) {       // no (output) twist: the B / REC kernels with R = 1
         c->alpha = 0.0; c->beta = 0.0; c->scale = 1.0;
     } else if (kt == TM_DSLASH_TWIST_XPAY) {
         c->alpha = a; c->beta = b; c->scale = 1.0;
@@ -546,10 +570,13 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
 {
     if (!out || !in || !g || !p) return fail(TM_ERR_ARG, "tm_dslash_apply: NULL argument");
     if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
-    if ((int)kt < 0 || (int)kt > 5) return fail(TM_ERR_ARG, "bad kernel type %d", (int)kt);
-    // out = x - kappa^2 D in  and  out = x + kappa D in  run the B / REC kernels with the identity twist
-    const int kcode = kt == TM_DSLASH_XPAY ? (int)TM_DSLASH_TWIST_XPAY : kt == TM_DSLASH_AXPY ? (int)TM_RECONSTRUCT : (int)kt;
-    if (kt != TM_TWIST_INV_DSLASH && !x) return fail(TM_ERR_ARG, "kernel type %d needs x", (int)kt);
+    if ((int)kt < 0 || (int)kt > 8) return fail(TM_ERR_ARG, "bad kernel type %d", (int)kt);
+    // out = x - kappa^2 D in  and  out = x + kappa D in  run the B / REC kernels with the identity twist; the D R^-1 forms
+    // (kt 6, 7, 8) run the A / REC kernels with the inverse twist applied to the input sites (TWIN)
+    const bool twin = (int)kt >= (int)TM_TWIST_INV_DSLASH_TWIST_INV;
+    const int kcode = kt == TM_DSLASH_XPAY ? (int)TM_DSLASH_TWIST_XPAY : (kt == TM_DSLASH_AXPY || kt == TM_RECONSTRUCT_TWIST_INV || kt == TM_DSLASH_TWIST_INV_AXPY) ? (int)TM_RECONSTRUCT
+                      : kt == TM_TWIST_INV_DSLASH_TWIST_INV ? (int)TM_TWIST_INV_DSLASH : (int)kt;
+    if (kt != TM_TWIST_INV_DSLASH && kt != TM_TWIST_INV_DSLASH_TWIST_INV && !x) return fail(TM_ERR_ARG, "kernel type %d needs x", (int)kt);
     tm_ctx *c = out->ctx;
     if (in->ctx != c || g->ctx != c || (x && x->ctx != c)) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
     if (out->prec != (int)prec || in->prec != (int)prec || g->prec != (int)prec || (x && x->prec != (int)prec))
@@ -568,6 +595,13 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.dXh = tm_fastdiv(a.Xh); a.dY = tm_fastdiv(a.Y); a.dZ = tm_fastdiv(a.Z);
     a.parity = (int)parity;
     a.alpha = co.alpha; a.beta = co.beta; a.scale = co.scale;
+    a.alpha_in = 0.0; a.beta_in = 0.0; a.scale_in = 1.0;
+    if (twin) {
+        Coeffs ci;
+        rc = make_coeffs(p, out->nf, dagger ? 1 : 0, (int)TM_TWIST_INV_DSLASH, &ci);       // R^-1 (R^dag^-1 when daggered) on the input
+        if (rc) return rc;
+        a.alpha_in = ci.alpha; a.beta_in = ci.beta; a.scale_in = ci.scale;
+    }
     a.kappa = p->kappa; a.kappa2 = p->kappa * p->kappa;
     a.tbound = (c->open_mask & 8) ? 0.0 : (double)p->t_boundary;      // cut directions: the wrapped hops come from tm_halo_apply
     a.wrap_y = (c->open_mask & 2) ? 0.f : 1.f;
@@ -577,7 +611,7 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_DOUBLE && out->nf == 2 && g->recon == 12 ? 8 : 0);
     int stage = c->stage >= 0 ? c->stage : ((int)prec == TM_HALF ? 1 : 0);
     a.block_threads = c->block_threads ? c->block_threads : 128;
-    if (g->recon == 8) stage = 0;        // 8-real links: direct loads
+    if (g->recon == 8 || twin) stage = 0;        // 8-real links and the D R^-1 kernels: direct loads
     while (stage && (size_t)8 * g->recon * (int)prec * a.block_threads > 96 * 1024 && a.block_threads > 32) a.block_threads /= 2;
 
     // z-chunked traversal: the input spinor is re-read over a window of three time slices; when those (next to the streaming
@@ -596,11 +630,12 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     }
 
     // path 0: fp32 / half run the packed-FP32 kernels, fp64 the scalar kernel; path 1 forces the scalar kernel
-    // (8-real links: packed kernels exist for fp32 only; half takes the scalar kernel)
+    // (8-real links: packed kernels with direct loads only)
     const int kidx = (((g->recon == 18 ? 0 : g->recon == 12 ? 1 : 2) * 4 + kcode) * 2 + (dagger ? 1 : 0)) * 2 + stage;
     const TmKernelEntry *tab = (c->path == 0 && (int)prec != TM_DOUBLE) ? tm_f2_table((int)prec, out->nf) : nullptr;
     if (!tab || !tab[kidx].fn) tab = tm_generic_table((int)prec, out->nf);
-    const TmKernelEntry &k = tab[kidx];
+    const TmKernelEntry &k = twin ? tm_twin_table((int)prec, out->nf, c->path == 0)[((g->recon == 18 ? 0 : g->recon == 12 ? 1 : 2) * 2 + (kcode == 3 ? 1 : 0)) * 2 + (dagger ? 1 : 0)]
+                                  : tab[kidx];
     cudaError_t e;
     if (c->timing) {
         tm_ctx::TimedLaunch t;
@@ -628,12 +663,17 @@ int tm_mat_pc(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_g
     if (overlap(tmp_o, in_e) || overlap(tmp_o, out_e)) return fail(TM_ERR_ALIAS, "tmp_o aliases in_e or out_e");
     const tm_precision prec = (tm_precision)out_e->prec;
     if (type == TM_MATPC_SYM && dagger) {
-        // M^_sym^dag = 1 - kappa^2 D^dag_eo R^dag^-1_oo D^dag_oe R^dag^-1_ee  (C7): the twist stands in FRONT of
-        // the first hopping term, so it runs as the local kernel, with out_e as scratch.
-        if (overlap(out_e, in_e)) return fail(TM_ERR_ALIAS, "out_e aliases in_e (SYM dagger uses out_e as scratch)");
-        int rc = tm_twist_apply(out_e, in_e, p, 1, 1);                                             // out_e = R^dag^-1 in_e
-        if (!rc) rc = tm_dslash_apply(tmp_o, out_e, nullptr, g, p, TM_ODD, 1, TM_TWIST_INV_DSLASH, prec);   // tmp_o = R^dag^-1 D^dag out_e
-        if (!rc) rc = tm_dslash_apply(out_e, tmp_o, in_e, g, p, TM_EVEN, 1, TM_DSLASH_XPAY, prec);           // out_e = in_e - kappa^2 D^dag tmp_o
+        // M^_sym^dag = 1 - kappa^2 D^dag_eo R^dag^-1_oo D^dag_oe R^dag^-1_ee  (C7): the twist stands in FRONT of the first
+        // hopping term: the fused D R^-1 kernel applies it to the neighbour sites in registers.
+        if (overlap(out_e, in_e)) return fail(TM_ERR_ALIAS, "out_e aliases in_e");
+        int rc;
+        if (fused_twist_in_pays(out_e)) {
+            rc = tm_dslash_apply(tmp_o, in_e, nullptr, g, p, TM_ODD, 1, TM_TWIST_INV_DSLASH_TWIST_INV, prec);   // tmp_o = R^dag^-1 D^dag R^dag^-1 in_e
+        } else {
+            rc = tm_twist_apply(out_e, in_e, p, 1, 1);                                                           // out_e = R^dag^-1 in_e (scratch)
+            if (!rc) rc = tm_dslash_apply(tmp_o, out_e, nullptr, g, p, TM_ODD, 1, TM_TWIST_INV_DSLASH, prec);
+        }
+        if (!rc) rc = tm_dslash_apply(out_e, tmp_o, in_e, g, p, TM_EVEN, 1, TM_DSLASH_XPAY, prec);               // out_e = in_e - kappa^2 D^dag tmp_o
         return rc;
     }
     // tmp_o = R_oo^-1 D_oe in_e
@@ -669,10 +709,14 @@ int tm_prepare_rhs(tm_field *rhs_e, const tm_field *b_e, const tm_field *b_o, tm
     if (type != TM_MATPC_ASYM && type != TM_MATPC_SYM) return fail(TM_ERR_ARG, "bad matpc type %d", (int)type);
     if (overlap(tmp_o, b_e) || overlap(tmp_o, rhs_e) || overlap(tmp_o, b_o)) return fail(TM_ERR_ALIAS, "tmp_o aliases b_e, b_o or rhs_e");
     const tm_precision prec = (tm_precision)rhs_e->prec;
-    int rc = tm_twist_apply(tmp_o, b_o, p, 1, 0);                                     // tmp_o = R_oo^-1 b_o
-    if (rc) return rc;
-    // Eq. 2.2: b_e + kappa D_eo tmp_o ;  Eq. 2.3: R_ee^-1 (b_e + kappa D_eo tmp_o)   (reading C4)
-    return tm_dslash_apply(rhs_e, tmp_o, b_e, g, p, TM_EVEN, 0, type == TM_MATPC_ASYM ? TM_DSLASH_AXPY : TM_RECONSTRUCT, prec);
+    // Eq. 2.2: b_e + kappa D_eo R_oo^-1 b_o ;  Eq. 2.3: R_ee^-1 (b_e + kappa D_eo R_oo^-1 b_o)   (reading C4)
+    if (!fused_twist_in_pays(rhs_e)) {
+        int rc = tm_twist_apply(tmp_o, b_o, p, 1, 0);                                     // tmp_o = R_oo^-1 b_o
+        if (rc) return rc;
+        return tm_dslash_apply(rhs_e, tmp_o, b_e, g, p, TM_EVEN, 0, type == TM_MATPC_ASYM ? TM_DSLASH_AXPY : TM_RECONSTRUCT, prec);
+    }
+    // one launch of the fused D R^-1 kernel; tmp_o is not needed
+    return tm_dslash_apply(rhs_e, b_o, b_e, g, p, TM_EVEN, 0, type == TM_MATPC_ASYM ? TM_DSLASH_TWIST_INV_AXPY : TM_RECONSTRUCT_TWIST_INV, prec);
 }
 
 // ---- domain decomposition in y, z, t ---------------------------------------------------------
@@ -721,7 +765,7 @@ int tm_halo_apply(tm_field *out, const void *dev_from_prev, const void *dev_from
 {
     if (!out || !dev_from_prev || !dev_from_next || !g || !p) return fail(TM_ERR_ARG, "tm_halo_apply: NULL argument");
     if (out_parity != TM_EVEN && out_parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)out_parity);
-    if ((int)kt < 0 || (int)kt > 5) return fail(TM_ERR_ARG, "bad kernel type %d", (int)kt);
+    if ((int)kt < 0 || (int)kt > 5) return fail(TM_ERR_ARG, "bad kernel type %d (the D R^-1 forms have no distributed completion)", (int)kt);
     if (dir < 1 || dir > 3) return fail(TM_ERR_ARG, "tm_halo_apply: dir %d is not 1 (y), 2 (z) or 3 (t)", dir);
     if ((sign_prev != 1 && sign_prev != -1) || (sign_next != 1 && sign_next != -1)) return fail(TM_ERR_ARG, "boundary signs must be +1 or -1");
     if (dir != 3 && (sign_prev != 1 || sign_next != 1)) return fail(TM_ERR_ARG, "space is periodic: boundary signs must be +1 for dir %d", dir);

@@ -110,9 +110,13 @@ TM_DEV void reconstruct_acc(real *acc, const real *g, real w)
 // H = hop number (+x -x +y -y +z -z +t -t).  `lp` = site pointer of the link in global memory, `sp` = site pointer
 // of flavor 0 of the neighbour spinor, `lane` = neighbour index & 31.  STG: the link was staged in shared memory
 // (tm_stream.cuh) and 7 - H younger cp.async groups may still be pending.
-template <int PREC, int NF, int RECON, int H, bool DAG, bool STG>
+template <typename real> struct TwistIn { real alpha, beta, scale; };      // the twist applied to the INPUT sites (TWIN kernels)
+template <int NF, typename real>
+TM_DEV void twist(real *w, const real *v, const real *o, real alpha, real beta, real scale);
+
+template <int PREC, int NF, int RECON, int H, bool DAG, bool STG, bool TWIN = false>
 TM_DEV void hop(typename PrecTraits<PREC>::real *acc, const char *sp, int lane, const char *lp, int llane,
-                typename PrecTraits<PREC>::real w)
+                typename PrecTraits<PREC>::real w, TwistIn<typename PrecTraits<PREC>::real> ti = TwistIn<typename PrecTraits<PREC>::real>())
 {
     typedef typename PrecTraits<PREC>::real real;
     constexpr int MU = H / 2;
@@ -124,6 +128,28 @@ TM_DEV void hop(typename PrecTraits<PREC>::real *acc, const char *sp, int lane, 
         load_link<PREC, RECON, true>(u, stage_slot<PREC, RECON>(H), threadIdx.x & 31);
     } else {
         load_link<PREC, RECON, false>(u, lp, llane);
+    }
+    if constexpr (TWIN) {
+        // D R^-1: the neighbour spinor is twisted in registers before the projection.  gamma5 mixes the upper and lower spin
+        // halves and tau1 the flavors, so every hop (the time hops too) reads the whole neighbour site, all flavors.
+        real v[NF * 24], tv[NF * 24];
+#pragma unroll
+        for (int f = 0; f < NF; f++) load_spinor<PREC, 0>(v + 24 * f, sp + f * spinor_tile_bytes(PREC), lane);
+#pragma unroll
+        for (int f = 0; f < NF; f++) twist<NF>(tv + 24 * f, v + 24 * f, v + 24 * (NF - 1 - f), f == 0 ? ti.alpha : -ti.alpha, ti.beta, ti.scale);
+#pragma unroll
+        for (int f = 0; f < NF; f++) {
+            real h[12], g[12];
+            if constexpr (MU == 3) {
+#pragma unroll
+                for (int i = 0; i < 12; i++) h[i] = (SGN > 0) ? tv[24 * f + 12 + i] : tv[24 * f + i];
+            } else {
+                project<MU, SGN>(h, tv + 24 * f);
+            }
+            su3_mul<!FWD>(g, u, h);
+            reconstruct_acc<MU, SGN>(acc + 24 * f, g, w);
+        }
+        return;
     }
 #pragma unroll
     for (int f = 0; f < NF; f++) {
@@ -187,7 +213,7 @@ TM_DEV void epilogue(real *acc, const real *xv, real alpha, real beta, real scal
 #ifndef TM_MINB_8_1
 #define TM_MINB_8_1 3
 #endif
-template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, bool TWIN = false>
 __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? TM_MINB_8_1 : (PREC == 8 ? 2 : 1)) tm_dslash_generic(const DslashArgs a)
 {
     typedef typename PrecTraits<PREC>::real real;
@@ -240,11 +266,13 @@ __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? TM_MINB_
 #pragma unroll
     for (int i = 0; i < NF * 24; i++) acc[i] = 0;
 
+    TwistIn<real> ti;
+    ti.alpha = (real)a.alpha_in; ti.beta = (real)a.beta_in; ti.scale = (real)a.scale_in;
 #define TM_HOP(H, W)                                                                                              \
-    hop<PREC, NF, RECON, (H), DAG, STG>(acc, in + spinor_site_off(PREC, NF, nbr[(H)], 0), nbr[(H)] & (TM_TILE - 1),  \
+    hop<PREC, NF, RECON, (H), DAG, STG, TWIN>(acc, in + spinor_site_off(PREC, NF, nbr[(H)], 0), nbr[(H)] & (TM_TILE - 1),  \
                                         ((H) & 1) ? gb + link_site_off(PREC, RECON, nbr[(H)], (H) >> 1)             \
                                                   : lf + ((H) >> 1) * link_tile_bytes(PREC, RECON),                 \
-                                        ((H) & 1) ? (nbr[(H)] & (TM_TILE - 1)) : lane, (W))
+                                        ((H) & 1) ? (nbr[(H)] & (TM_TILE - 1)) : lane, (W), ti)
     TM_HOP(0, (real)1); TM_HOP(1, (real)1); TM_HOP(2, wyp); TM_HOP(3, wym);
     TM_HOP(4, wzp); TM_HOP(5, wzm); TM_HOP(6, wtp); TM_HOP(7, wtm);
 #undef TM_HOP
@@ -264,7 +292,7 @@ __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? TM_MINB_
     for (int f = 0; f < NF; f++) store_spinor<PREC>(acc + 24 * f, os + f * spinor_tile_bytes(PREC), lane);
 }
 
-template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, bool TWIN = false>
 cudaError_t tm_launch_generic(const DslashArgs &a, cudaStream_t s)
 {
     const int threads = a.block_threads;
@@ -272,10 +300,10 @@ cudaError_t tm_launch_generic(const DslashArgs &a, cudaStream_t s)
     const size_t smem = STG ? (size_t)8 * RECON * PREC * threads : 0;
     if (smem > 48 * 1024) {
         static std::atomic<unsigned long long> raised{0};      // per instantiation, one bit per device
-        cudaError_t e = tm_raise_smem(tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG>, raised);
+        cudaError_t e = tm_raise_smem(tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG, TWIN>, raised);
         if (e != cudaSuccess) return e;
     }
-    tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG><<<blocks, threads, smem, s>>>(a);
+    tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG, TWIN><<<blocks, threads, smem, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -290,7 +318,16 @@ cudaError_t tm_launch_generic(const DslashArgs &a, cudaStream_t s)
     {tm_launch_generic<P, N, R, K, false, true>, "generic_staged<" #P "," #N "," #R "," #K ",plain>"},     \
     {tm_launch_generic<P, N, R, K, true, false>, "generic<" #P "," #N "," #R "," #K ",dagger>"},           \
     {tm_launch_generic<P, N, R, K, true, true>, "generic_staged<" #P "," #N "," #R "," #K ",dagger>"}
+// input-twist (D R^-1) kernels, direct loads only: index [recon 18 / 12 / 8 -> 0 / 1 / 2][A, REC -> 0, 1][dagger 0..1]
+#define TM_GENERIC_TWIN_ROW(P, N, R)                                                                                 \
+    {tm_launch_generic<P, N, R, 0, false, false, true>, "generic_twin<" #P "," #N "," #R ",0,plain>"},              \
+    {tm_launch_generic<P, N, R, 0, true, false, true>, "generic_twin<" #P "," #N "," #R ",0,dagger>"},              \
+    {tm_launch_generic<P, N, R, 3, false, false, true>, "generic_twin<" #P "," #N "," #R ",3,plain>"},              \
+    {tm_launch_generic<P, N, R, 3, true, false, true>, "generic_twin<" #P "," #N "," #R ",3,dagger>"}
 #define TM_GENERIC_TABLE(P, N)                                                                        \
+    static const TmKernelEntry twin_table_##P##_##N[12] = {TM_GENERIC_TWIN_ROW(P, N, 18), TM_GENERIC_TWIN_ROW(P, N, 12),  \
+                                                           TM_GENERIC_TWIN_ROW(P, N, 8)};             \
+    const TmKernelEntry *tm_generic_twin_table_##P##_##N() { return twin_table_##P##_##N; }          \
     static const TmKernelEntry table_##P##_##N[48] = {                                               \
         TM_GENERIC_ROW(P, N, 18, 0), TM_GENERIC_ROW(P, N, 18, 1), TM_GENERIC_ROW(P, N, 18, 2),       \
         TM_GENERIC_ROW(P, N, 18, 3), TM_GENERIC_ROW(P, N, 12, 0), TM_GENERIC_ROW(P, N, 12, 1),       \

@@ -66,7 +66,7 @@ template <int PREC, int NF> __host__ __device__ constexpr int f2_pipeline_depth(
 // in flight costs 19 registers per flavor-site, in fp32 36 + 24 NF.
 template <int PREC, int NF, int RECON>
 struct HopRaw {
-    static constexpr int NL = (PREC == 4) ? (RECON == 18 ? 4 : RECON == 12 ? 3 : 2) : (RECON == 18 ? 2 : 1);   // 128-bit link words
+    static constexpr int NL = (PREC == 4) ? (RECON == 18 ? 4 : RECON == 12 ? 3 : 2) : (RECON == 18 ? 2 : 1);   // 128-bit link words (half 8-real: 1)
     static constexpr int NS = (PREC == 4) ? 6 : 3;                                          // 128-bit spinor words
     uint4 l[NL];
     uint2 lt;            // link tail: fp32/18 float2, half/12 int2, half/18 int (.x)
@@ -196,10 +196,16 @@ TM_DEV void rows01_from8_fast(f2 *W, const float *p)
 template <int PREC, int NF, int RECON>
 TM_DEV void raw_to_link(f2 *W, const HopRaw<PREC, NF, RECON> &r)
 {
-    if constexpr (RECON == 8) {
-        static_assert(PREC == 4, "packed kernels take 8-real links in fp32 only");
+    if constexpr (RECON == 8 && PREC == 4) {
         const float p[8] = {__uint_as_float(r.l[0].x), __uint_as_float(r.l[0].y), __uint_as_float(r.l[0].z), __uint_as_float(r.l[0].w),
                             __uint_as_float(r.l[1].x), __uint_as_float(r.l[1].y), __uint_as_float(r.l[1].z), __uint_as_float(r.l[1].w)};
+        rows01_from8_fast(W, p);
+    } else if constexpr (RECON == 8) {
+        // half: the 8 stored reals are one 128-bit word of int16 at scale 32767; the rebuilt rows come out at TRUE scale
+        // (consume_hop then folds only the spinor's 1 / 32767 into the weight)
+        const f2 a = mul2(cvt_pair(r.l[0].x), bc2(TM_INV15)), b = mul2(cvt_pair(r.l[0].y), bc2(TM_INV15));
+        const f2 c = mul2(cvt_pair(r.l[0].z), bc2(TM_INV15)), d = mul2(cvt_pair(r.l[0].w), bc2(TM_INV15));
+        const float p[8] = {a.x, a.y, b.x, b.y, c.x, c.y, d.x, d.y};
         rows01_from8_fast(W, p);
     } else if constexpr (PREC == 4) {
 #pragma unroll
@@ -371,14 +377,14 @@ TM_DEV void site_ctx(HopCtx &c, const DslashArgs &a, int site)
 
 // Pipeline slot H of a site: 0..7 = the hops in the order of HopCtx::nbr, 8 = the xpay input of the site, > 8 nothing.
 // One address computation per neighbour (spinor_site_off / link_site_off); every load then uses an immediate offset.
-template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, int H>
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, int H, bool TWIN = false>
 TM_DEV void issue_slot(HopRaw<PREC, NF, RECON> &r, const HopPtrs &p, const HopCtx &c)
 {
     if constexpr (H < 8) {
         constexpr int MU = H / 2;
         constexpr bool FWD = (H % 2) == 0;
         constexpr int SGN = (FWD != DAG) ? +1 : -1;
-        constexpr int PART = (MU == 3) ? ((SGN > 0) ? 2 : 1) : 0;
+        constexpr int PART = (MU == 3 && !TWIN) ? ((SGN > 0) ? 2 : 1) : 0;      // TWIN: the input twist needs the whole neighbour site
         const int n = c.nbr[H];
         if constexpr (!STG) {
             if constexpr (FWD) issue_link<PREC, NF, RECON, false>(r, p.gf + link_site_off(PREC, RECON, c.site, MU), c.site & (TM_TILE - 1));
@@ -390,14 +396,18 @@ TM_DEV void issue_slot(HopRaw<PREC, NF, RECON> &r, const HopPtrs &p, const HopCt
     }
 }
 
+template <int NF>
+TM_DEV void twist_f2(f2 *Wo, const f2 *V, const f2 *O, float alpha, float beta, float scale);
+struct TwistInF { float alpha, beta, scale; };      // the twist applied to the INPUT sites (TWIN kernels)
+
 // a6: the link is converted and rebuilt once and applied to every flavor.
-template <int PREC, int NF, int RECON, bool DAG, bool STG, int H>
-TM_DEV void consume_hop(f2 *A, HopRaw<PREC, NF, RECON> &r, const HopCtx &c)
+template <int PREC, int NF, int RECON, bool DAG, bool STG, int H, bool TWIN = false>
+TM_DEV void consume_hop(f2 *A, HopRaw<PREC, NF, RECON> &r, const HopCtx &c, TwistInF ti = TwistInF())
 {
     constexpr int MU = H / 2;
     constexpr bool FWD = (H % 2) == 0;
     constexpr int SGN = (FWD != DAG) ? +1 : -1;
-    constexpr int PART = (MU == 3) ? ((SGN > 0) ? 2 : 1) : 0;
+    constexpr int PART = (MU == 3 && !TWIN) ? ((SGN > 0) ? 2 : 1) : 0;
     if constexpr (STG) {
         cp_async_wait<7 - H>();
         issue_link<PREC, NF, RECON, true>(r, stage_slot<PREC, RECON>(H), threadIdx.x & 31);
@@ -405,10 +415,33 @@ TM_DEV void consume_hop(f2 *A, HopRaw<PREC, NF, RECON> &r, const HopCtx &c)
     f2 W[9];
     raw_to_link<PREC, NF, RECON>(W, r);
     const float w = (MU == 3) ? c.wt[H & 1] : (MU == 0) ? 1.f : c.ws[H - 2];
+    f2 T[TWIN ? NF * 12 : 1];
+    if constexpr (TWIN) {
+        // D R^-1: every flavor of the neighbour site at true scale (half: raw integers x norm / 32767), twisted in registers
+        f2 V[NF * 12];
+#pragma unroll
+        for (int f = 0; f < NF; f++) {
+            raw_to_spinor<PREC, 0>(V + 12 * f, r.s[f]);
+            if constexpr (PREC == 2) {
+                const float sc = r.n[f] * TM_INV15;
+#pragma unroll
+                for (int i = 0; i < 12; i++) V[12 * f + i] = mul2(V[12 * f + i], bc2(sc));
+            }
+        }
+#pragma unroll
+        for (int f = 0; f < NF; f++) twist_f2<NF>(T + 12 * f, V + 12 * f, V + 12 * (NF - 1 - f), f == 0 ? ti.alpha : -ti.alpha, ti.beta, ti.scale);
+    }
 #pragma unroll
     for (int f = 0; f < NF; f++) {
         f2 S[12], H6[6], G[6];
-        if constexpr (MU == 3) {
+        if constexpr (TWIN) {
+            if constexpr (MU == 3) {
+#pragma unroll
+                for (int i = 0; i < 6; i++) H6[i] = (SGN > 0) ? T[12 * f + 6 + i] : T[12 * f + i];
+            } else {
+                project_f2<MU, SGN>(H6, T + 12 * f);
+            }
+        } else if constexpr (MU == 3) {
             raw_to_spinor<PREC, PART>(S, r.s[f]);
 #pragma unroll
             for (int i = 0; i < 6; i++) H6[i] = (SGN > 0) ? S[6 + i] : S[i];
@@ -418,7 +451,8 @@ TM_DEV void consume_hop(f2 *A, HopRaw<PREC, NF, RECON> &r, const HopCtx &c)
         }
         float wf = w, wf2 = w;
         if constexpr (PREC == 2) {
-            wf *= r.n[f] * (TM_INV15 * TM_INV15);                        // site norm x link scale
+            // site norm x spinor scale (already applied when TWIN) x link scale (8-real links are rebuilt at true scale)
+            wf *= (TWIN ? 1.f : r.n[f] * TM_INV15) * (RECON == 8 ? 1.f : TM_INV15);
             wf2 = wf;
             if constexpr (RECON == 12) {                                 // row 2 of the link carries an extra 32767
                 if constexpr (FWD) wf2 = wf * TM_INV15;                  // U h: row 2 -> output color 2
@@ -514,7 +548,7 @@ TM_DEV void load_x(f2 *X, const HopRaw<PREC, NF, RECON> &rx)
 
 // One thread per output site, all flavors.  The 8 hops and the xpay input are 9 pipeline slots; slot h + PD is
 // issued before hop h is computed (PD = f2_pipeline_depth, PD + 1 rotating raw buffers).
-template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, bool TWIN = false>
 __global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(const DslashArgs a)
 {
     constexpr int PD = f2_pipeline_depth<PREC, NF>();
@@ -545,11 +579,13 @@ __global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(c
     for (int i = 0; i < NF * 12; i++) A[i] = mk2(0.f, 0.f);
 
     HopRaw<PREC, NF, RECON> buf[PD + 1];
-#define TM_ISSUE(S) issue_slot<PREC, NF, RECON, KT, DAG, STG, (S)>(buf[(S) % (PD + 1)], p, c)
+    TwistInF ti;
+    ti.alpha = (float)a.alpha_in; ti.beta = (float)a.beta_in; ti.scale = (float)a.scale_in;
+#define TM_ISSUE(S) issue_slot<PREC, NF, RECON, KT, DAG, STG, (S), TWIN>(buf[(S) % (PD + 1)], p, c)
 #define TM_STEP(H)                                                                  \
     do {                                                                            \
         TM_ISSUE((H) + PD);                                                         \
-        consume_hop<PREC, NF, RECON, DAG, STG, (H)>(A, buf[(H) % (PD + 1)], c);     \
+        consume_hop<PREC, NF, RECON, DAG, STG, (H), TWIN>(A, buf[(H) % (PD + 1)], c, ti);     \
     } while (0)
     if constexpr (PD >= 1) TM_ISSUE(0);
     if constexpr (PD >= 2) TM_ISSUE(1);
@@ -567,7 +603,7 @@ __global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(c
     for (int f = 0; f < NF; f++) store_spinor_f2<PREC>(A + 12 * f, os + f * spinor_tile_bytes(PREC), site & (TM_TILE - 1));
 }
 
-template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG>
+template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, bool TWIN = false>
 cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
 {
     const int threads = a.block_threads;
@@ -575,10 +611,10 @@ cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
     const size_t smem = STG ? (size_t)8 * RECON * PREC * threads : 0;
     if (smem > 48 * 1024) {
         static std::atomic<unsigned long long> raised{0};      // per instantiation, one bit per device
-        cudaError_t e = tm_raise_smem(tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG>, raised);
+        cudaError_t e = tm_raise_smem(tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG, TWIN>, raised);
         if (e != cudaSuccess) return e;
     }
-    tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG><<<blocks, threads, smem, s>>>(a);
+    tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG, TWIN><<<blocks, threads, smem, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -588,18 +624,24 @@ cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
     {tm_launch_f2<P, N, R, K, false, true>, "f2_staged<" #P "," #N "," #R "," #K ",plain>"},       \
     {tm_launch_f2<P, N, R, K, true, false>, "f2<" #P "," #N "," #R "," #K ",dagger>"},             \
     {tm_launch_f2<P, N, R, K, true, true>, "f2_staged<" #P "," #N "," #R "," #K ",dagger>"}
-// 8-real links: fp32 only, direct loads only (both staging slots hold the direct kernel); half has no entry (nullptr ->
-// tm_dslash_apply takes the scalar kernel)
-#define TM_F2_ROW8(N, K)                                                                           \
-    {tm_launch_f2<4, N, 8, K, false, false>, "f2<4," #N ",8," #K ",plain>"},                      \
-    {tm_launch_f2<4, N, 8, K, false, false>, "f2<4," #N ",8," #K ",plain>"},                      \
-    {tm_launch_f2<4, N, 8, K, true, false>, "f2<4," #N ",8," #K ",dagger>"},                      \
-    {tm_launch_f2<4, N, 8, K, true, false>, "f2<4," #N ",8," #K ",dagger>"}
-#define TM_F2_ROWS8_4(N) , TM_F2_ROW8(N, 0), TM_F2_ROW8(N, 1), TM_F2_ROW8(N, 2), TM_F2_ROW8(N, 3)
-#define TM_F2_ROWS8_2(N)
+// 8-real links: direct loads only (both staging slots hold the direct kernel)
+#define TM_F2_ROW8(P, N, K)                                                                        \
+    {tm_launch_f2<P, N, 8, K, false, false>, "f2<" #P "," #N ",8," #K ",plain>"},                 \
+    {tm_launch_f2<P, N, 8, K, false, false>, "f2<" #P "," #N ",8," #K ",plain>"},                 \
+    {tm_launch_f2<P, N, 8, K, true, false>, "f2<" #P "," #N ",8," #K ",dagger>"},                 \
+    {tm_launch_f2<P, N, 8, K, true, false>, "f2<" #P "," #N ",8," #K ",dagger>"}
+#define TM_F2_ROWS8(P, N) , TM_F2_ROW8(P, N, 0), TM_F2_ROW8(P, N, 1), TM_F2_ROW8(P, N, 2), TM_F2_ROW8(P, N, 3)
+// input-twist (D R^-1) kernels, direct loads only: index [recon 18 / 12 / 8 -> 0 / 1 / 2][A, REC -> 0, 1][dagger 0..1]
+#define TM_F2_TWIN_ROW(P, N, R)                                                                      \
+    {tm_launch_f2<P, N, R, 0, false, false, true>, "f2_twin<" #P "," #N "," #R ",0,plain>"},        \
+    {tm_launch_f2<P, N, R, 0, true, false, true>, "f2_twin<" #P "," #N "," #R ",0,dagger>"},        \
+    {tm_launch_f2<P, N, R, 3, false, false, true>, "f2_twin<" #P "," #N "," #R ",3,plain>"},        \
+    {tm_launch_f2<P, N, R, 3, true, false, true>, "f2_twin<" #P "," #N "," #R ",3,dagger>"}
 #define TM_F2_TABLE(P, N)                                                                    \
+    static const TmKernelEntry f2twin_##P##_##N[12] = {TM_F2_TWIN_ROW(P, N, 18), TM_F2_TWIN_ROW(P, N, 12), TM_F2_TWIN_ROW(P, N, 8)};   \
+    const TmKernelEntry *tm_f2_twin_table_##P##_##N() { return f2twin_##P##_##N; }          \
     static const TmKernelEntry f2table_##P##_##N[48] = {                                    \
         TM_F2_ROW(P, N, 18, 0), TM_F2_ROW(P, N, 18, 1), TM_F2_ROW(P, N, 18, 2),             \
         TM_F2_ROW(P, N, 18, 3), TM_F2_ROW(P, N, 12, 0), TM_F2_ROW(P, N, 12, 1),             \
-        TM_F2_ROW(P, N, 12, 2), TM_F2_ROW(P, N, 12, 3) TM_F2_ROWS8_##P(N)};                 \
+        TM_F2_ROW(P, N, 12, 2), TM_F2_ROW(P, N, 12, 3) TM_F2_ROWS8(P, N)};                 \
     const TmKernelEntry *tm_f2_table_##P##_##N() { return f2table_##P##_##N; }

@@ -113,6 +113,7 @@ struct DslashArgs {
     double alpha;        // local twist, flavor 0:  w = scale * (v + i alpha gamma5 v + beta v_otherflavor)
     double beta;
     double scale;
+    double alpha_in, beta_in, scale_in;   // TWIN kernels: the twist applied to the input sites (same form as alpha / beta / scale)
     double kappa;        // REC
     double kappa2;       // A-xpay, B
     double tbound;       // +-1 (0 when the time direction is decomposed), multiplies the time hop that wraps

@@ -455,6 +455,30 @@ def test_t3d_plain_xpay_axpy_kernels_match_oracle(kw):
                 assert rel_l2(got, want) <= TOL[prec], (PREC_NAME[prec], recon, parity, dagger, kt)
 
 
+@pytest.mark.parametrize("dims,kind", [((4, 4, 4, 8), "haar"), ((4, 6, 8, 10), "near_identity"), ((6, 6, 6, 6), "haar")])
+@pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
+@pytest.mark.parametrize("path", [0, 1], ids=["packed", "scalar"])
+def test_t3g_fused_dslash_twist_inv_kernels_match_oracle(dims, kind, kw, path):
+    """The fused D R^-1 kernel types (TM_TWIST_INV_DSLASH_TWIST_INV, TM_RECONSTRUCT_TWIST_INV, TM_DSLASH_TWIST_INV_AXPY: the inverse
+    twist applied to the neighbour sites in registers) against oracle.kernel_twist_in: every parity, dagger,
+    precision and link compression; the time hops of these kernels read the whole neighbour site."""
+    nf = nf_of(kw)
+    bench = bench_for(dims, kind, 1)
+    tm.tm_set_path(bench.lat.ctx, path)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    full_in, full_x = si.spinor_field(dims, nf, 18), si.spinor_field(dims, nf, 19)
+    for parity, dagger, (kt, form) in itertools.product((0, 1), (0, 1), ((tm.TM_TWIST_INV_DSLASH_TWIST_INV, "A"),
+                                                                        (tm.TM_RECONSTRUCT_TWIST_INV, "REC"), (tm.TM_DSLASH_TWIST_INV_AXPY, "AXPY"))):
+        inp, x = si.mask_parity(full_in, dims, 1 - parity), si.mask_parity(full_x, dims, parity)
+        want = oracle.kernel_twist_in(inp, x, bench.U, po, parity, dagger, form)
+        for prec, recon in itertools.product(PRECS, RECONS + [tm.TM_RECON_8]):
+            got = bench.kernel(inp, None if form == "A" else x, pg, parity, dagger, kt, prec, recon, nf)
+            assert "twin" in tm.tm_last_kernel_name(bench.lat.ctx)
+            err = rel_l2(got, want)
+            assert err <= TOL[prec], (PREC_NAME[prec], recon, parity, dagger, form, err)
+            assert np.abs(si.mask_parity(got, dims, 1 - parity)).max() == 0
+
+
 @pytest.mark.parametrize("kw", FLAVORS, ids=["deg+", "deg-", "ndeg"])
 def test_t3e_sym_dagger_is_the_adjoint_and_rhs_preparation(kw):
     dims = (4, 4, 4, 8)
@@ -471,6 +495,22 @@ def test_t3e_sym_dagger_is_the_adjoint_and_rhs_preparation(kw):
             assert rel_l2(bench.prepare_rhs(b, pg, typ, prec, recon, nf), want) <= TOL[prec], (PREC_NAME[prec], recon, typ)
         assert rel_l2(bench.prepare_rhs(b, pg, tm.TM_MATPC_SYM, prec, recon, nf, alias=True),
                       oracle.prepare_rhs(b, bench.U, po, tm.TM_MATPC_SYM)) <= TOL[prec]
+    # the normal operator M^_sym^dag M^_sym is four launches (the adjoint's leading twist is fused into the D R^-1 kernel) -- five for
+    # the half-precision doublet, which keeps the local pass -- and the right-hand side of Eq. 2.2 / 2.3 one launch (two)
+    lat = bench.lat
+    for prec in PRECS:
+        g = bench.gauge(prec, tm.TM_RECON_12)
+        f = [lat.field(prec, nf) for _ in range(4)]
+        f[0].upload(0, phi)
+        n0 = lat.launches()
+        tm.mat_pc(f[1], f[0], f[2], g, pg, tm.TM_MATPC_SYM, 0)
+        tm.mat_pc(f[3], f[1], f[2], g, pg, tm.TM_MATPC_SYM, 1)
+        extra = 1 if (prec == tm.TM_HALF and nf == 2) else 0
+        assert lat.launches() - n0 == 4 + extra
+        n0 = lat.launches()
+        tm.prepare_rhs(f[3], f[0], f[1], f[2], g, pg, tm.TM_MATPC_SYM)
+        assert lat.launches() - n0 == 1 + extra
+    lat.sync()
 
 
 def test_t3f_full_solve_pipeline_on_gpu():
@@ -631,7 +671,8 @@ def test_t6_error_paths():
     assert status(lambda: tm.twist_apply(t2, t3, sing, 1, 0)) == tm.TM_ERR_PARAM
     assert status(lambda: tm.twist_apply(a, t3, p, 0, 0)) == tm.TM_ERR_MISMATCH
     assert status(lambda: tm.dslash_apply(a, b, None, g, p, 0, 0, tm.TM_DSLASH_XPAY)) == tm.TM_ERR_ARG   # needs x
-    assert status(lambda: tm.dslash_apply(a, b, c, g, p, 0, 0, 6)) == tm.TM_ERR_ARG
+    assert status(lambda: tm.dslash_apply(a, b, c, g, p, 0, 0, 9)) == tm.TM_ERR_ARG
+    assert status(lambda: tm.dslash_apply(a, b, None, g, p, 0, 0, tm.TM_RECONSTRUCT_TWIST_INV)) == tm.TM_ERR_ARG   # needs x
     assert status(lambda: tm.prepare_rhs(a, b, c, b, g, p, tm.TM_MATPC_ASYM)) == tm.TM_ERR_ALIAS
     assert status(lambda: tm.mat_pc(a, b, b, g, p, tm.TM_MATPC_ASYM, 0)) == tm.TM_ERR_ALIAS
     assert status(lambda: tm.tm_init((4, 4, 4, 7))) == tm.TM_ERR_DIMS

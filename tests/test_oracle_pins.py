@@ -363,6 +363,14 @@ def test_p14_rhs_preparation_against_the_full_operator(kw):
     assert rel(oracle.hop_xpay(psi_o, r_e, U, p, 0, 0, -KAPPA), si.mask_parity(b, dims, 0)) < 1e-13
     r_o = oracle.twist(psi_o, p, 0, 0)
     assert rel(oracle.hop_xpay(psi_e, si.mask_parity(b, dims, 1), U, p, 1, 0, +KAPPA), r_o) < 1e-13
+    # the fused D R^-1 forms are pinned the same way: Eq. 2.2 / 2.3 right-hand sides (P14's prepare_rhs, tied to b = M psi above)
+    # and the first stage of the exact SYM adjoint (P13's matpc_adjoint)
+    be, bo = si.mask_parity(b, dims, 0), si.mask_parity(b, dims, 1)
+    assert rel(oracle.kernel_twist_in(bo, be, U, p, 0, 0, "AXPY"), oracle.prepare_rhs(b, U, p, oracle.ASYM)) < 1e-13
+    assert rel(oracle.kernel_twist_in(bo, be, U, p, 0, 0, "REC"), oracle.prepare_rhs(b, U, p, oracle.SYM)) < 1e-13
+    assert rel(oracle.kernel_twist_in(bo, be, U, p, 0, 0, "AXPY"), oracle.matpc(psi_e, U, p, oracle.ASYM)) < 1e-12
+    t_o = oracle.kernel_twist_in(psi_e, None, U, p, 1, 1, "A")
+    assert rel(oracle.hop_xpay(t_o, psi_e, U, p, 0, 1, -KAPPA * KAPPA), oracle.matpc_adjoint(psi_e, U, p, oracle.SYM)) < 1e-13
     # the daggered form is the adjoint of the plain one between the two parities: <phi_e, D_eo psi_o> = <D^dag_oe phi_e, psi_o>
     phi_e = si.mask_parity(si.spinor_field(dims, nf, 74), dims, 0)
     zero = np.zeros_like(psi)
