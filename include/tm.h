@@ -189,16 +189,31 @@ int tm_field_axpby(tm_field *z, double a, const tm_field *x, double b, const tm_
  * a fixed order (deterministic).  x = y gives |x|^2.  Synchronises the context stream. */
 int tm_field_redot(const tm_field *x, const tm_field *y, double *result);
 
+/* Multi-GPU reductions: after tm_set_allreduce(ctx, fn, user) every sum the library forms (tm_field_redot, the scalars of
+ * tm_invert_cg) is passed through fn(dev_sums, n, cuda_stream, user): dev_sums is a DEVICE array of n doubles holding this
+ * rank's partial sums; fn must replace them by the sums over all ranks, ordered on `cuda_stream` (e.g. ncclAllReduce, or
+ * torch.distributed.all_reduce on a tensor that aliases the memory), and return 0.  fn = NULL: single GPU (default). */
+typedef int (*tm_allreduce_fn)(double *dev_sums, int n, void *cuda_stream, void *user);
+int tm_set_allreduce(tm_ctx *ctx, tm_allreduce_fn fn, void *user);
+
+/* The operator of the solver: by default tm_mat_pc on the context's lattice.  A distributed caller supplies its own
+ * application of M (dagger = 0) / M^dag (dagger = 1) with the face exchange inside (paper_1311_4462_b200.sharded.Slab.mat_pc);
+ * it must enqueue on the context stream and return 0. */
+typedef int (*tm_cg_op_fn)(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p,
+                           tm_matpc type, int dagger, void *user);
 typedef struct {
     double tol;                    /* stop when |b - A x| / |b| <= tol, the residual formed in double                 */
-    int max_iter;                  /* cap on the total number of inner CG iterations                                  */
-    tm_precision sloppy_precision; /* precision of the inner CG (TM_DOUBLE: plain double CG)                          */
-    double delta;                  /* each inner solve reduces its residual by this factor before the next double
-                                      precision residual (0 < delta < 1; e.g. 0.1 for single, 0.3 for half)          */
+    int max_iter;                  /* cap on the number of CG iterations                                              */
+    tm_precision sloppy_precision; /* precision of the CG iteration (TM_DOUBLE: plain double CG)                      */
+    double delta;                  /* reliable update (true residual in double, solution accumulated in double) whenever
+                                      the iterated residual has dropped by this factor since the last one
+                                      (0 < delta < 1; e.g. 0.1 for single, 0.3 for half)                               */
+    tm_cg_op_fn op;                /* NULL: tm_mat_pc                                                                  */
+    void *op_user;
 } tm_cg_params;
 typedef struct {
-    int iterations;                /* inner CG iterations (applications of A = M^dag M in the sloppy precision)       */
-    int restarts;                  /* double-precision residual computations                                           */
+    int iterations;                /* CG iterations (applications of A = M^dag M in the sloppy precision)             */
+    int restarts;                  /* reliable updates (double-precision residual computations)                        */
     double residual;               /* last true relative residual |b - A x| / |b|                                      */
     int converged;                 /* 1 if residual <= tol                                                            */
 } tm_cg_info;
@@ -245,14 +260,19 @@ int tm_halo_apply(tm_field *out, const void *dev_from_prev, const void *dev_from
                   const unsigned *dev_wait_prev, const unsigned *dev_wait_next, unsigned epoch);
 
 /* Mixed-precision conjugate gradient on the normal equations of the even-odd preconditioned operator (the paper's
- * "double-single" / "double-half" CG, as defect correction): solves
+ * "double-single" / "double-half" CG) with RELIABLE UPDATES: solves
  *     M^dag M x_e = b_e ,   M = the LHS of Eq. 2.2 (ASYM) or Eq. 2.3 (SYM),
- * starting from x_e = 0 (the content of x_e on entry is ignored).  x_e, b_e and g_precise are double; g_sloppy is the
- * same gauge field loaded in sloppy_precision (ignored, may be NULL, when that is TM_DOUBLE).  Work fields are
- * allocated and freed inside the call.  Returns TM_OK also when max_iter was reached (see info->converged);
- * TM_ERR_PARAM on breakdown (<p, A p> <= 0).  Synchronous (every iteration reads two sums back). */
+ * starting from x_e = 0 (the content of x_e on entry is ignored).  One CG recurrence runs in sloppy_precision; whenever
+ * its residual has dropped by `delta` the partial solution is added to x_e in double, the true residual b - A x is formed
+ * in double and replaces the iterated one, and the recurrence continues with the same search direction (no restart).
+ * x_e, b_e and g_precise are double; g_sloppy is the same gauge field loaded in sloppy_precision (ignored, may be NULL,
+ * when that is TM_DOUBLE).  The work fields live on the context and are reused by later solves (tm_cg_release frees
+ * them; tm_finalize does too); nothing is allocated in a solve after the first.  The scalars of the recurrence stay on the
+ * device; the host looks at them one iteration late (no stream synchronisation per iteration).  Returns TM_OK also when
+ * max_iter was reached or the true residual stagnated (see info->converged); TM_ERR_PARAM on breakdown (<p, A p> <= 0). */
 int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, const tm_gauge *g_sloppy,
                  const tm_params *p, tm_matpc type, const tm_cg_params *cp, tm_cg_info *info);
+void tm_cg_release(tm_ctx *ctx);
 
 /* ---- diagnostics ----------------------------------------------------------------------------------- */
 const char *tm_last_error(void);       /* thread-local, never NULL */

@@ -34,7 +34,7 @@ EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
     "tm_field_device_ptr", "tm_set_host_basis", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb", "tm_field_upload_cb_async", "tm_field_download_cb_async",
     "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_twist_apply",
-    "tm_prepare_rhs", "tm_set_open_time", "tm_set_open_dirs", "tm_halo_bytes", "tm_halo_pack", "tm_halo_apply", "tm_field_axpby", "tm_field_redot", "tm_invert_cg", "tm_last_error",
+    "tm_prepare_rhs", "tm_set_open_time", "tm_set_open_dirs", "tm_halo_bytes", "tm_halo_pack", "tm_halo_apply", "tm_field_axpby", "tm_field_redot", "tm_invert_cg", "tm_cg_release", "tm_set_allreduce", "tm_last_error",
     "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_set_tuning", "tm_timing_enable", "tm_timing_read",
 ]
 
@@ -45,19 +45,25 @@ class TmError(RuntimeError):
         self.status = status
 
 
+class tm_params(ctypes.Structure):
+    _fields_ = [("kappa", ctypes.c_double), ("mu", ctypes.c_double), ("epsilon", ctypes.c_double),
+                ("twist_flavor", ctypes.c_int), ("t_boundary", ctypes.c_int)]
+
+
+# int op(out_e, in_e, tmp_o, gauge, params, matpc type, dagger, user)  /  int allreduce(dev_sums, n, cuda_stream, user)
+TM_CG_OP_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(tm_params),
+                               ctypes.c_int, ctypes.c_int, ctypes.c_void_p)
+TM_ALLREDUCE_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p)
+
+
 class tm_cg_params(ctypes.Structure):
     _fields_ = [("tol", ctypes.c_double), ("max_iter", ctypes.c_int), ("sloppy_precision", ctypes.c_int),
-                ("delta", ctypes.c_double)]
+                ("delta", ctypes.c_double), ("op", TM_CG_OP_FN), ("op_user", ctypes.c_void_p)]
 
 
 class tm_cg_info(ctypes.Structure):
     _fields_ = [("iterations", ctypes.c_int), ("restarts", ctypes.c_int), ("residual", ctypes.c_double),
                 ("converged", ctypes.c_int)]
-
-
-class tm_params(ctypes.Structure):
-    _fields_ = [("kappa", ctypes.c_double), ("mu", ctypes.c_double), ("epsilon", ctypes.c_double),
-                ("twist_flavor", ctypes.c_int), ("t_boundary", ctypes.c_int)]
 
 
 def params(kappa, mu, epsilon=0.0, twist_flavor=1, t_boundary=-1):
@@ -110,6 +116,9 @@ def lib():
     L.tm_field_axpby.argtypes = [vp, d, vp, d, vp]
     L.tm_field_redot.argtypes = [vp, vp, ctypes.POINTER(d)]
     L.tm_invert_cg.argtypes = [vp, vp, vp, vp, pp, i, ctypes.POINTER(tm_cg_params), ctypes.POINTER(tm_cg_info)]
+    L.tm_cg_release.argtypes = [vp]
+    L.tm_cg_release.restype = None
+    L.tm_set_allreduce.argtypes = [vp, TM_ALLREDUCE_FN, vp]
     L.tm_last_error.restype = ctypes.c_char_p
     L.tm_launch_count.argtypes = [vp]
     L.tm_launch_count.restype = ctypes.c_long
@@ -269,13 +278,22 @@ def tm_field_redot(x, y):
     return r.value
 
 
-def tm_invert_cg(x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol, max_iter, sloppy_precision, delta):
-    """-> dict(iterations, restarts, residual, converged)"""
-    cp = tm_cg_params(float(tol), int(max_iter), int(sloppy_precision), float(delta))
+def tm_invert_cg(x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol, max_iter, sloppy_precision, delta, op=None):
+    """-> dict(iterations, restarts, residual, converged).  op: a TM_CG_OP_FN (the caller's operator, e.g. a sharded one)."""
+    cp = tm_cg_params(float(tol), int(max_iter), int(sloppy_precision), float(delta), op if op is not None else TM_CG_OP_FN(), None)
     info = tm_cg_info()
     _check(lib().tm_invert_cg(x_e, b_e, g_precise, g_sloppy, ctypes.byref(p), int(matpc_type), ctypes.byref(cp),
                               ctypes.byref(info)))
     return dict(iterations=info.iterations, restarts=info.restarts, residual=info.residual, converged=bool(info.converged))
+
+
+def tm_cg_release(ctx):
+    lib().tm_cg_release(ctx)
+
+
+def tm_set_allreduce(ctx, fn):
+    """fn: a TM_ALLREDUCE_FN instance (keep a reference to it while it is set) or None."""
+    _check(lib().tm_set_allreduce(ctx, fn if fn is not None else TM_ALLREDUCE_FN(), None))
 
 
 def tm_launch_count(ctx):
@@ -436,6 +454,6 @@ def field_redot(x, y):
     return tm_field_redot(x.h, y.h)
 
 
-def invert_cg(x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol=1e-10, max_iter=10000, sloppy_precision=TM_SINGLE, delta=0.1):
+def invert_cg(x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol=1e-10, max_iter=10000, sloppy_precision=TM_SINGLE, delta=0.1, op=None):
     return tm_invert_cg(x_e.h, b_e.h, g_precise.h, None if g_sloppy is None else g_sloppy.h, p, matpc_type, tol, max_iter,
-                        sloppy_precision, delta)
+                        sloppy_precision, delta, op)

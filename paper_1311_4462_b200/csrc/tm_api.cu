@@ -194,6 +194,9 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->red_n = 0;
     c->cgs = nullptr;
     c->cgs_host = nullptr;
+    c->cg_ev[0] = c->cg_ev[1] = nullptr;
+    c->allreduce = nullptr;
+    c->allreduce_user = nullptr;
     c->up_stream = c->down_stream = nullptr;
     c->ev_compute = c->ev_up = c->ev_down = nullptr;
     c->up_staging = c->down_staging = nullptr;
@@ -243,6 +246,8 @@ void tm_finalize(tm_ctx *ctx)
     }
     if (ctx->up_staging) cudaFree(ctx->up_staging);
     if (ctx->down_staging) cudaFree(ctx->down_staging);
+    for (tm_field *f : ctx->cg_ws) tm_field_free(f);
+    for (auto e : ctx->cg_ev) if (e) cudaEventDestroy(e);
     if (ctx->cgs) cudaFree(ctx->cgs);
     if (ctx->halo_counter) cudaFree(ctx->halo_counter);
     if (ctx->cgs_host) cudaFreeHost(ctx->cgs_host);
@@ -824,32 +829,54 @@ int tm_field_redot(const tm_field *x, const tm_field *y, double *result)
 
 namespace {
 
-// work fields of one solve (library-owned device memory, zero-filled so that tile padding is defined)
-struct WorkFields {
-    std::vector<tm_field *> f;
-    ~WorkFields() { for (tm_field *p : f) tm_field_free(p); }
-    tm_field *make(tm_ctx *c, int prec, int nf)
-    {
-        tm_field *p = nullptr;
-        if (tm_field_alloc(c, (tm_precision)prec, nf, nullptr, 0, &p) != TM_OK) return nullptr;
-        f.push_back(p);
-        if (cudaMemsetAsync(p->ptr, 0, p->bytes, c->stream) != cudaSuccess) return nullptr;
-        return p;
-    }
-};
-
-// out = M^dag M in on the even sites; t_e and tmp_o are scratch of in's precision
-int apply_normal(tm_field *out, const tm_field *in, tm_field *t_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p, tm_matpc type)
+// Work fields of tm_invert_cg: library-owned device memory kept on the context between solves (zero-filled once so that tile
+// padding is defined).  Slot k of a (precision, flavors) pair is created on first use.
+tm_field *ws_field(tm_ctx *c, int prec, int nf, int k)
 {
-    int rc = tm_mat_pc(t_e, in, tmp_o, g, p, type, 0);
-    if (!rc) rc = tm_mat_pc(out, t_e, tmp_o, g, p, type, 1);
-    return rc;
+    int seen = 0;
+    for (tm_field *f : c->cg_ws)
+        if (f->prec == prec && f->nf == nf && seen++ == k) return f;
+    tm_field *p = nullptr;
+    if (tm_field_alloc(c, (tm_precision)prec, nf, nullptr, 0, &p) != TM_OK) return nullptr;
+    if (cudaMemsetAsync(p->ptr, 0, p->bytes, c->stream) != cudaSuccess) { tm_field_free(p); return nullptr; }
+    c->cg_ws.push_back(p);
+    return p;
 }
 
 #define TM_TRY_CUDA(call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, what); } while (0)
 #define TM_TRY(call) do { int rc_ = (call); if (rc_) return rc_; } while (0)
 
+// out = M^dag M in on the even sites; t_e and tmp_o are scratch of in's precision
+int apply_normal(tm_field *out, const tm_field *in, tm_field *t_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p, tm_matpc type,
+                 const tm_cg_params *cp)
+{
+    if (cp->op) {
+        if (cp->op(t_e, in, tmp_o, g, p, type, 0, cp->op_user)) return fail(TM_ERR_CUDA, "tm_invert_cg: the caller's operator failed");
+        if (cp->op(out, t_e, tmp_o, g, p, type, 1, cp->op_user)) return fail(TM_ERR_CUDA, "tm_invert_cg: the caller's operator failed");
+        return TM_OK;
+    }
+    int rc = tm_mat_pc(t_e, in, tmp_o, g, p, type, 0);
+    if (!rc) rc = tm_mat_pc(out, t_e, tmp_o, g, p, type, 1);
+    return rc;
+}
+
 }  // namespace
+
+int tm_set_allreduce(tm_ctx *ctx, tm_allreduce_fn fn, void *user)
+{
+    if (!ctx) return fail(TM_ERR_ARG, "tm_set_allreduce: NULL context");
+    ctx->allreduce = fn;
+    ctx->allreduce_user = user;
+    return TM_OK;
+}
+
+void tm_cg_release(tm_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    for (tm_field *f : ctx->cg_ws) tm_field_free(f);
+    ctx->cg_ws.clear();
+}
 
 int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, const tm_gauge *g_sloppy, const tm_params *p,
                  tm_matpc type, const tm_cg_params *cp, tm_cg_info *info)
@@ -872,76 +899,79 @@ int tm_invert_cg(tm_field *x_e, const tm_field *b_e, const tm_gauge *g_precise, 
     const int nf = x_e->nf;
     TM_USE_DEVICE(c);
 
-    WorkFields w;
-    tm_field *r_d = w.make(c, TM_DOUBLE, nf), *t_d = w.make(c, TM_DOUBLE, nf), *te_d = w.make(c, TM_DOUBLE, nf), *to_d = w.make(c, TM_DOUBLE, nf);
-    tm_field *r_s = w.make(c, ps, nf), *p_s = w.make(c, ps, nf), *ap_s = w.make(c, ps, nf), *x_s = w.make(c, ps, nf);
-    tm_field *te_s = w.make(c, ps, nf), *to_s = w.make(c, ps, nf);
+    // double: residual, A x, two scratch fields; sloppy: residual, direction, A p, partial solution, two scratch fields
+    const int d0 = ps == TM_DOUBLE ? 4 : 0;        // sloppy = double: the two sets share one pool
+    tm_field *r_d = ws_field(c, TM_DOUBLE, nf, 0), *t_d = ws_field(c, TM_DOUBLE, nf, 1), *te_d = ws_field(c, TM_DOUBLE, nf, 2), *to_d = ws_field(c, TM_DOUBLE, nf, 3);
+    tm_field *r_s = ws_field(c, ps, nf, d0 + 0), *p_s = ws_field(c, ps, nf, d0 + 1), *ap_s = ws_field(c, ps, nf, d0 + 2), *x_s = ws_field(c, ps, nf, d0 + 3);
+    tm_field *te_s = ps == TM_DOUBLE ? te_d : ws_field(c, ps, nf, 4), *to_s = ps == TM_DOUBLE ? to_d : ws_field(c, ps, nf, 5);
     if (!r_d || !t_d || !te_d || !to_d || !r_s || !p_s || !ap_s || !x_s || !te_s || !to_s) return fail(TM_ERR_NOMEM, "tm_invert_cg: work fields");
 
     if (!c->cgs) TM_TRY_CUDA(cudaMalloc(&c->cgs, 4 * sizeof(double)), "cudaMalloc(cg scalars)");
     if (!c->cgs_host) TM_TRY_CUDA(cudaHostAlloc(&c->cgs_host, 6 * sizeof(double), cudaHostAllocDefault), "cudaHostAlloc(cg scalars)");
-    struct EventRing {
-        cudaEvent_t ev[2] = {nullptr, nullptr};
-        ~EventRing() { for (auto e : ev) if (e) cudaEventDestroy(e); }
-    } ring;
-    for (auto &e : ring.ev) TM_TRY_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
+    if (!c->cg_ev[0])
+        for (auto &e : c->cg_ev) TM_TRY_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
 
     double bnorm2 = 0.0, rnorm2 = 0.0;
     TM_TRY_CUDA(tm_blas_redot(b_e, b_e, &bnorm2), "redot");
     TM_TRY_CUDA(tm_blas_axpbyz(x_e, 0.0, b_e, 0.0, nullptr, nullptr), "zero x");        // x = 0
     if (bnorm2 == 0.0) { info->converged = 1; return TM_OK; }
-    TM_TRY_CUDA(tm_blas_axpbyz(r_d, 1.0, b_e, 0.0, nullptr, &rnorm2), "copy b");          // r = b
+    TM_TRY_CUDA(tm_blas_axpbyz(r_d, 1.0, b_e, 0.0, nullptr, nullptr), "copy b");          // r = b
+    rnorm2 = bnorm2;
 
-    // defect correction: the inner CG runs in the sloppy precision on A e = r / |r| until the residual has dropped by
-    // delta (or as far as the outer tolerance needs); x += |r| e and the residual b - A x are formed in double.
-    for (;;) {
-        const double relres = std::sqrt(rnorm2 / bnorm2);
-        info->residual = relres;
-        if (relres <= cp->tol) { info->converged = 1; break; }
-        if (info->iterations >= cp->max_iter) break;
-        const double rn = std::sqrt(rnorm2);
-        double rr = 0.0, rr0;
-        TM_TRY_CUDA(tm_blas_axpbyz(r_s, 1.0 / rn, r_d, 0.0, nullptr, &rr), "scale r");                // r_s = r / |r|
-        TM_TRY_CUDA(tm_blas_axpbyz(x_s, 0.0, r_s, 0.0, nullptr, nullptr), "zero e");                  // e = 0
-        TM_TRY_CUDA(tm_blas_axpbyz(p_s, 1.0, r_s, 0.0, nullptr, nullptr), "copy p");                  // p = r_s
-        rr0 = rr;
-        const double target = std::max(cp->delta, 0.5 * cp->tol / relres);
-        // Inner loop with DEVICE-RESIDENT scalars: alpha = |r|^2 / <p, A p> and beta = |r_new|^2 / |r|^2 are formed inside the
-        // update kernels from c->cgs, so no step waits for the host.  The scalars of every iteration are copied to a pinned
-        // ring and the host looks at them ONE ITERATION LATE (by then they have arrived): the stopping test and the
-        // breakdown test lag by one iteration, i.e. at most one update more than needed is applied to e.
-        double *sc = c->cgs, *hs = c->cgs_host;
-        hs[0] = rr;
-        TM_TRY_CUDA(cudaMemcpyAsync(sc, hs, sizeof(double), cudaMemcpyHostToDevice, c->stream), "rr -> device");
-        TM_TRY_CUDA(cudaStreamSynchronize(c->stream), "rr -> device");       // hs is reused as the ring below
-        int cur = 0, it = 0, stop = 0;
-        auto look = [&](int slot, int rr_idx) -> int {                        // the scalars of an iteration whose copy has landed
-            TM_TRY_CUDA(cudaEventSynchronize(ring.ev[slot]), "cg scalars");
-            const double pap = hs[3 * slot + 2], rr_new = hs[3 * slot + rr_idx];
-            if (!(pap > 0.0)) return fail(TM_ERR_PARAM, "tm_invert_cg: <p, A p> = %g is not positive (breakdown)", pap);
-            if (!(rr_new >= 0.0)) return fail(TM_ERR_PARAM, "tm_invert_cg: |r|^2 = %g (breakdown)", rr_new);
-            if (std::sqrt(rr_new / rr0) <= target) stop = 1;
-            return TM_OK;
-        };
-        int prev_idx = 0;
-        for (;; it++) {
-            TM_TRY(apply_normal(ap_s, p_s, te_s, to_s, gs, p, type));                                                  // Ap
-            TM_TRY_CUDA(tm_blas_redot_dev(p_s, ap_s, nullptr, sc + 2), "redot");                                         // <p, A p>
-            TM_TRY_CUDA(tm_blas_cg_update_dev(x_s, r_s, p_s, ap_s, 0.0, nullptr, sc + cur, sc + 2, sc + (1 - cur)), "cg_update");
-            TM_TRY_CUDA(cudaMemcpyAsync(hs + 3 * (it & 1), sc, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "cg scalars");
-            TM_TRY_CUDA(cudaEventRecord(ring.ev[it & 1], c->stream), "cg scalars");
-            info->iterations++;
-            if (it > 0) TM_TRY(look((it - 1) & 1, prev_idx));
-            prev_idx = 1 - cur;
-            if (stop || info->iterations >= cp->max_iter) break;
-            TM_TRY_CUDA(tm_blas_axpbyz_dev(p_s, 1.0, r_s, 0.0, p_s, nullptr, sc + (1 - cur), sc + cur), "xpay");        // p = r_s + beta p
-            cur = 1 - cur;
+    // One CG recurrence in the sloppy precision with DEVICE-RESIDENT scalars: alpha = |r|^2 / <p, A p> and beta = |r_new|^2 / |r|^2
+    // are formed inside the update kernels from c->cgs, so no step waits for the host.  The scalars of every iteration are copied
+    // to a pinned ring and the host looks at them ONE ITERATION LATE (by then they have arrived): the reliable-update decision,
+    // the stopping test and the breakdown test lag by one iteration.
+    double *sc = c->cgs, *hs = c->cgs_host;
+    TM_TRY_CUDA(tm_blas_axpbyz(r_s, 1.0, r_d, 0.0, nullptr, nullptr), "r_s = r");
+    TM_TRY_CUDA(tm_blas_axpbyz(p_s, 1.0, r_s, 0.0, nullptr, nullptr), "p = r_s");
+    TM_TRY_CUDA(tm_blas_axpbyz(x_s, 0.0, r_s, 0.0, nullptr, nullptr), "x_s = 0");
+    int cur = 0;
+    TM_TRY_CUDA(tm_blas_redot_dev(r_s, r_s, nullptr, sc + cur), "|r_s|^2");
+    double rmax = std::sqrt(rnorm2), last_true = rnorm2;
+    int stagnant = 0, update = 0, stop = 0;
+    auto look = [&](int slot, int rr_idx) -> int {                        // the scalars of an iteration whose copy has landed
+        TM_TRY_CUDA(cudaEventSynchronize(c->cg_ev[slot]), "cg scalars");
+        const double pap = hs[3 * slot + 2], rr_new = hs[3 * slot + rr_idx];
+        if (!(pap > 0.0)) return fail(TM_ERR_PARAM, "tm_invert_cg: <p, A p> = %g is not positive (breakdown)", pap);
+        if (!(rr_new >= 0.0)) return fail(TM_ERR_PARAM, "tm_invert_cg: |r|^2 = %g (breakdown)", rr_new);
+        const double rn = std::sqrt(rr_new);
+        if (rn < cp->delta * rmax || rn <= cp->tol * std::sqrt(bnorm2)) update = 1;
+        if (rn > rmax) rmax = rn;
+        return TM_OK;
+    };
+    int prev_idx = 0;
+    for (int it = 0;; it++) {
+        TM_TRY(apply_normal(ap_s, p_s, te_s, to_s, gs, p, type, cp));                                                  // A p
+        TM_TRY_CUDA(tm_blas_redot_dev(p_s, ap_s, nullptr, sc + 2), "redot");                                             // <p, A p>
+        TM_TRY_CUDA(tm_blas_cg_update_dev(x_s, r_s, p_s, ap_s, 0.0, nullptr, sc + cur, sc + 2, sc + (1 - cur)), "cg_update");
+        TM_TRY_CUDA(cudaMemcpyAsync(hs + 3 * (it & 1), sc, 3 * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "cg scalars");
+        TM_TRY_CUDA(cudaEventRecord(c->cg_ev[it & 1], c->stream), "cg scalars");
+        info->iterations++;
+        if (it > 0) TM_TRY(look((it - 1) & 1, prev_idx));
+        prev_idx = 1 - cur;
+        const bool last = info->iterations >= cp->max_iter;
+        if (last) TM_TRY(look(it & 1, prev_idx));                           // the final iteration's scalars (breakdown test)
+        if (update || last) {
+            // reliable update: x += x_s, x_s = 0, r = b - A x in double replaces the iterated residual; the direction is kept
+            TM_TRY_CUDA(tm_blas_axpbyz(x_e, 1.0, x_s, 1.0, x_e, nullptr), "x += x_s");
+            TM_TRY_CUDA(tm_blas_axpbyz(x_s, 0.0, r_s, 0.0, nullptr, nullptr), "x_s = 0");
+            TM_TRY(apply_normal(t_d, x_e, te_d, to_d, g_precise, p, type, cp));
+            TM_TRY_CUDA(tm_blas_axpbyz(r_d, 1.0, b_e, -1.0, t_d, &rnorm2), "r = b - A x");
+            info->restarts++;
+            info->residual = std::sqrt(rnorm2 / bnorm2);
+            if (info->residual <= cp->tol) { info->converged = 1; stop = 1; }
+            stagnant = rnorm2 > 0.81 * last_true ? stagnant + 1 : 0;       // the true residual must keep falling (by 10 % at least)
+            if (stagnant >= 3) stop = 1;                                  // e.g. a half-precision recurrence below its own noise
+            last_true = rnorm2;
+            if (stop || last) break;
+            TM_TRY_CUDA(tm_blas_axpbyz(r_s, 1.0, r_d, 0.0, nullptr, nullptr), "r_s = r");
+            TM_TRY_CUDA(tm_blas_redot_dev(r_s, r_s, nullptr, sc + (1 - cur)), "|r_s|^2");
+            rmax = std::sqrt(rnorm2);
+            update = 0;
         }
-        TM_TRY(look(it & 1, prev_idx));                                        // the last iteration's scalars (breakdown test)
-        TM_TRY_CUDA(tm_blas_axpbyz(x_e, rn, x_s, 1.0, x_e, nullptr), "x += |r| e");
-        TM_TRY(apply_normal(t_d, x_e, te_d, to_d, g_precise, p, type));                                // true residual in double
-        TM_TRY_CUDA(tm_blas_axpbyz(r_d, 1.0, b_e, -1.0, t_d, &rnorm2), "r = b - A x");
-        info->restarts++;
+        TM_TRY_CUDA(tm_blas_axpbyz_dev(p_s, 1.0, r_s, 0.0, p_s, nullptr, sc + (1 - cur), sc + cur), "xpay");            // p = r_s + beta p
+        cur = 1 - cur;
     }
     return TM_OK;
 }

@@ -140,11 +140,20 @@ cudaError_t reduce_buffers(tm_ctx *c, int blocks)
     return cudaSuccess;
 }
 
+// multi-GPU: the caller's all-reduce (tm_set_allreduce) sums the device word over the ranks, in stream order
+cudaError_t global_sum(tm_ctx *c, double *dev_word)
+{
+    if (!c->allreduce) return cudaSuccess;
+    return c->allreduce(dev_word, 1, static_cast<void *>(c->stream), c->allreduce_user) == 0 ? cudaSuccess : cudaErrorUnknown;
+}
+
 // partials are in c->red[1..blocks]; the sum goes to *dev_out and stays on the device (no synchronisation)
 cudaError_t finish_sum_dev(tm_ctx *c, int blocks, double *dev_out)
 {
     final_sum_kernel<<<1, 256, 0, c->stream>>>(c->red + 1, blocks, dev_out);
-    return cudaGetLastError();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return global_sum(c, dev_out);
 }
 
 // partials are in c->red[1..blocks]; the sum goes to c->red[0] and from there to *host (synchronises the stream)
@@ -153,6 +162,7 @@ cudaError_t finish_sum(tm_ctx *c, int blocks, double *host)
     final_sum_kernel<<<1, 256, 0, c->stream>>>(c->red + 1, blocks, c->red);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if ((e = global_sum(c, c->red)) != cudaSuccess) return e;
     e = cudaMemcpyAsync(host, c->red, sizeof(double), cudaMemcpyDeviceToHost, c->stream);
     if (e != cudaSuccess) return e;
     return cudaStreamSynchronize(c->stream);

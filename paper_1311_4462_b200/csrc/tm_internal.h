@@ -51,8 +51,12 @@ struct tm_ctx {
     bool async_ready;
     int open_mask;        // tm_set_open_dirs: bit mu set = the fused kernels drop the mu hops that leave the sub-lattice (tm_halo.cu adds them)
     unsigned *halo_counter;   // device word: blocks of the running halo_pack kernel that have finished (flag signalling)
+    tm_allreduce_fn allreduce;   // tm_set_allreduce: sums a device word over the ranks (NULL: one GPU)
+    void *allreduce_user;
+    std::vector<tm_field *> cg_ws;   // work fields of tm_invert_cg, kept between solves (freed by tm_cg_release / tm_finalize)
     double *cgs;          // inner CG scalars on the device: [0], [1] |r|^2 (ping-pong), [2] <p, A p>
     double *cgs_host;     // pinned host ring the scalars are copied to: 2 x 3 doubles
+    cudaEvent_t cg_ev[2]; // one event per ring slot
     double *red;          // reduction scratch of tm_blas.cu: [0] result, [1..] per-block partial sums
     size_t red_n;
     size_t staging_bytes;

@@ -278,3 +278,51 @@ class Slab:
         self.dslash_apply(tmp_o, in_e, None, gauge, p, tm.TM_ODD, dagger, tm.TM_TWIST_INV_DSLASH)
         self.dslash_apply(out_e, tmp_o, in_e, gauge, p, tm.TM_EVEN, dagger,
                           tm.TM_DSLASH_TWIST_XPAY if matpc_type == tm.TM_MATPC_ASYM else tm.TM_TWIST_INV_DSLASH_XPAY)
+
+    # ---- the solver on the decomposed lattice (the paper's CG runs on many GPUs) -----------------------
+    def allreduce_hook(self):
+        """A tm.TM_ALLREDUCE_FN that sums the library's device scalars over the ranks with torch.distributed.all_reduce (NCCL) on
+        the current stream; install with tm.tm_set_allreduce(self.lat.ctx, hook) and keep the reference."""
+        group = self.group
+
+        class _Words:
+            def __init__(self, ptr, n):
+                self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+
+        def fn(dev_sums, n, stream, user):
+            try:
+                if self.world > 1:
+                    import torch.distributed as dist
+                    dist.all_reduce(torch.as_tensor(_Words(dev_sums, n), device=self.device), group=group)
+                return 0
+            except Exception:
+                return 1
+        return tm.TM_ALLREDUCE_FN(fn)
+
+    def invert_cg(self, x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol=1e-10, max_iter=10000, sloppy_precision=tm.TM_SINGLE, delta=0.1):
+        """tm_invert_cg on this rank's part of the lattice: the operator is Slab.mat_pc (face exchange inside every hopping
+        term), the dot products are summed over the ranks (allreduce_hook).  Every rank calls it with its part of b_e."""
+        by_gauge = {g_precise.h.value if hasattr(g_precise.h, "value") else g_precise.h: g_precise}
+        if g_sloppy is not None:
+            by_gauge[g_sloppy.h.value if hasattr(g_sloppy.h, "value") else g_sloppy.h] = g_sloppy
+        nf = x_e.nf
+
+        class _F:                                  # a field the library hands to the callback: handle + what Slab.mat_pc reads
+            def __init__(self, h, prec):
+                self.h, self.prec, self.nf = h, prec, nf
+
+        def op(out_e, in_e, tmp_o, g, pp, typ, dagger, user):
+            try:
+                gauge = by_gauge[g]
+                self.mat_pc(_F(out_e, gauge.prec), _F(in_e, gauge.prec), _F(tmp_o, gauge.prec), gauge, pp.contents, typ, dagger)
+                return 0
+            except Exception:
+                import traceback
+                traceback.print_exc()
+                return 1
+        hook = self.allreduce_hook()
+        tm.tm_set_allreduce(self.lat.ctx, hook)
+        try:
+            return tm.invert_cg(x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol, max_iter, sloppy_precision, delta, op=tm.TM_CG_OP_FN(op))
+        finally:
+            tm.tm_set_allreduce(self.lat.ctx, None)

@@ -107,3 +107,74 @@ def test_s3_cg_edge_cases():
     assert status(lambda: tm.invert_cg(fx, fb, gs, gs, pg, tm.TM_MATPC_ASYM)) == tm.TM_ERR_MISMATCH
     assert status(lambda: tm.invert_cg(fx, fb, gd, None, pg, tm.TM_MATPC_ASYM)) == tm.TM_ERR_MISMATCH
     assert status(lambda: tm.invert_cg(fx, fb, gd, gs, pg, tm.TM_MATPC_ASYM, delta=1.5)) == tm.TM_ERR_ARG
+
+
+@pytest.mark.parametrize("kw,typ", [(FLAVORS[0], tm.TM_MATPC_SYM), (FLAVORS[1], tm.TM_MATPC_ASYM)], ids=["deg-sym", "ndeg-asym"])
+def test_s4_cg_16c16_reliable_updates_and_workspace_reuse(kw, typ):
+    """16^4 (beyond the 4^3 x 8 toy): the solution of every precision mix has residual <= 5 tol under the ORACLE's
+    fp64 M^dag M; reliable updates keep one recurrence going (the sloppy solvers need about as many iterations as plain double,
+    where defect-correction restarts needed many more); the work fields live on the context: no device allocation after the
+    first solve of a precision mix."""
+    import torch
+    dims = (16, 16, 16, 16)
+    nf = nf_of(kw)
+    U = si.gauge_field(dims, 36, "near_identity")
+    bench = Bench(dims, U)
+    lat = bench.lat
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    A = lambda v: oracle.matpc_adjoint(oracle.matpc(v, U, po, typ), U, po, typ)
+    psi_e = si.mask_parity(si.spinor_field(dims, nf, 37), dims, 0)
+    b = A(psi_e)
+    gd = bench.gauge(tm.TM_DOUBLE, tm.TM_RECON_12)
+    fb = lat.field(tm.TM_DOUBLE, nf).upload(0, b)
+    fx = lat.field(tm.TM_DOUBLE, nf)
+    tol, iters = 1e-9, {}
+    for ps, delta in ((tm.TM_DOUBLE, 0.1), (tm.TM_SINGLE, 0.1), (tm.TM_HALF, 0.3)):
+        gs = None if ps == tm.TM_DOUBLE else bench.gauge(ps, tm.TM_RECON_12)
+        info = tm.invert_cg(fx, fb, gd, gs, pg, typ, tol=tol, max_iter=5000, sloppy_precision=ps, delta=delta)
+        assert info["converged"] and info["residual"] <= tol, (ps, info)
+        x = fx.download(0)
+        assert rel_l2(A(x), b) <= 5 * tol, (ps, info)
+        assert rel_l2(x, psi_e) <= 1e-6, (ps, info)
+        iters[ps] = info
+        lat.sync()
+        free0 = torch.cuda.mem_get_info()[0]
+        again = tm.invert_cg(fx, fb, gd, gs, pg, typ, tol=tol, max_iter=5000, sloppy_precision=ps, delta=delta)
+        lat.sync()
+        assert torch.cuda.mem_get_info()[0] == free0                     # the second solve allocates nothing
+        assert again["iterations"] == info["iterations"] and again["residual"] == info["residual"]      # and is deterministic
+    print("16^4 iterations / reliable updates:", {k: (v["iterations"], v["restarts"]) for k, v in iters.items()})
+    assert iters[tm.TM_SINGLE]["iterations"] <= 1.15 * iters[tm.TM_DOUBLE]["iterations"] + 5
+    assert iters[tm.TM_HALF]["iterations"] <= 1.6 * iters[tm.TM_DOUBLE]["iterations"] + 10
+    tm.tm_cg_release(lat.ctx)
+    lat.sync()
+
+
+def test_s5_cg_on_the_decomposed_lattice_world_1():
+    """Slab.invert_cg: the solver with the distributed operator (face exchange inside every hopping term, through the peer-buffer
+    transport) and the dot products passed through the all-reduce hook; one rank that is its own neighbour in z and t.  The
+    solution equals the undecomposed solver's and solves the oracle's normal equations."""
+    from paper_1311_4462_b200 import sharded
+    dims = (8, 8, 8, 8)
+    kw = FLAVORS[1]
+    U = si.gauge_field(dims, 38, "near_identity")
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    typ = tm.TM_MATPC_SYM
+    A = lambda v: oracle.matpc_adjoint(oracle.matpc(v, U, po, typ), U, po, typ)
+    b = A(si.mask_parity(si.spinor_field(dims, 2, 39), dims, 0))
+    s = sharded.Slab(dims, 0, 1, cut=(2, 3), peer=True)
+    lat = s.lat
+    gd, gs = lat.gauge(U, tm.TM_DOUBLE, tm.TM_RECON_12), lat.gauge(U, tm.TM_SINGLE, tm.TM_RECON_12)
+    fb, fx = lat.field(tm.TM_DOUBLE, 2).upload(0, b), lat.field(tm.TM_DOUBLE, 2)
+    n0 = lat.launches()
+    info = s.invert_cg(fx, fb, gd, gs, pg, typ, tol=1e-9, max_iter=2000, sloppy_precision=tm.TM_SINGLE, delta=0.1)
+    assert info["converged"], info
+    x = fx.download(0)
+    assert rel_l2(A(x), b) <= 5e-9, info
+    assert lat.launches() - n0 > info["iterations"] * (4 + 2 * 4 * 2)      # 4 hopping terms, each with 2 directions x (pack + completion)
+    plain = tm.Lattice(dims)
+    gd2, gs2 = plain.gauge(U, tm.TM_DOUBLE, tm.TM_RECON_12), plain.gauge(U, tm.TM_SINGLE, tm.TM_RECON_12)
+    fb2, fx2 = plain.field(tm.TM_DOUBLE, 2).upload(0, b), plain.field(tm.TM_DOUBLE, 2)
+    info2 = tm.invert_cg(fx2, fb2, gd2, gs2, pg, typ, tol=1e-9, max_iter=2000, sloppy_precision=tm.TM_SINGLE, delta=0.1)
+    assert abs(info2["iterations"] - info["iterations"]) <= 2
+    assert rel_l2(x, fx2.download(0)) <= 1e-7
