@@ -18,7 +18,8 @@ rank runs the same step on its own GPU, value = N x units / max-over-ranks time,
 
 --impl reference times the CPU oracle (oracle/, fp64, as it stands) on the host cores on the same full-lattice step.
 The JSON line also carries `kernels` (every launch of the step, timed inside the loop) and `kernels_extra` (every kernel type x
-precision x flavors x link compression of the library + the Wilson limit, each timed alone in the same run).
+precision x flavors x link compression of the library + the Wilson limit, each timed alone in the same run) and `cg`
+(tm_invert_cg: iterations and ms per iteration, double / double-single / double-half, Eq. 2.2 against Eq. 2.3).
 """
 import argparse
 import json
@@ -219,11 +220,12 @@ def write_sass_mix():
         txt = subprocess.run(["cuobjdump", "-sass", obj], capture_output=True, text=True).stdout
         for blk in txt.split("Function : ")[1:]:
             mangled = blk.split("\n", 1)[0].strip()
-            m = re.match(r"_Z\d+tm_dslash_(f2|generic)ILi(\d)ELi(\d)ELi(\d+)ELi(\d)ELb([01])ELb([01])E", mangled)
+            m = re.match(r"_Z\d+tm_dslash_(f2|generic)ILi(\d)ELi(\d)ELi(\d+)ELi(\d)ELb([01])ELb([01])ELb([01])EE", mangled)
             if not m:
                 continue
-            fam, prec, nf, recon, kt, dag, stg = m.groups()
-            name = "%s%s<%s,%s,%s,%s,%s>" % (fam, "_staged" if stg == "1" else "", prec, nf, recon, kt, "dagger" if dag == "1" else "plain")
+            fam, prec, nf, recon, kt, dag, stg, twin = m.groups()
+            name = "%s%s%s<%s,%s,%s,%s,%s>" % (fam, "_twin" if twin == "1" else "", "_staged" if stg == "1" else "", prec, nf, recon, kt,
+                                              "dagger" if dag == "1" else "plain")
             hist = {}
             for line in blk.splitlines():
                 mm = re.match(r"\s+/\*[0-9a-f]{4,}\*/\s+(?:@!?U?P\w+\s+)?([A-Z][A-Z0-9_]*)", line)
@@ -257,29 +259,28 @@ def import_ncu(csv_path):
     import csv
     import re
     acc = {}
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
     with open(csv_path, newline="") as f:
-        rd = csv.reader(f)
-        hdr = None
-        for row in rd:
-            if hdr is None:
-                if "Kernel Name" in row:
-                    hdr = row
-                continue
-            if len(row) != len(hdr) or not row[0].isdigit():
-                continue
-            d = dict(zip(hdr, row))
-            m = re.search(r"tm_dslash_(f2|generic)<\(?int\)?(\d), \(?int\)?(\d), \(?int\)?(\d+), \(?int\)?(\d), \(?bool\)?(\w+), \(?bool\)?(\w+)>", d["Kernel Name"].replace("(int)", "").replace("(bool)", ""))
-            if not m:
-                continue
-            fam, prec, nf, recon, kt, dag, stg = m.groups()
-            name = "%s%s<%s,%s,%s,%s,%s>" % (fam, "_staged" if stg in ("1", "true") else "", prec, nf, recon, kt, "dagger" if dag in ("1", "true") else "plain")
-            try:
-                b = float(d["dram__bytes_read.sum"].replace(",", "")) + float(d["dram__bytes_write.sum"].replace(",", ""))
-            except (KeyError, ValueError):
-                continue
-            a = acc.setdefault(name, [0.0, 0])
-            a[0] += b
-            a[1] += 1
+        rows = list(csv.reader(f))
+    hdr = next(r for r in rows if "Kernel Name" in r)
+    units = dict(zip(hdr, rows[rows.index(hdr) + 1]))            # the line under the header carries the unit of every column
+    for row in rows:
+        if len(row) != len(hdr) or not row[0].isdigit():
+            continue
+        d = dict(zip(hdr, row))
+        m = re.search(r"tm_dslash_(f2|generic)<(\d), (\d), (\d+), (\d), (\w+), (\w+)(?:, (\w+))?>", d["Kernel Name"].replace("(int)", "").replace("(bool)", ""))
+        if not m:
+            continue
+        fam, prec, nf, recon, kt, dag, stg, twin = m.groups()
+        name = "%s%s%s<%s,%s,%s,%s,%s>" % (fam, "_twin" if twin in ("1", "true") else "", "_staged" if stg in ("1", "true") else "", prec, nf, recon, kt,
+                                          "dagger" if dag in ("1", "true") else "plain")
+        try:
+            b = sum(float(d[k].replace(",", "")) * scale[units[k]] for k in ("dram__bytes_read.sum", "dram__bytes_write.sum"))
+        except (KeyError, ValueError):
+            continue
+        a = acc.setdefault(name, [0.0, 0])
+        a[0] += b
+        a[1] += 1
     commit = subprocess.run(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip()
     with open(os.path.join(ROOT, "profiles", "traffic.csv"), "w") as f:
         f.write("# source_hash=%s parent_commit=%s  kernel ; DRAM bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean over "
@@ -489,6 +490,130 @@ def kernels_extra(w, args, sm_mhz, peak):
     return out
 
 
+def cg_leg(w):
+    """Mixed-precision CG (tm_invert_cg, reliable updates) on M^dag M x = b at 32^3x64, 12-real links: iterations and device time per
+    iteration for double, double-single (DS) and double-half (DH), Eq. 2.2 (asym) against Eq. 2.3 (sym) preconditioning -- the
+    comparison of the paper's Table 2 with its parameters kappa = 0.156361, mu = 0.0015 for the degenerate
+    doublet and mu = 0.15, eps = 0.19 for the non-degenerate one, but on SYNTHETIC exp(i 0.3 H) links, which are far better
+    conditioned than the paper's ensembles (tens of iterations, not thousands): context for the cost per iteration, not a target."""
+    import torch
+    tm, lat = w.tm, w.lat
+    host_u = w.host_gauge[2]
+    gauges = {prec: (w.gauge.get((2, prec)) or lat.gauge(host_u, prec, RECON)) for prec in (8, 4, 2)}
+    out = []
+    for nf, kw, label in ((1, dict(mu=0.0015, epsilon=0.0, twist_flavor=1), "degenerate"), (2, NDEG, "non-degenerate")):
+        p = tm.params(0.156361, **kw)
+        fb = lat.field(8, nf).upload_cb(0, w.host_in[nf])
+        fx = lat.field(8, nf)
+        for typ, tname in ((ASYM, "asym (Eq. 2.2)"), (SYM, "sym (Eq. 2.3)")):
+            for ps, pname, delta in ((8, "double", 0.1), (4, "double-single", 0.1), (2, "double-half", 0.3)):
+                kwargs = dict(tol=1e-8, max_iter=2000, sloppy_precision=ps, delta=delta)
+                tm.invert_cg(fx, fb, gauges[8], None if ps == 8 else gauges[ps], p, typ, **kwargs)      # warm-up: work fields allocated
+                lat.sync()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                info = tm.invert_cg(fx, fb, gauges[8], None if ps == 8 else gauges[ps], p, typ, **kwargs)
+                e1.record()
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1)
+                out.append({"doublet": label, "preconditioning": tname, "precision": pname, "iterations": info["iterations"],
+                            "reliable_updates": info["restarts"], "converged": info["converged"], "residual": info["residual"],
+                            "ms": ms, "ms_per_iteration": ms / max(info["iterations"], 1)})
+        del fb, fx
+    tm.tm_cg_release(lat.ctx)
+    return out
+
+
+def run_kernels(args, log):
+    """--kernels PREC:NF:RECON:KT[,...] [--dims X,Y,Z,T] [--tune key=value,...]: single kernels timed alone (30 launches between two
+    CUDA events, best of 3) through tm_dslash_apply -- the tuning runs of profiles/r2_tuning.md.  KT = tm_kernel_type (0..8).  Inputs: links drawn
+    from a pool of 4096 Haar matrices (seed 3), Gaussian spinors: fast to generate at 48^3x96; the kernels have no data-dependent control flow."""
+    import torch
+    import paper_1311_4462_b200 as tm
+    import synth_inputs as si
+    dims = tuple(int(v) for v in args.dims.split(","))
+    specs = [tuple(int(v) for v in a.split(":")) for a in args.kernels.split(",")]
+    V = si.volume(dims)
+    vh = V // 2
+    rng = np.random.default_rng(7)
+    U = si.haar_su3(4096, 3)[rng.integers(0, 4096, size=4 * V)].reshape(4, V, 3, 3)
+    lat = tm.Lattice(dims, 0)
+    for kv in [t for t in args.tune.split(",") if t]:
+        k, v = kv.split("=")
+        tm.tm_set_tuning(lat.ctx, k, int(v))
+    peak, _ = measured_peak()
+    gauges, fields, out = {}, {}, []
+    for prec, nf, recon, kt in specs:
+        if (prec, recon) not in gauges:
+            gauges[(prec, recon)] = lat.gauge(U, prec, recon)
+        if (prec, nf) not in fields:
+            h = rng.standard_normal((nf, vh, 4, 3)) + 1j * rng.standard_normal((nf, vh, 4, 3))
+            fields[(prec, nf)] = (lat.field(prec, nf).upload_cb(0, h), lat.field(prec, nf).upload_cb(0, h), lat.field(prec, nf))
+    pd, pn = tm.params(KAPPA, **DEG), tm.params(KAPPA, **NDEG)
+    for prec, nf, recon, kt in specs:
+        fin, fx, fout = fields[(prec, nf)]
+        g, p = gauges[(prec, recon)], (pd if nf == 1 else pn)
+        no_x = kt in (0, 6)
+        us = time_alone(lambda: tm.dslash_apply(fout, fin, None if no_x else fx, g, p, 1, 0, kt), lat.sync, launches=30)
+        kcode = {4: 2, 5: 3, 6: 0, 7: 3, 8: 3}.get(kt, kt)
+        b = (bytes_per_site(nf, prec, recon, kcode) + (nf * 12 * prec + (4 * nf if prec == 2 else 0) if kt >= 6 else 0)) * vh     # D R^-1: full time-hop sites
+        out.append({"spec": "%d:%d:%d:%d" % (prec, nf, recon, kt), "kernel": tm.tm_last_kernel_name(lat.ctx), "us": us, "alg_gbs": b / us / 1e3,
+                    "frac_of_measured_peak": b / us / 1e3 / peak})
+        log("%-12s %-36s %8.1f us  %6.0f GB/s  frac %.3f" % (out[-1]["spec"], out[-1]["kernel"], us, b / us / 1e3, b / us / 1e3 / peak))
+    print(json.dumps({"mode": "kernels", "dims": list(dims), "tune": args.tune, "kernels": out}))
+
+
+def run_config5(args, log):
+    """--config5: BASELINE.json configs[4] -- 48^3x96 non-degenerate doublet, fp64, Haar links (18-real), kappa = 0.1632, mu = 0.135,
+    eps = 0.17, the symmetric-preconditioned Eq. 2.3 operator applied 100 times back to back (one timed region); prints its own JSON line."""
+    import torch
+    import paper_1311_4462_b200 as tm
+    import synth_inputs as si
+    dims = (48, 48, 48, 96)
+    torch.cuda.set_device(0)
+    t = time.time()
+    U = si.gauge_field(dims, 5, "haar")
+    psi = si.to_parity(si.spinor_field(dims, 2, 5), dims, 0)
+    log("48^3x96 host inputs generated in %.1f s" % (time.time() - t))
+    lat = tm.Lattice(dims, 0)
+    vh = lat.Vh
+    g = lat.gauge(U, 8, 18)
+    fin, ftmp, fout = lat.field(8, 2).upload_cb(0, psi), lat.field(8, 2), lat.field(8, 2)
+    p = tm.params(KAPPA, mu=0.135, epsilon=0.17, twist_flavor=0)
+    for _ in range(10):
+        tm.mat_pc(fout, fin, ftmp, g, p, SYM, 0)
+    lat.sync()
+    tm.tm_timing_enable(lat.ctx, 1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(100):
+        tm.mat_pc(fout, fin, ftmp, g, p, SYM, 0)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    rec = tm.tm_timing_read(lat.ctx, 1 << 12)
+    tm.tm_timing_enable(lat.ctx, 0)
+    peak, peak_src = measured_peak()
+    flops = (flops_per_site(2, 0) + flops_per_site(2, 1)) * vh * 100
+    byts = (bytes_per_site(2, 8, 18, 0) + bytes_per_site(2, 8, 18, 1)) * vh * 100
+    per = {}
+    for name, tms in rec:
+        a = per.setdefault(name, [0.0, 0])
+        a[0] += tms
+        a[1] += 1
+    kern = []
+    for kt, (name, (tot, cnt)) in zip((0, 1), per.items()):
+        us = 1e3 * tot / cnt
+        b = bytes_per_site(2, 8, 18, kt) * vh
+        kern.append({"kernel": name, "type": KT_NAME[kt], "us": us, "alg_gbs": b / us / 1e3, "frac_of_measured_peak": b / us / 1e3 / peak})
+    print(json.dumps({"metric": "twisted-mass dslash GFLOPS (Eq. 2.3 operator, 48^3x96 non-degenerate fp64, 100 applications back to back)",
+                      "value": flops / (ms * 1e-3) / 1e9, "unit": "GFLOPS", "n_gpus": 1, "steps": 100, "ms_total": ms, "ms_per_application": ms / 100,
+                      "dtype": "f64", "data": "synthetic", "config": {"workload": "BASELINE.json configs[4]: 48^3x96 non-degenerate doublet, fp64, Haar links "
+                      "18-real, kappa=0.1632, mu=0.135, eps=0.17, SYM (Eq. 2.3) x 100", "lattice": list(dims), "recon": 18},
+                      "alg_gbs": byts / (ms * 1e-3) / 1e9, "frac_of_measured_peak": byts / (ms * 1e-3) / 1e9 / peak, "peak_source": peak_src,
+                      "kernels": kern, "gpu_launches": 200}))
+
+
 def run_ours(args, log):
     import torch
     rank = int(os.environ.get("RANK", "0"))
@@ -615,6 +740,7 @@ def run_ours(args, log):
     for k in kernels:
         annotate_bound(k, vh, sm_mhz)
     extra = kernels_extra(w, args, sm_mhz, peak) if (rank == 0 and world == 1 and not args.no_extra) else None
+    cg = cg_leg(w) if (rank == 0 and world == 1 and not args.no_extra and not args.sharded) else None
     if rank == 0:
         out = {"metric": METRIC, "value": value, "unit": "GFLOPS", "n_gpus": world, "steps": args.steps,
                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -625,7 +751,7 @@ def run_ours(args, log):
                           if args.sharded else ("replicas only (north_star: no sharding)" if world > 1 else "single GPU"),
                           "l2": "inputs larger than L2 (gauge fields 201-805 MB each, 2.3 GB touched per step)"},
                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-               "step_flops": step_flops, "step_alg_bytes": step_bytes, "kernels": kernels, "kernels_extra": extra,
+               "step_flops": step_flops, "step_alg_bytes": step_bytes, "kernels": kernels, "kernels_extra": extra, "cg": cg,
                "paper_table1_gflops_12real": {"%s/%s" % ("deg" if k[0] == 1 else "ndeg", PREC_NAME[k[1]]): v
                                               for k, v in PAPER_GFLOPS.items()},
                "paper_table1_gflops_8real": {"%s/%s" % ("deg" if k[0] == 1 else "ndeg", PREC_NAME[k[1]]): v
@@ -645,6 +771,10 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--ref-steps", type=int, default=5, help="--impl reference: cap on the timed full-lattice oracle steps (1.6 s each)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernels", default="", help="time single kernels alone instead: PREC:NF:RECON:KT[,...] (tuning runs; see run_kernels)")
+    ap.add_argument("--dims", default="32,32,32,64", help="--kernels: lattice extents")
+    ap.add_argument("--tune", default="", help="--kernels: tm_set_tuning overrides, key=value[,...]")
+    ap.add_argument("--config5", action="store_true", help="time BASELINE.json configs[4] instead (48^3x96 fp64 doublet, Eq. 2.3 operator x 100; ~25 GB of host memory)")
     ap.add_argument("--no-extra", action="store_true", help="skip the kernels_extra table (every kernel type x precision x compression, timed alone)")
     ap.add_argument("--sass-mix", action="store_true", help="host only: write profiles/sass_mix.csv + profiles/r2_sass_histogram.md from the built objects")
     ap.add_argument("--import-ncu", metavar="CSV", help="host only: turn an `ncu --csv --page raw` export of this build into profiles/traffic.csv")
@@ -683,6 +813,10 @@ def main():
         if rank == 0:
             sys.stderr.write("[bench] %s\n" % msg)
 
+    if args.kernels:
+        return run_kernels(args, log)
+    if args.config5:
+        return run_config5(args, log)
     if args.impl == "reference":
         if rank == 0:
             run_reference(args, log)
