@@ -18,6 +18,8 @@ const TmKernelEntry *tm_generic_table_4_2();
 const TmKernelEntry *tm_generic_table_2_1();
 const TmKernelEntry *tm_generic_table_2_2();
 
+const TmKernelEntry *tm_tile_table_2_1();
+const TmKernelEntry *tm_tile_table_2_2();
 const TmKernelEntry *tm_generic_twin_table_8_1();
 const TmKernelEntry *tm_generic_twin_table_8_2();
 const TmKernelEntry *tm_generic_twin_table_4_1();
@@ -185,6 +187,7 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->pf_dist = -1;
     c->stage = -1;
     c->z_chunks = -1;
+    c->tile_kernel = -1;
     c->block_threads = 0;
     c->sm_count = 0;
     c->basis_on = 0;
@@ -346,6 +349,11 @@ int tm_set_tuning(tm_ctx *ctx, const char *key, int value)
     if (!strcmp(key, "stage_links")) {
         if (value < -1 || value > 1) return fail(TM_ERR_ARG, "stage_links must be -1 (default), 0 or 1");
         ctx->stage = value;
+        return TM_OK;
+    }
+    if (!strcmp(key, "tile_kernel")) {
+        if (value < -1 || value > 1) return fail(TM_ERR_ARG, "tile_kernel must be -1 (default), 0 or 1");
+        ctx->tile_kernel = value;
         return TM_OK;
     }
     if (!strcmp(key, "z_chunks")) {
@@ -640,7 +648,13 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     const int kidx = (((g->recon == 18 ? 0 : g->recon == 12 ? 1 : 2) * 4 + kcode) * 2 + (dagger ? 1 : 0)) * 2 + stage;
     const TmKernelEntry *tab = (c->path == 0 && (int)prec != TM_DOUBLE) ? tm_f2_table((int)prec, out->nf) : nullptr;
     if (!tab || !tab[kidx].fn) tab = tm_generic_table((int)prec, out->nf);
-    const TmKernelEntry &k = twin ? tm_twin_table((int)prec, out->nf, c->path == 0)[((g->recon == 18 ? 0 : g->recon == 12 ? 1 : 2) * 2 + (kcode == 3 ? 1 : 0)) * 2 + (dagger ? 1 : 0)]
+    // half precision: the warp-per-tile kernel with shared-memory staged operands (tm_dslash_tile.cuh) where the lattice allows it.
+    // Measured (profiles/r2_tuning.md): 4-6 % faster than the staged thread-per-site kernel for one flavor, no faster (A) or slower (B)
+    // for the doublet, whose 26 KB of shared memory per warp leave 8 warps per SM: default for one flavor only ("tile_kernel" = 1 forces it)
+    const bool tile = (int)prec == TM_HALF && c->path == 0 && !twin && g->recon != 8 && (c->tile_kernel == 1 || (c->tile_kernel < 0 && out->nf == 1)) &&
+                      (c->g.Xh == 4 || c->g.Xh == 8 || c->g.Xh == 16) && c->g.X[1] % (32 / c->g.Xh) == 0 && c->g.Vh % 32 == 0;
+    const TmKernelEntry &k = tile ? (out->nf == 1 ? tm_tile_table_2_1() : tm_tile_table_2_2())[((g->recon == 18 ? 0 : 1) * 4 + kcode) * 2 + (dagger ? 1 : 0)]
+                           : twin ? tm_twin_table((int)prec, out->nf, c->path == 0)[((g->recon == 18 ? 0 : g->recon == 12 ? 1 : 2) * 2 + (kcode == 3 ? 1 : 0)) * 2 + (dagger ? 1 : 0)]
                                   : tab[kidx];
     cudaError_t e;
     if (c->timing) {

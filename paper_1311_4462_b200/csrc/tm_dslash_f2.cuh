@@ -193,6 +193,21 @@ TM_DEV void rows01_from8_fast(f2 *W, const float *p)
                (fmaf(a2r, r2i, -(a2i * r2r)) + fmaf(a3r, r1i, a3i * r1r)) * iN);
 }
 
+// row2[c] = conj(row0[c1] row1[c2] - row0[c2] row1[c1]),  pairs are (re, im):
+//   S = a.re*b - c.re*d ,  T = a.im*sw(b) - c.im*sw(d) ;  a*b - c*d = (S.x - T.x, S.y + T.y)
+// half: row 2 stays at raw * raw scale (32767 x the raw scale of rows 0, 1); consume_hop compensates
+TM_DEV void link_row2_f2(f2 *W)
+{
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        const f2 A = W[c1], B = W[3 + c2], C = W[c2], D = W[3 + c1];
+        const f2 S = fma2(bc2(-C.x), D, mul2(bc2(A.x), B));
+        const f2 T = fma2(bc2(-C.y), sw2(D), mul2(bc2(A.y), sw2(B)));
+        W[6 + c] = mk2(S.x - T.x, -S.y - T.y);
+    }
+}
+
 template <int PREC, int NF, int RECON>
 TM_DEV void raw_to_link(f2 *W, const HopRaw<PREC, NF, RECON> &r)
 {
@@ -223,19 +238,7 @@ TM_DEV void raw_to_link(f2 *W, const HopRaw<PREC, NF, RECON> &r)
             W[4] = cvt_pair(r.lt.x); W[5] = cvt_pair(r.lt.y);
         }
     }
-    if constexpr (RECON != 18) {
-        // row2[c] = conj(row0[c1] row1[c2] - row0[c2] row1[c1]),  pairs are (re, im):
-        //   S = a.re*b - c.re*d ,  T = a.im*sw(b) - c.im*sw(d) ;  a*b - c*d = (S.x - T.x, S.y + T.y)
-#pragma unroll
-        for (int c = 0; c < 3; c++) {
-            const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
-            const f2 A = W[c1], B = W[3 + c2], C = W[c2], D = W[3 + c1];
-            const f2 S = fma2(bc2(-C.x), D, mul2(bc2(A.x), B));
-            const f2 T = fma2(bc2(-C.y), sw2(D), mul2(bc2(A.y), sw2(B)));
-            // half: row 2 stays at raw * raw scale (32767 x the raw scale of rows 0, 1); consume_hop compensates
-            W[6 + c] = mk2(S.x - T.x, -S.y - T.y);
-        }
-    }
+    if constexpr (RECON != 18) link_row2_f2(W);
 }
 
 // ---- a3: spin projection, packed ----------------------------------------------------------------------
@@ -273,28 +276,37 @@ TM_DEV void project_f2(f2 *H, const f2 *S)
 }
 
 // ---- a5: color multiply on both spin components at once: 36 packed instructions ------------------------
+// Order: for every input colour d, the six accumulations that read H_re[d] one after the other, then the six that read H_im[d].
+// Consecutive FFMA2 then share their pair operand, which ptxas serves from the register reuse cache: an FFMA2 with three distinct
+// register sources occupies the sub-partition for 3 cycles, with a cached pair for 2 (profiles/r2_pipes.md).  The six accumulators of
+// a group are independent, and every accumulator still sums its terms in the order d = 0, 1, 2 (re, im within d): same bits as before.
 template <bool ADJ>
 TM_DEV void su3_mul_f2(f2 *G, const f2 *W, const f2 *H)
 {
+    f2 re[3], im[3];
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        float ur[3], ui[3];
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const f2 w = ADJ ? W[3 * d + c] : W[3 * c + d];
+            ur[c] = w.x;
+            ui[c] = ADJ ? -w.y : w.y;
+        }
+        const f2 hr = H[2 * d], hi = H[2 * d + 1];
+#pragma unroll
+        for (int c = 0; c < 3; c++) re[c] = (d == 0) ? mul2(bc2(ur[c]), hr) : fma2(bc2(ur[c]), hr, re[c]);
+#pragma unroll
+        for (int c = 0; c < 3; c++) im[c] = (d == 0) ? mul2(bc2(ui[c]), hr) : fma2(bc2(ui[c]), hr, im[c]);
+#pragma unroll
+        for (int c = 0; c < 3; c++) re[c] = fma2(bc2(-ui[c]), hi, re[c]);
+#pragma unroll
+        for (int c = 0; c < 3; c++) im[c] = fma2(bc2(ur[c]), hi, im[c]);
+    }
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-        f2 re, im;
-#pragma unroll
-        for (int d = 0; d < 3; d++) {
-            const f2 w = ADJ ? W[3 * d + c] : W[3 * c + d];
-            const float ur = w.x, ui = ADJ ? -w.y : w.y;
-            if (d == 0) {
-                re = mul2(bc2(ur), H[2 * d]);
-                im = mul2(bc2(ur), H[2 * d + 1]);
-            } else {
-                re = fma2(bc2(ur), H[2 * d], re);
-                im = fma2(bc2(ur), H[2 * d + 1], im);
-            }
-            re = fma2(bc2(-ui), H[2 * d + 1], re);
-            im = fma2(bc2(ui), H[2 * d], im);
-        }
-        G[2 * c] = re;
-        G[2 * c + 1] = im;
+        G[2 * c] = re[c];
+        G[2 * c + 1] = im[c];
     }
 }
 

@@ -37,6 +37,7 @@ struct tm_ctx {
     int pf_dist; // tm_set_tuning("prefetch_blocks")
     int stage;   // tm_set_tuning("stage_links"): -1 library default, 0 direct loads, 1 links staged through shared memory
     int block_threads;   // tm_set_tuning("block_threads"): 0 library default, else 32 / 64 / 128
+    int tile_kernel;     // tm_set_tuning("tile_kernel"): -1 library default (on where the geometry allows), 0 off, 1 on
     int z_chunks;        // tm_set_tuning("z_chunks"): -1 library default (from the L2 working set), else the number of z-chunks
     int sm_count;
     int basis_on;         // tm_set_host_basis: host spinors are in another spin basis, psi_device = S psi_host

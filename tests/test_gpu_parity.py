@@ -53,6 +53,7 @@ def bench_for(dims, kind, seed):
     tm.tm_set_tuning(ctx, "block_threads", 0)
     tm.tm_set_tuning(ctx, "prefetch_blocks", -1)
     tm.tm_set_tuning(ctx, "z_chunks", -1)
+    tm.tm_set_tuning(ctx, "tile_kernel", -1)
     return _cache[key]
 
 
@@ -176,6 +177,34 @@ def test_t2e_z_chunked_traversal_matches_oracle(kw, chunks, threads):
         want = oracle.matpc(inp, bench.U, po, oracle.SYM, 0)
         got = bench.matpc(inp, pg, tm.TM_MATPC_SYM, 0, tm.TM_SINGLE, tm.TM_RECON_18, nf)
         assert rel_l2(got, want) <= TOL[tm.TM_SINGLE]
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 4, 4), (16, 4, 4, 4), (16, 8, 4, 6), (32, 4, 4, 4), (32, 6, 4, 4)],
+                         ids=["Xh4-1tile-per-slab", "Xh8-1", "Xh8-2", "Xh16-2", "Xh16-3"])
+@pytest.mark.parametrize("kw", [FLAVORS[1], FLAVORS[2]], ids=["deg-", "ndeg"])
+def test_t2f_warp_per_tile_half_kernel_matches_oracle(dims, kw):
+    """The warp-per-tile half-precision kernel (tm_dslash_tile.cuh: every operand staged through shared memory, neighbours addressed
+    by slot) on the lattices it covers -- X/2 in {4, 8, 16}, one, two and three tiles per (z, t) slab, so that the y-wrap inside one
+    tile, between two tiles and across the slab are all exercised -- against the oracle: every kernel type, parity, dagger, link
+    compression; and bit-identical to the thread-per-site packed kernel (same arithmetic, different data path)."""
+    nf = nf_of(kw)
+    bench = bench_for(dims, "haar", 5)
+    po, pg = oracle.params(dims, KAPPA, **kw), tm.params(KAPPA, **kw)
+    full_in, full_x = si.spinor_field(dims, nf, 2), si.spinor_field(dims, nf, 3)
+    for parity, dagger, kt in itertools.product((0, 1), (0, 1), (0, 1, 2, 3, 4, 5)):
+        inp, x = si.mask_parity(full_in, dims, 1 - parity), si.mask_parity(full_x, dims, parity)
+        want = oracle.kernel(inp, x, bench.U, po, parity, dagger, kt) if kt < 4 else \
+            oracle.hop_xpay(inp, x, bench.U, po, parity, dagger, -KAPPA ** 2 if kt == 4 else KAPPA)
+        for recon in RECONS:
+            tm.tm_set_tuning(bench.lat.ctx, "tile_kernel", 1)          # default: on for one flavor; 1 forces it for the doublet too
+            got = bench.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, tm.TM_HALF, recon, nf)
+            assert tm.tm_last_kernel_name(bench.lat.ctx).startswith("tile<"), tm.tm_last_kernel_name(bench.lat.ctx)
+            assert rel_l2(got, want) <= TOL[tm.TM_HALF], (recon, parity, dagger, kt, rel_l2(got, want))
+            tm.tm_set_tuning(bench.lat.ctx, "tile_kernel", 0)
+            ref = bench.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, tm.TM_HALF, recon, nf)
+            assert tm.tm_last_kernel_name(bench.lat.ctx).startswith("f2")
+            assert np.array_equal(got, ref), (recon, parity, dagger, kt, np.abs(got - ref).max())
+    tm.tm_set_tuning(bench.lat.ctx, "tile_kernel", -1)
 
 
 def test_t2b_periodic_time_and_wilson_limit():
