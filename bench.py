@@ -216,14 +216,15 @@ def write_sass_mix():
     import re
     build = os.path.join(ROOT, "paper_1311_4462_b200", "csrc", "build")
     rows, md = [], []
-    for obj in sorted(glob.glob(os.path.join(build, "tm_f2_*.o")) + glob.glob(os.path.join(build, "tm_generic_*.o"))):
+    for obj in sorted(glob.glob(os.path.join(build, "tm_f2_*.o")) + glob.glob(os.path.join(build, "tm_generic_*.o")) + glob.glob(os.path.join(build, "tm_tile_*.o"))):
         txt = subprocess.run(["cuobjdump", "-sass", obj], capture_output=True, text=True).stdout
         for blk in txt.split("Function : ")[1:]:
             mangled = blk.split("\n", 1)[0].strip()
             m = re.match(r"_Z\d+tm_dslash_(f2|generic)ILi(\d)ELi(\d)ELi(\d+)ELi(\d)ELb([01])ELb([01])ELb([01])EE", mangled)
-            if not m:
+            mt = re.match(r"_Z\d+tm_dslash_(tile)ILi(\d)ELi(\d)ELi(\d+)ELi(\d)ELb([01])EE", mangled)
+            if not m and not mt:
                 continue
-            fam, prec, nf, recon, kt, dag, stg, twin = m.groups()
+            fam, prec, nf, recon, kt, dag, stg, twin = m.groups() if m else mt.groups() + ("0", "0")
             name = "%s%s%s<%s,%s,%s,%s,%s>" % (fam, "_twin" if twin == "1" else "", "_staged" if stg == "1" else "", prec, nf, recon, kt,
                                               "dagger" if dag == "1" else "plain")
             hist = {}
@@ -268,10 +269,12 @@ def import_ncu(csv_path):
         if len(row) != len(hdr) or not row[0].isdigit():
             continue
         d = dict(zip(hdr, row))
-        m = re.search(r"tm_dslash_(f2|generic)<(\d), (\d), (\d+), (\d), (\w+), (\w+)(?:, (\w+))?>", d["Kernel Name"].replace("(int)", "").replace("(bool)", ""))
-        if not m:
+        kn = d["Kernel Name"].replace("(int)", "").replace("(bool)", "")
+        m = re.search(r"tm_dslash_(f2|generic)<(\d), (\d), (\d+), (\d), (\w+), (\w+)(?:, (\w+))?>", kn)
+        mt = re.search(r"tm_dslash_(tile)<(\d), (\d), (\d+), (\d), (\w+)>", kn)
+        if not m and not mt:
             continue
-        fam, prec, nf, recon, kt, dag, stg, twin = m.groups()
+        fam, prec, nf, recon, kt, dag, stg, twin = m.groups() if m else mt.groups() + ("0", "0")
         name = "%s%s%s<%s,%s,%s,%s,%s>" % (fam, "_twin" if twin in ("1", "true") else "", "_staged" if stg in ("1", "true") else "", prec, nf, recon, kt,
                                           "dagger" if dag in ("1", "true") else "plain")
         try:
