@@ -153,15 +153,17 @@ def reduce_over_ranks(ms_local, world):
     return float(t.item())
 
 
+KERNEL_SOURCES = ("tm_dslash.cuh", "tm_dslash_f2.cuh", "tm_dslash_tile.cuh", "tm_layout.cuh", "tm_f2.cuh", "tm_stream.cuh")
+
+
 def source_hash():
-    """sha256 (12 hex digits) over the kernel sources: ties the stored ncu traffic / SASS mix to the build being timed."""
-    import glob
+    """sha256 (12 hex digits) over the fused-dslash kernel sources: ties the stored ncu traffic / SASS mix to the kernels being timed."""
     import hashlib
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_1311_4462_b200", "csrc")
-    for f in sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh")) + glob.glob(os.path.join(csrc, "*.h"))):
-        h.update(os.path.basename(f).encode())
-        h.update(open(f, "rb").read())
+    for name in KERNEL_SOURCES:
+        h.update(name.encode())
+        h.update(open(os.path.join(csrc, name), "rb").read())
     return h.hexdigest()[:12]
 
 
@@ -333,28 +335,34 @@ class Workload:
             self.mat_pc((nf, prec), nf, typ, dagger)
 
     def make_pinned(self):
+        """Pinned host buffers in the precision a user of that field precision holds: double for fp64 fields, float for fp32 / half."""
         torch = self.torch
         self.pin_in, self.pin_out = {}, {}
         for nf in (1, 2):
             n = nf * self.vh * 24
-            a = torch.empty(n, dtype=torch.float64, pin_memory=True)
-            a.numpy()[:] = self.host_in[nf].view(np.float64).reshape(-1)
-            self.pin_in[nf] = a
-            self.pin_out[nf] = torch.empty(n, dtype=torch.float64, pin_memory=True)
+            for dt, key in ((torch.float64, 8), (torch.float32, 4)):
+                a = torch.empty(n, dtype=dt, pin_memory=True)
+                a.numpy()[:] = self.host_in[nf].view(np.float64).reshape(-1)
+                self.pin_in[(nf, key)] = a
+                self.pin_out[(nf, key)] = torch.empty(n, dtype=dt, pin_memory=True)
 
     def step_e2e(self):
         """The same step through the C-ABI with HOST buffers: upload in_e, tm_mat_pc, download out_e, per composite.
         The asynchronous entry points overlap the H2D copy of the next input, the kernels and the D2H copy of the
-        previous result; tm_sync at the end of the step: every result of the step is on the host when it returns."""
+        previous result; tm_sync at the end of the step: every result of the step is on the host when it returns.
+        fp64 fields travel as double arrays, fp32 and half fields as float arrays (tm_field_upload_cb_async_f32)."""
         tm = self.tm
         h2d = d2h = 0
         for nf, prec, typ, dagger in step_ops():
             key = (nf, prec)
-            tm.tm_field_upload_cb_async(self.fin[key].h, 0, self.pin_in[nf].data_ptr())
+            hk = (nf, 8 if prec == 8 else 4)
+            up, down = (tm.tm_field_upload_cb_async, tm.tm_field_download_cb_async) if prec == 8 else \
+                (tm.tm_field_upload_cb_async_f32, tm.tm_field_download_cb_async_f32)
+            up(self.fin[key].h, 0, self.pin_in[hk].data_ptr())
             self.mat_pc(key, nf, typ, dagger)
-            tm.tm_field_download_cb_async(self.fout[key].h, 0, self.pin_out[nf].data_ptr())
-            h2d += self.pin_in[nf].numel() * 8
-            d2h += self.pin_out[nf].numel() * 8
+            down(self.fout[key].h, 0, self.pin_out[hk].data_ptr())
+            h2d += self.pin_in[hk].numel() * self.pin_in[hk].element_size()
+            d2h += self.pin_out[hk].numel() * self.pin_out[hk].element_size()
         self.lat.sync()
         return h2d, d2h
 
@@ -720,7 +728,7 @@ def run_ours(args, log):
     e2e_ms = reduce_over_ranks(max(ev0.elapsed_time(ev1), 1e3 * (time.time() - tw0)), world) / e2e_steps
     e2e = {"value": world * step_flops / (e2e_ms * 1e-3) / 1e9, "unit": "GFLOPS", "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps,
-           "note": "per composite: tm_field_upload_cb_async (pinned host, fp64 canonical) + tm_mat_pc + tm_field_download_cb_async, "
+           "note": "per composite: tm_field_upload_cb_async (pinned host arrays: double for fp64 fields, float for fp32 / half fields) + tm_mat_pc + tm_field_download_cb_async, "
                    "tm_sync per step; copies in both directions overlap each other and the kernels"}
 
     # ---- CPU baseline: the oracle as it stands, on this box's host cores (rank 0, N = 1 only)
@@ -768,8 +776,8 @@ def run_ours(args, log):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--ref-steps", type=int, default=5, help="--impl reference: cap on the timed full-lattice oracle steps (1.6 s each)")

@@ -124,6 +124,11 @@ int tm_field_download_cb(const tm_field *f, tm_parity parity, double *host_cb);
  * Consecutive transfers in the same direction run in issue order.                                                        */
 int tm_field_upload_cb_async(tm_field *f, tm_parity parity, const double *host_cb);
 int tm_field_download_cb_async(const tm_field *f, tm_parity parity, double *host_cb);
+/* The same with the host array in SINGLE precision (same index order, float instead of double): half the bytes over PCIe for
+ * fields whose device precision is single or half anyway (the conversion to the field's format happens in the pack kernel on
+ * the device; a double field takes float input too, with float accuracy). */
+int tm_field_upload_cb_async_f32(tm_field *f, tm_parity parity, const float *host_cb);
+int tm_field_download_cb_async_f32(const tm_field *f, tm_parity parity, float *host_cb);
 
 /* ---- host spin basis (SURVEY.md section 8f "minor": chiral <-> non-relativistic rotation in the pack kernels) ---- */
 /* The kernels work in the non-relativistic basis of PAPER.md:52 (gamma_4 diagonal; reading C5), which is also

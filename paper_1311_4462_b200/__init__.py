@@ -32,7 +32,7 @@ TM_BASIS_NONREL, TM_BASIS_CHIRAL, TM_BASIS_CUSTOM = 0, 1, 2
 
 EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
-    "tm_field_device_ptr", "tm_set_host_basis", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb", "tm_field_upload_cb_async", "tm_field_download_cb_async",
+    "tm_field_device_ptr", "tm_set_host_basis", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb", "tm_field_upload_cb_async", "tm_field_download_cb_async", "tm_field_upload_cb_async_f32", "tm_field_download_cb_async_f32",
     "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_twist_apply",
     "tm_prepare_rhs", "tm_set_open_time", "tm_set_open_dirs", "tm_halo_bytes", "tm_halo_pack", "tm_halo_apply", "tm_field_axpby", "tm_field_redot", "tm_invert_cg", "tm_cg_release", "tm_set_allreduce", "tm_last_error",
     "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_set_tuning", "tm_timing_enable", "tm_timing_read",
@@ -97,7 +97,7 @@ def lib():
     L.tm_field_device_ptr.argtypes = [vp]
     L.tm_field_device_ptr.restype = vp
     for name in ("tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb",
-                 "tm_field_upload_cb_async", "tm_field_download_cb_async"):
+                 "tm_field_upload_cb_async", "tm_field_download_cb_async", "tm_field_upload_cb_async_f32", "tm_field_download_cb_async_f32"):
         getattr(L, name).argtypes = [vp, i, vp]
     L.tm_gauge_load.argtypes = [vp, vp, i, i, ctypes.POINTER(vp)]
     L.tm_gauge_free.argtypes = [vp]
@@ -210,6 +210,17 @@ def tm_field_upload_cb_async(f, parity, host_cb):
 def tm_field_download_cb_async(f, parity, host_cb):
     ptr = host_cb if isinstance(host_cb, int) else host_cb.ctypes.data
     _check(lib().tm_field_download_cb_async(f, int(parity), ctypes.c_void_p(ptr)))
+
+
+def tm_field_upload_cb_async_f32(f, parity, host_cb):
+    """The same from a float32 host array (address of PINNED memory or a numpy array backed by it)."""
+    ptr = host_cb if isinstance(host_cb, int) else host_cb.ctypes.data
+    _check(lib().tm_field_upload_cb_async_f32(f, int(parity), ctypes.c_void_p(ptr)))
+
+
+def tm_field_download_cb_async_f32(f, parity, host_cb):
+    ptr = host_cb if isinstance(host_cb, int) else host_cb.ctypes.data
+    _check(lib().tm_field_download_cb_async_f32(f, int(parity), ctypes.c_void_p(ptr)))
 
 
 def tm_gauge_load(ctx, host_links, prec, recon):

@@ -423,7 +423,7 @@ static int field_upload(tm_field *f, int parity, const double *host, bool cb)
     if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
     e = cudaMemcpyAsync(st.p, host, n, cudaMemcpyHostToDevice, c->stream);
     if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync H2D");
-    e = tm_pack_spinor(f, parity, static_cast<const double *>(st.p), cb, c->stream);
+    e = tm_pack_spinor(f, parity, st.p, 8, cb, c->stream);
     if (e != cudaSuccess) return cuda_fail(e, "pack_spinor launch");
     e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return cuda_fail(e, "upload sync");
@@ -444,7 +444,7 @@ static int field_download(const tm_field *f, int parity, double *host, bool cb)
         e = cudaMemcpyAsync(st.p, host, n, cudaMemcpyHostToDevice, c->stream);
         if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync H2D");
     }
-    e = tm_unpack_spinor(f, parity, static_cast<double *>(st.p), cb, c->stream);
+    e = tm_unpack_spinor(f, parity, st.p, 8, cb, c->stream);
     if (e != cudaSuccess) return cuda_fail(e, "unpack_spinor launch");
     e = cudaMemcpyAsync(host, st.p, n, cudaMemcpyDeviceToHost, c->stream);
     if (e != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync D2H");
@@ -479,7 +479,7 @@ static cudaError_t grow(void **p, size_t *have, size_t need, cudaStream_t owner)
     return e;
 }
 
-int tm_field_upload_cb_async(tm_field *f, tm_parity parity, const double *host_cb)
+static int upload_cb_async(tm_field *f, tm_parity parity, const void *host_cb, int host_prec)
 {
     if (!f || !host_cb) return fail(TM_ERR_ARG, "tm_field_upload_cb_async: NULL argument");
     if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
@@ -487,7 +487,7 @@ int tm_field_upload_cb_async(tm_field *f, tm_parity parity, const double *host_c
     TM_USE_DEVICE(c);
     int rc = async_setup(c);
     if (rc) return rc;
-    const size_t n = (size_t)f->nf * (size_t)c->g.Vh * 24 * sizeof(double);
+    const size_t n = (size_t)f->nf * (size_t)c->g.Vh * 24 * (size_t)host_prec;
     cudaError_t e = grow(&c->up_staging, &c->up_bytes, n, c->up_stream);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
     // H2D copy: free to run now (the staging buffer is ordered by the upload stream itself)
@@ -495,14 +495,14 @@ int tm_field_upload_cb_async(tm_field *f, tm_parity parity, const double *host_c
     // the pack kernel overwrites f: it waits for every kernel already queued on the context stream (they may read f)
     if ((e = cudaEventRecord(c->ev_compute, c->stream)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     if ((e = cudaStreamWaitEvent(c->up_stream, c->ev_compute, 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
-    if ((e = tm_pack_spinor(f, (int)parity, static_cast<const double *>(c->up_staging), true, c->up_stream)) != cudaSuccess) return cuda_fail(e, "pack_spinor launch");
+    if ((e = tm_pack_spinor(f, (int)parity, c->up_staging, host_prec, true, c->up_stream)) != cudaSuccess) return cuda_fail(e, "pack_spinor launch");
     // later kernels of the context stream see the uploaded field
     if ((e = cudaEventRecord(c->ev_up, c->up_stream)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     if ((e = cudaStreamWaitEvent(c->stream, c->ev_up, 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
     return TM_OK;
 }
 
-int tm_field_download_cb_async(const tm_field *f, tm_parity parity, double *host_cb)
+static int download_cb_async(const tm_field *f, tm_parity parity, void *host_cb, int host_prec)
 {
     if (!f || !host_cb) return fail(TM_ERR_ARG, "tm_field_download_cb_async: NULL argument");
     if (parity != TM_EVEN && parity != TM_ODD) return fail(TM_ERR_ARG, "bad parity %d", (int)parity);
@@ -510,19 +510,24 @@ int tm_field_download_cb_async(const tm_field *f, tm_parity parity, double *host
     TM_USE_DEVICE(c);
     int rc = async_setup(c);
     if (rc) return rc;
-    const size_t n = (size_t)f->nf * (size_t)c->g.Vh * 24 * sizeof(double);
+    const size_t n = (size_t)f->nf * (size_t)c->g.Vh * 24 * (size_t)host_prec;
     cudaError_t e = grow(&c->down_staging, &c->down_bytes, n, c->down_stream);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(TM_ERR_NOMEM, "staging cudaMalloc(%zu): %s", n, cudaGetErrorString(e)); }
     // the unpack kernel reads f after everything queued on the context stream so far
     if ((e = cudaEventRecord(c->ev_compute, c->stream)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     if ((e = cudaStreamWaitEvent(c->down_stream, c->ev_compute, 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
-    if ((e = tm_unpack_spinor(f, (int)parity, static_cast<double *>(c->down_staging), true, c->down_stream)) != cudaSuccess) return cuda_fail(e, "unpack_spinor launch");
+    if ((e = tm_unpack_spinor(f, (int)parity, c->down_staging, host_prec, true, c->down_stream)) != cudaSuccess) return cuda_fail(e, "unpack_spinor launch");
     // later kernels of the context stream may overwrite f once it has been unpacked; the D2H copy itself overlaps them
     if ((e = cudaEventRecord(c->ev_down, c->down_stream)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
     if ((e = cudaStreamWaitEvent(c->stream, c->ev_down, 0)) != cudaSuccess) return cuda_fail(e, "cudaStreamWaitEvent");
     if ((e = cudaMemcpyAsync(host_cb, c->down_staging, n, cudaMemcpyDeviceToHost, c->down_stream)) != cudaSuccess) return cuda_fail(e, "cudaMemcpyAsync D2H");
     return TM_OK;
 }
+
+int tm_field_upload_cb_async(tm_field *f, tm_parity parity, const double *host_cb) { return upload_cb_async(f, parity, host_cb, 8); }
+int tm_field_download_cb_async(const tm_field *f, tm_parity parity, double *host_cb) { return download_cb_async(f, parity, host_cb, 8); }
+int tm_field_upload_cb_async_f32(tm_field *f, tm_parity parity, const float *host_cb) { return upload_cb_async(f, parity, host_cb, 4); }
+int tm_field_download_cb_async_f32(const tm_field *f, tm_parity parity, float *host_cb) { return download_cb_async(f, parity, host_cb, 4); }
 
 int tm_field_upload(tm_field *f, tm_parity parity, const double *host_full) { return field_upload(f, parity, host_full, false); }
 int tm_field_download(const tm_field *f, tm_parity parity, double *host_full) { return field_download(f, parity, host_full, false); }

@@ -192,6 +192,7 @@ cudaError_t tm_launch_halo_apply(tm_field *out, const void *from_prev, const voi
 
 // pack / unpack (tm_pack.cu)
 // (both apply the context's host spin basis: S on the way in, S^dag on the way out)
-cudaError_t tm_pack_spinor(const tm_field *f, int parity, const double *dev_src, bool src_is_cb, cudaStream_t s);
-cudaError_t tm_unpack_spinor(const tm_field *f, int parity, double *dev_dst, bool dst_is_cb, cudaStream_t s);
+// host_prec: 8 = double arrays (the canonical form), 4 = float arrays
+cudaError_t tm_pack_spinor(const tm_field *f, int parity, const void *dev_src, int host_prec, bool src_is_cb, cudaStream_t s);
+cudaError_t tm_unpack_spinor(const tm_field *f, int parity, void *dev_dst, int host_prec, bool dst_is_cb, cudaStream_t s);
 cudaError_t tm_pack_gauge(const tm_gauge *g, const double *dev_src, cudaStream_t s);

@@ -49,17 +49,18 @@ __device__ __forceinline__ long cb_to_lex(const PackGeom &g, int i, int parity)
     return 2L * i + ((y + z + t + parity) & 1);      // lex / 2 == i, x1 parity fixed by the row
 }
 
-template <int PREC>
-__global__ void pack_spinor_kernel(char *dst, const double *src, PackGeom g, int parity, int nf, bool src_is_cb, SpinRot rot)
+// HT = the host array's real type: double (the canonical form) or float (tm_field_upload_cb_async_f32: half the PCIe bytes)
+template <int PREC, typename HT>
+__global__ void pack_spinor_kernel(char *dst, const HT *src, PackGeom g, int parity, int nf, bool src_is_cb, SpinRot rot)
 {
     typedef typename PrecTraits<PREC>::real real;
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= nf * g.Vh) return;
     const int f = tid / g.Vh, i = tid % g.Vh;
-    const double *s = src_is_cb ? src + ((size_t)f * g.Vh + i) * 24 : src + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
+    const HT *s = src_is_cb ? src + ((size_t)f * g.Vh + i) * 24 : src + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
     double d[24];
 #pragma unroll
-    for (int k = 0; k < 24; k++) d[k] = s[k];
+    for (int k = 0; k < 24; k++) d[k] = (double)s[k];
     if (rot.on) spin_rotate<false>(d, rot);
     real v[24];
 #pragma unroll
@@ -67,8 +68,8 @@ __global__ void pack_spinor_kernel(char *dst, const double *src, PackGeom g, int
     store_spinor<PREC>(v, dst + spinor_site_off(PREC, nf, i, f), i & (TM_TILE - 1));
 }
 
-template <int PREC>
-__global__ void unpack_spinor_kernel(double *dst, const char *src, PackGeom g, int parity, int nf, bool dst_is_cb, SpinRot rot)
+template <int PREC, typename HT>
+__global__ void unpack_spinor_kernel(HT *dst, const char *src, PackGeom g, int parity, int nf, bool dst_is_cb, SpinRot rot)
 {
     typedef typename PrecTraits<PREC>::real real;
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -76,13 +77,13 @@ __global__ void unpack_spinor_kernel(double *dst, const char *src, PackGeom g, i
     const int f = tid / g.Vh, i = tid % g.Vh;
     real v[24];
     load_spinor<PREC, 0>(v, src + spinor_site_off(PREC, nf, i, f), i & (TM_TILE - 1));
-    double *d = dst_is_cb ? dst + ((size_t)f * g.Vh + i) * 24 : dst + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
+    HT *d = dst_is_cb ? dst + ((size_t)f * g.Vh + i) * 24 : dst + ((size_t)f * g.V + cb_to_lex(g, i, parity)) * 24;
     double o[24];
 #pragma unroll
     for (int k = 0; k < 24; k++) o[k] = (double)v[k];
     if (rot.on) spin_rotate<true>(o, rot);
 #pragma unroll
-    for (int k = 0; k < 24; k++) d[k] = o[k];
+    for (int k = 0; k < 24; k++) d[k] = (HT)o[k];
 }
 
 // one thread per (parity, mu, cb site): U_mu(x) for x of that parity
@@ -164,27 +165,29 @@ PackGeom geom_of(const tm_ctx *c)
 
 }  // namespace
 
-cudaError_t tm_pack_spinor(const tm_field *f, int parity, const double *dev_src, bool src_is_cb, cudaStream_t s)
+cudaError_t tm_pack_spinor(const tm_field *f, int parity, const void *dev_src, int host_prec, bool src_is_cb, cudaStream_t s)
 {
     const PackGeom g = geom_of(f->ctx);
     const SpinRot rot = rot_of(f->ctx);
     const int n = f->nf * g.Vh, threads = 128, blocks = (n + threads - 1) / threads;
     char *dst = static_cast<char *>(f->ptr);
-    if (f->prec == 8) pack_spinor_kernel<8><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb, rot);
-    else if (f->prec == 4) pack_spinor_kernel<4><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb, rot);
-    else pack_spinor_kernel<2><<<blocks, threads, 0, s>>>(dst, dev_src, g, parity, f->nf, src_is_cb, rot);
+#define TM_PS(P, HT) pack_spinor_kernel<P, HT><<<blocks, threads, 0, s>>>(dst, static_cast<const HT *>(dev_src), g, parity, f->nf, src_is_cb, rot)
+    if (host_prec == 8) { if (f->prec == 8) TM_PS(8, double); else if (f->prec == 4) TM_PS(4, double); else TM_PS(2, double); }
+    else { if (f->prec == 8) TM_PS(8, float); else if (f->prec == 4) TM_PS(4, float); else TM_PS(2, float); }
+#undef TM_PS
     return cudaGetLastError();
 }
 
-cudaError_t tm_unpack_spinor(const tm_field *f, int parity, double *dev_dst, bool dst_is_cb, cudaStream_t s)
+cudaError_t tm_unpack_spinor(const tm_field *f, int parity, void *dev_dst, int host_prec, bool dst_is_cb, cudaStream_t s)
 {
     const PackGeom g = geom_of(f->ctx);
     const SpinRot rot = rot_of(f->ctx);
     const int n = f->nf * g.Vh, threads = 128, blocks = (n + threads - 1) / threads;
     const char *src = static_cast<const char *>(f->ptr);
-    if (f->prec == 8) unpack_spinor_kernel<8><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb, rot);
-    else if (f->prec == 4) unpack_spinor_kernel<4><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb, rot);
-    else unpack_spinor_kernel<2><<<blocks, threads, 0, s>>>(dev_dst, src, g, parity, f->nf, dst_is_cb, rot);
+#define TM_US(P, HT) unpack_spinor_kernel<P, HT><<<blocks, threads, 0, s>>>(static_cast<HT *>(dev_dst), src, g, parity, f->nf, dst_is_cb, rot)
+    if (host_prec == 8) { if (f->prec == 8) TM_US(8, double); else if (f->prec == 4) TM_US(4, double); else TM_US(2, double); }
+    else { if (f->prec == 8) TM_US(8, float); else if (f->prec == 4) TM_US(4, float); else TM_US(2, float); }
+#undef TM_US
     return cudaGetLastError();
 }
 

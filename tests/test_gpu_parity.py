@@ -124,6 +124,36 @@ def test_t1b_async_transfers_overlap_safely():
             assert np.array_equal(got, want[k]), (PREC_NAME[prec], k)
 
 
+def test_t1c_float_host_arrays_round_trip():
+    """tm_field_upload_cb_async_f32 / tm_field_download_cb_async_f32: float host arrays (half the PCIe bytes for single and half
+    fields).  Round trip: exact for a single field, float rounding for a double field, 1/2 LSB of the site norm for a half field;
+    and the uploaded field equals the one uploaded from the double array (single, half: bit for bit)."""
+    import torch
+    dims, nf = (6, 6, 6, 6), 2
+    lat = tm.Lattice(dims)
+    vh = lat.Vh
+    x = si.to_parity(si.spinor_field(dims, nf, 9), dims, 0)
+    x32 = x.view(np.float64).astype(np.float32)
+    pin = torch.empty(x32.size, dtype=torch.float32, pin_memory=True)
+    pin.numpy()[:] = x32.reshape(-1)
+    back = torch.zeros(x32.size, dtype=torch.float32, pin_memory=True)
+    for prec in PRECS:
+        f, fd = lat.field(prec, nf), lat.field(prec, nf)
+        tm.tm_field_upload_cb_async_f32(f.h, 0, pin.data_ptr())
+        tm.tm_field_download_cb_async_f32(f.h, 0, back.data_ptr())
+        lat.sync()
+        got = back.numpy().reshape(nf, vh, 24)
+        want = x32.reshape(nf, vh, 24)
+        if prec == tm.TM_HALF:
+            lsb = np.abs(got - want) / (np.abs(want).max(axis=2, keepdims=True) / 32767.0)
+            assert lsb.max() <= 0.51, lsb.max()
+        else:
+            assert np.array_equal(got, want)
+        fd.upload_cb(0, x32.astype(np.float64).view(np.complex128).reshape(nf, vh, 4, 3))      # the same values through the double entry point
+        lat.sync()
+        assert bool((f.storage == fd.storage).all()), prec
+
+
 # ---- T2: every kernel variant vs the oracle -------------------------------------------------------
 
 @pytest.mark.parametrize("dims,kind", [((4, 4, 4, 8), "haar"), ((4, 6, 8, 10), "near_identity"), ((8, 4, 6, 4), "haar"),
