@@ -8,6 +8,8 @@
 #define ITER 512
 typedef unsigned long long u64;
 __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+// d = (s, s) * b + c with the scalar broadcast operand the kernels use (SASS: FFMA2 Rd, Rs.F32, Rb.F32x2, Rc.F32x2)
+__device__ __forceinline__ u64 fma2s(float s, u64 b, u64 c) { u64 d; asm volatile("{.reg .b64 t; mov.b64 t, {%1, %1}; fma.rn.f32x2 %0, t, %2, %3;}" : "=l"(d) : "f"(s), "l"(b), "l"(c)); return d; }
 __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t s) { uint32_t d; asm volatile("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(s)); return d; }
 __device__ __forceinline__ float i2f_lo(uint32_t w) { float f; asm volatile("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f32.s16 %0, l;}" : "=f"(f) : "r"(w)); return f; }
 __device__ __forceinline__ float i2f_hi(uint32_t w) { float f; asm volatile("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f32.s16 %0, h;}" : "=f"(f) : "r"(w)); return f; }
@@ -20,7 +22,7 @@ __device__ __forceinline__ uint32_t lop(uint32_t a, uint32_t b, uint32_t c) { ui
 template <int T> __global__ void __launch_bounds__(512, 1) kern(u64 *cyc, float *sink, const uint32_t *in)
 {
     u64 a[8]; uint32_t r[8]; float f[8];
-    for (int i = 0; i < 8; i++) { a[i] = ((u64)in[i] << 32) | in[i + 8]; r[i] = in[16 + i] + threadIdx.x; f[i] = 0.f; }
+    for (int i = 0; i < 8; i++) { a[i] = ((u64)in[i] << 32) | in[i + 8]; r[i] = in[16 + i] + threadIdx.x; f[i] = (T >= 16 && T <= 18) ? __uint_as_float(in[40 + i]) : 0.f; }
     const u64 b = ((u64)in[24] << 32) | in[25], c = ((u64)in[26] << 32) | in[27];
     const u64 b2 = ((u64)in[28] << 32) | in[29], c2 = ((u64)in[30] << 32) | in[31];
     const uint32_t m = in[32], s = in[33];
@@ -73,6 +75,15 @@ template <int T> __global__ void __launch_bounds__(512, 1) kern(u64 *cyc, float 
         } else if constexpr (T == 14) {    // LOP3 x8
 #pragma unroll
             for (int i = 0; i < 8; i++) r[i] = lop(r[i], m, s);
+        } else if constexpr (T == 16) {    // the kernels' form, nothing shared: scalar x pair + accumulator pair, all distinct
+#pragma unroll
+            for (int i = 0; i < 8; i++) a[i] = fma2s(f[i], a[(i + 3) & 7], a[i]);
+        } else if constexpr (T == 17) {    // the same scalar in all 8 (reuse of the scalar operand)
+#pragma unroll
+            for (int i = 0; i < 8; i++) a[i] = fma2s(f[0], a[(i + 3) & 7], a[i]);
+        } else if constexpr (T == 18) {    // the same pair in all 8, distinct scalars (reuse of the pair operand)
+#pragma unroll
+            for (int i = 0; i < 8; i++) a[i] = fma2s(f[i], b, a[i]);
         } else if constexpr (T == 15) {    // FFMA2 alternating two operand sets + I2F 4:1
 #pragma unroll
             for (int i = 0; i < 8; i++) { a[i] = fma2(a[i], (i & 1) ? b : b2, (i & 2) ? c : c2); if ((i & 3) == 3) r[i] = __float_as_uint(i2f_hi(r[i])); }
@@ -100,10 +111,14 @@ int main()
 {
     u64 *cyc; float *sink; uint32_t *in;
     cudaMalloc(&cyc, 148 * 8); cudaMalloc(&sink, 148 * 512 * 4); cudaMalloc(&in, 64 * 4);
-    uint32_t h[64]; for (int i = 0; i < 64; i++) h[i] = 0x3f800000u + i * 12345u; h[32] = 0x4B000000u; h[33] = 0x7610;
+    uint32_t h[64]; for (int i = 0; i < 64; i++) h[i] = 0x3f800000u + i * 12345u;
+    for (int i = 40; i < 48; i++) h[i] = 0x3f000000u + i * 77u;     // scalars ~0.5: the chains stay finite h[32] = 0x4B000000u; h[33] = 0x7610;
     cudaMemcpy(in, h, sizeof(h), cudaMemcpyHostToDevice);
     run<0>("FFMA2", 8, cyc, sink, in);
     run<10>("FFMA2 3 distinct regs", 8, cyc, sink, in);
+    run<16>("FFMA2 scalar x pair + pair, distinct", 8, cyc, sink, in);
+    run<17>("FFMA2 scalar x pair + pair, same scalar", 8, cyc, sink, in);
+    run<18>("FFMA2 scalar x pair + pair, same pair", 8, cyc, sink, in);
     run<12>("FFMA scalar", 8, cyc, sink, in);
     run<1>("PRMT", 8, cyc, sink, in);
     run<14>("LOP3", 8, cyc, sink, in);
