@@ -463,7 +463,8 @@ def time_alone(fn, sync, launches=20, reps=3):
 
 def kernels_extra(w, args, sm_mhz, peak):
     """Every (kernel type x precision x flavors x link compression) of the library, each timed ALONE in this run (20 launches
-    between two CUDA events, best of 3) at 32^3x64 through tm_dslash_apply -- outside `value`, whose step stays BASELINE.json's.
+    between two CUDA events, best of 3, 50 ms of idle before each kernel) at 32^3x64 through tm_dslash_apply -- outside `value`, whose step
+    stays BASELINE.json's.
     Rows: 12- / 18- / 8-real x fp64 / fp32 / half x degenerate / doublet x A / A-xpay / B / REC, and the Wilson limit
     (mu = eps = 0: the paper's Table 1 Wilson column) of kernel A."""
     tm, lat, vh = w.tm, w.lat, w.vh
@@ -489,6 +490,7 @@ def kernels_extra(w, args, sm_mhz, peak):
                     if label == "A wilson" and (nf == 2 or recon != 12):
                         continue
                     p = wilson if label == "A wilson" else w.params[nf]
+                    time.sleep(0.05)         # "alone": not on top of the power / thermal state the previous kernel's launches left behind
                     us = time_alone(lambda: tm.dslash_apply(fout, fin, None if kt == 0 else fx, g, p, 1, 0, kt), lat.sync)
                     b = bytes_per_site(nf, prec, recon, kt) * vh
                     f = flops_per_site(nf, kt) * vh

@@ -627,7 +627,10 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     a.wrap_z = (c->open_mask & 4) ? 0.f : 1.f;
     // measured defaults (profiles/): the fp64 doublet kernels with 12-real links gain from an L2 prefetch 8 tiles ahead, the half
     // kernels from staging the link stream through shared memory; everything else runs plain
-    a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : ((int)prec == TM_DOUBLE && out->nf == 2 && g->recon == 12 ? 8 : 0);
+    // L2 prefetch of the tiles 8 blocks ahead (tm_stream.cuh), where it measured faster at both 32^3 x 64 and 48^3 x 96 (profiles/r2_tuning.md
+    // section 5): the fp32 doublet kernels (+6..11 %), the fp64 kernels without an x input (+2..5 %), the fp64 doublet with 12-real links
+    const bool pf_on = ((int)prec == TM_SINGLE && out->nf == 2) || ((int)prec == TM_DOUBLE && (kcode == 0 || (out->nf == 2 && g->recon == 12)));
+    a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : (pf_on ? 8 : 0);
     int stage = c->stage >= 0 ? c->stage : ((int)prec == TM_HALF ? 1 : 0);
     a.block_threads = c->block_threads ? c->block_threads : 128;
     if (g->recon == 8 || twin) stage = 0;        // 8-real links and the D R^-1 kernels: direct loads
