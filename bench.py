@@ -168,8 +168,8 @@ def source_hash():
 
 
 def read_profile_table(fname):
-    """profiles/<fname>: '# source_hash=<h> ...' header, then 'kernel;v1;v2...' rows -> (hash or None, {kernel: [floats]})."""
-    path = os.path.join(ROOT, "profiles", fname)
+    """profiles/<fname> (or an absolute path): '# source_hash=<h> ...' header, then 'kernel;v1;v2...' rows -> (hash or None, {kernel: [floats]})."""
+    path = fname if os.path.isabs(fname) else os.path.join(ROOT, "profiles", fname)
     rows, h = {}, None
     if not os.path.exists(path):
         return None, rows
@@ -256,7 +256,7 @@ def write_sass_mix():
     print("wrote profiles/sass_mix.csv (%d kernels), profiles/r2_sass_histogram.md" % len(rows))
 
 
-def import_ncu(csv_path):
+def import_ncu(csv_path, out_path=None):
     """--import-ncu FILE: an `ncu --csv --page raw` export (metrics dram__bytes_read.sum, dram__bytes_write.sum) of THIS build
     -> profiles/traffic.csv with the source hash, mean per launch and kernel."""
     import csv
@@ -287,7 +287,7 @@ def import_ncu(csv_path):
         a[0] += b
         a[1] += 1
     commit = subprocess.run(["git", "-C", ROOT, "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip()
-    with open(os.path.join(ROOT, "profiles", "traffic.csv"), "w") as f:
+    with open(out_path or os.path.join(ROOT, "profiles", "traffic.csv"), "w") as f:
         f.write("# source_hash=%s parent_commit=%s  kernel ; DRAM bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, mean over "
                 "the captured launches; written by `python bench.py --import-ncu %s`)\n" % (source_hash(), commit, os.path.basename(csv_path)))
         for name, (tot, n) in sorted(acc.items()):

@@ -95,3 +95,45 @@ def test_reference_arm_other_ranks_do_no_work(monkeypatch, capsys):
     monkeypatch.setattr(sys, "argv", ["bench.py", "--impl", "reference", "--steps", "1", "--warmup", "0"])
     bench.main()
     assert capsys.readouterr().out == ""
+
+
+def test_ncu_import_ties_the_traffic_to_the_kernel_sources(tmp_path):
+    """`bench.py --import-ncu`: an `ncu --page raw --csv` export (header row, units row, one row per launch) becomes the table
+    bench.py reads for roofline.traffic: bytes scaled by the unit column, launches of one kernel averaged, template arguments mapped
+    to the library's kernel names, and the hash of the kernel sources recorded so that a stale table reads as None."""
+    src = tmp_path / "raw.csv"
+    hdr = ["ID", "Kernel Name", "dram__bytes_read.sum", "dram__bytes_write.sum", "gpu__time_duration.sum"]
+    rows = [hdr, ["", "", "Gbyte", "Mbyte", "us"],
+            ["0", "void tm_dslash_generic<(int)8, (int)1, (int)12, (int)0, (bool)0, (bool)0, (bool)0>(DslashArgs)", "1.0", "200.0", "190"],
+            ["1", "void tm_dslash_generic<(int)8, (int)1, (int)12, (int)0, (bool)0, (bool)0, (bool)0>(DslashArgs)", "1.2", "200.0", "190"],
+            ["2", "void tm_dslash_f2<(int)2, (int)2, (int)12, (int)2, (bool)1, (bool)1, (bool)0>(DslashArgs)", "300.0", "100.0", "120"],
+            ["3", "void tm_dslash_tile<(int)2, (int)1, (int)12, (int)1, (bool)0>(DslashArgs, TileGeom)", "0.25", "50.0", "70"],
+            ["4", "void tm_dslash_f2<(int)4, (int)1, (int)12, (int)3, (bool)0, (bool)0, (bool)1>(DslashArgs)", "0.5", "100.0", "95"],
+            ["5", "void pack_spinor_kernel<2, double>(char *)", "1", "1", "1"]]
+    rows[1][2] = "Gbyte"
+    rows[4][2] = "300.0"                 # this launch reported in other units below
+    import csv
+    with open(src, "w", newline="") as f:
+        csv.writer(f, quoting=csv.QUOTE_ALL).writerows(rows)
+    out = tmp_path / "traffic.csv"
+    bench.import_ncu(str(src), str(out))
+    h, table = bench.read_profile_table(str(out))
+    assert h == bench.source_hash()
+    assert table["generic<8,1,12,0,plain>"] == [1.3e9]                       # mean of (1.0 + 0.2) and (1.2 + 0.2) GB
+    assert table["f2_staged<2,2,12,2,dagger>"] == [300.1e9]
+    assert table["tile<2,1,12,1,plain>"] == [0.3e9]
+    assert table["f2_twin<4,1,12,3,plain>"] == [0.6e9]
+    assert len(table) == 4                                                  # the pack kernel is not a dslash kernel
+    # a table made from other sources reads as "no traffic figure"
+    stale = tmp_path / "stale.csv"
+    stale.write_text(out.read_text().replace(h, "0" * 12))
+    assert bench.read_profile_table(str(stale))[0] != bench.source_hash()
+
+
+def test_gpus_flag_must_agree_with_the_launcher(monkeypatch):
+    """`--gpus N` under torch.distributed.run must equal WORLD_SIZE (a plain `python bench.py --gpus N` starts the ranks itself)."""
+    monkeypatch.setenv("WORLD_SIZE", "2")
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "4"])
+    with pytest.raises(SystemExit) as e:
+        bench.main()
+    assert "WORLD_SIZE" in str(e.value)
