@@ -209,12 +209,13 @@ TM_DEV void epilogue(real *acc, const real *xv, real alpha, real beta, real scal
 }
 
 
-// resident blocks of 128 threads per SM the register allocation of the fp64 degenerate kernel aims at (measured: profiles/r1_tuning.md)
+// resident blocks of 128 threads per SM the register allocation of the fp64 degenerate kernel aims at (measured: profiles/r1_tuning.md;
+// with 18-real links two blocks and more registers are 3-5 % faster, with 12-real links three: profiles/r2_tuning.md section 6)
 #ifndef TM_MINB_8_1
 #define TM_MINB_8_1 3
 #endif
 template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, bool TWIN = false>
-__global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? TM_MINB_8_1 : (PREC == 8 ? 2 : 1)) tm_dslash_generic(const DslashArgs a)
+__global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? (RECON == 18 ? 2 : TM_MINB_8_1) : (PREC == 8 ? 2 : 1)) tm_dslash_generic(const DslashArgs a)
 {
     typedef typename PrecTraits<PREC>::real real;
     const int Vh = a.Vh;
