@@ -88,12 +88,13 @@ def test_h1_sharded_kernels_match_the_global_oracle(dims, world, kw):
 
 
 @pytest.mark.parametrize("dims,grid", [((4, 4, 8, 8), (1, 2, 1)), ((4, 8, 4, 8), (2, 1, 1)), ((4, 4, 8, 8), (1, 2, 2)), ((6, 8, 8, 4), (2, 2, 1)),
-                                       ((4, 12, 4, 8), (3, 1, 2))],
-                         ids=["z2", "y2", "z2t2", "y2z2", "y3t2"])
+                                       ((4, 12, 4, 8), (3, 1, 2)), ((8, 8, 8, 8), (1, 2, 2)), ((8, 16, 4, 8), (2, 1, 1))],
+                         ids=["z2", "y2", "z2t2", "y2z2", "y3t2", "z2t2-tile-kernel", "y2-tile-kernel"])
 @pytest.mark.parametrize("kw", [dict(mu=0.3, epsilon=0.0, twist_flavor=-1), dict(mu=0.15, epsilon=0.19, twist_flavor=0)], ids=["deg-", "ndeg"])
 def test_h1b_spatial_and_mixed_splits_match_the_global_oracle(dims, grid, kw):
     """Cuts in non-temporal directions (the face gather is strided and flavor-aware) and in two directions at once:
-    every kernel type, parity, dagger and precision against the oracle on the GLOBAL lattice, sub-lattices processed in turn."""
+    every kernel type, parity, dagger and precision against the oracle on the GLOBAL lattice, sub-lattices processed in turn.
+    The last two cases have local extents 8 x 8 x 4 x 4 / 8 x 8 x 4 x 8, which the warp-per-tile half kernel covers (open z, t / y hops there)."""
     nf = 2 if kw["twist_flavor"] == 0 else 1
     world = grid[0] * grid[1] * grid[2]
     sp = split_for(dims, world, "haar", 31, grid)
