@@ -752,6 +752,9 @@ def run_ours(args, log):
     sm_mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz") or 1965.0
     for k in kernels:
         annotate_bound(k, vh, sm_mhz)
+    if roofline and dom:
+        roofline["bound"] = dom["bound"]                    # derived (annotate_bound), not asserted
+        roofline["frac_of_datapath"] = dom["frac_of_datapath"]
     extra = kernels_extra(w, args, sm_mhz, peak) if (rank == 0 and world == 1 and not args.no_extra) else None
     cg = cg_leg(w) if (rank == 0 and world == 1 and not args.no_extra and not args.sharded) else None
     if rank == 0:
