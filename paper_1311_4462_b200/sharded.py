@@ -179,7 +179,7 @@ class Slab:
     one rank, or time when there is a single rank: the sub-lattice is then its own neighbour).  peer = True: faces travel through
     peer-mapped buffers and flag words (PeerRing) instead of torch.distributed point-to-point operations."""
 
-    def __init__(self, global_dims, rank, world, device=0, group=None, grid=None, cut=None, peer=False):
+    def __init__(self, global_dims, rank, world, device=0, group=None, grid=None, cut=None, peer=False, host_sync=False):
         self.global_dims, self.rank, self.world, self.group = tuple(global_dims), int(rank), int(world), group
         self.grid = grid_of(world, grid)
         self.coords = grid_coords(self.rank, self.grid)
@@ -189,6 +189,9 @@ class Slab:
         tm.tm_set_open_dirs(self.lat.ctx, sum(1 << d for d in self.cut))
         self.device = torch.device("cuda", device)
         self.peer = bool(peer)
+        # host_sync (with peer): no flag words; the ranks meet at a host barrier between the pack kernels and the completion kernels
+        # instead.  For ranks that SHARE one GPU (tests), where a kernel spinning on a flag could starve the kernel that sets it.
+        self.host_sync = bool(host_sync)
         self._faces, self._rings = {}, {}
 
     def sites(self):
@@ -246,16 +249,26 @@ class Slab:
         """The distributed form of tm.dslash_apply: faces out, interior kernel while they travel, boundary sites completed."""
         if self.peer:
             pending = []
+            flags = not self.host_sync
             for d in self.cut:
                 epoch, t = self.ring(inp.prec, inp.nf, d).begin()
                 tm.tm_halo_pack(inp.h, gauge.h, parity, dagger, t["to_prev"].data_ptr(), t["to_next"].data_ptr(), d,
-                                _word_ptr(t["flag_prev"]), _word_ptr(t["flag_next"]), epoch)
+                                _word_ptr(t["flag_prev"]) if flags else None, _word_ptr(t["flag_next"]) if flags else None, epoch)
                 pending.append((d, epoch, t))
             tm.dslash_apply(out, inp, x, gauge, p, parity, dagger, kernel_type)        # overlaps the neighbours' stores
+            if self.host_sync:
+                import torch.distributed as dist
+                self.lat.sync()
+                if self.world > 1:
+                    dist.barrier(group=self.group)      # every rank's faces have landed
             for d, epoch, t in pending:
                 sp, sn = self.signs(p, d)
                 tm.tm_halo_apply(out.h, t["from_prev"].data_ptr(), t["from_next"].data_ptr(), gauge.h, p, parity, dagger, kernel_type,
-                                 sp, sn, d, _word_ptr(t["wait_prev"]), _word_ptr(t["wait_next"]), epoch)
+                                 sp, sn, d, _word_ptr(t["wait_prev"]) if flags else None, _word_ptr(t["wait_next"]) if flags else None, epoch)
+            if self.host_sync and self.world > 1:
+                import torch.distributed as dist
+                self.lat.sync()
+                dist.barrier(group=self.group)          # every rank has read its faces: the slot may be reused two exchanges later
             return
         handles = []
         for d in self.cut:

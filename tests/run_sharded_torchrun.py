@@ -2,7 +2,8 @@
 
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P tests/run_sharded_torchrun.py [--grid PY,PZ,PT] [--peer]
 
-(default grid: time slabs (1, 1, N); --peer: faces through peer-mapped buffers and flag words instead of NCCL send / recv.)
+(default grid: time slabs (1, 1, N); --peer: faces through peer-mapped buffers and flag words instead of NCCL send / recv;
+--one-gpu: every rank on cuda:0 over gloo, with --peer the ranks meet at host barriers instead of spinning on flag words.)
 Every rank cuts its sub-lattice out of the same seeded global inputs, applies the LHS of Eq. 2.2 and Eq. 2.3 through
 paper_1311_4462_b200.sharded.Slab.mat_pc (NCCL face exchange), the slabs are gathered on rank 0 and compared with the oracle
 on the global lattice (fp64 1e-12, fp32 1e-5, half 5e-3).  Test infrastructure: pytest runs it with N = 1 (test_gpu_sharded.py);
@@ -26,15 +27,21 @@ TOL = {tm.TM_DOUBLE: 1e-12, tm.TM_SINGLE: 1e-5, tm.TM_HALF: 5e-3}
 
 def main():
     rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
-    torch.cuda.set_device(local)
-    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if "--one-gpu" in sys.argv:
+        local = 0
+        torch.cuda.set_device(0)
+        dist.init_process_group("gloo")
+    else:
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     grid = tuple(int(v) for v in sys.argv[sys.argv.index("--grid") + 1].split(",")) if "--grid" in sys.argv else (1, 1, world)
     peer = "--peer" in sys.argv
+    one_gpu = "--one-gpu" in sys.argv          # all ranks on cuda:0, gloo, host barriers instead of flag words (tests on a 1-GPU box)
     dims, kappa = (8, 8 * grid[0], 8 * grid[1], 8 * grid[2]), 0.1632
     kw = dict(mu=0.15, epsilon=0.19, twist_flavor=0)
     U = si.gauge_field(dims, 31, "haar")
     psi_e = si.mask_parity(si.spinor_field(dims, 2, 32), dims, 0)
-    slab = sharded.Slab(dims, rank, world, local, grid=grid, peer=peer)
+    slab = sharded.Slab(dims, rank, world, local, grid=grid, peer=peer, host_sync=one_gpu)
     sl = slab.sites()
     order = np.concatenate([sharded.sub_sites(dims, grid, sharded.grid_coords(r, grid)) for r in range(world)])
     pg = tm.params(kappa, **kw)
@@ -46,7 +53,9 @@ def main():
         for typ, dagger in ((tm.TM_MATPC_ASYM, 0), (tm.TM_MATPC_SYM, 0), (tm.TM_MATPC_SYM, 1)):
             slab.mat_pc(fout, fin, ftmp, g, pg, typ, dagger)
             slab.lat.sync()
-            mine = torch.from_numpy(fout.download(0).view(np.float64).copy()).cuda()
+            mine = torch.from_numpy(fout.download(0).view(np.float64).copy())
+            if not one_gpu:
+                mine = mine.cuda()
             parts = [torch.empty_like(mine) for _ in range(world)] if rank == 0 else None
             dist.gather(mine, parts, dst=0)
             if rank == 0:

@@ -247,3 +247,91 @@ def test_h6_sharded_half_tight_against_the_oracle_on_the_quantised_inputs(dims, 
         assert err <= 6e-5, (parity, dagger, kt, err)
         assert lsb.max() <= 2.75, (parity, dagger, kt, lsb.max())
     print("sharded half, quantised inputs: worst rel L2 %.2e, worst component %.2f LSB" % (worst_l2, worst_lsb))
+
+
+def _ipc_worker(rank, world, port, q):
+    """One process of H7: maps its neighbours' receive buffers with CUDA IPC (PeerRing), stores into them with ordinary device work,
+    and checks what arrived in its own buffers after a HOST barrier (no kernel of one process ever waits for another process)."""
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ok = True
+    try:
+        torch.cuda.set_device(0)
+
+        def allgather(obj):
+            out = [None] * world
+            dist.all_gather_object(out, obj)
+            return out
+        prev, nxt = (rank - 1) % world, (rank + 1) % world
+        ring = sharded.PeerRing(rank, prev, nxt, 4096, torch.float32, torch.device("cuda", 0), allgather)
+        dist.barrier()
+        for it in range(4):                      # both buffer slots, twice
+            epoch, t = ring.begin()
+            t["to_prev"].fill_(1000.0 * rank + epoch + 0.25)
+            t["to_next"].fill_(1000.0 * rank + epoch + 0.5)
+            for name in ("flag_prev", "flag_next"):
+                f, i = t[name]
+                f[i] = epoch
+            torch.cuda.synchronize()
+            dist.barrier()                       # every rank's stores are complete
+            ok = ok and bool((t["from_prev"] == 1000.0 * prev + epoch + 0.5).all()) and bool((t["from_next"] == 1000.0 * nxt + epoch + 0.25).all())
+            ok = ok and int(t["wait_prev"][0][t["wait_prev"][1]]) == epoch and int(t["wait_next"][0][t["wait_next"][1]]) == epoch
+            dist.barrier()                       # nobody overwrites a slot before everyone has read it
+        q.put((rank, ok))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_h7_peer_buffers_map_across_processes_with_cuda_ipc(world):
+    """The part of the peer-buffer transport that CPU tests cannot reach: the receive buffers and flag words of one PROCESS mapped
+    into another with CUDA IPC (torch's tensor reductions through all_gather_object), routed as PeerRing routes them.  Two and three
+    processes share this box's one GPU; they synchronise on the host only."""
+    import socket
+    import torch.multiprocessing as mp
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_ipc_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = [q.get(timeout=300) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    assert sorted(r for r, _ in got) == list(range(world)) and all(ok for _, ok in got)
+
+
+@pytest.mark.parametrize("extra", [["--peer", "--grid", "1,1,2"], ["--peer", "--grid", "1,2,2"], ["--peer", "--grid", "2,1,2"]],
+                         ids=["peer-t2", "peer-z2t2", "peer-y2t2"])
+def test_h8_two_and_four_processes_on_one_gpu(extra):
+    """tests/run_sharded_torchrun.py with SEVERAL ranks, all on this box's one GPU (--one-gpu: gloo; the peer transport with host
+    barriers in place of the flag words, so that no kernel waits for another process): every rank holds its sub-lattice in its own
+    process, the pack kernels store the faces straight into the neighbour PROCESS's memory through CUDA IPC, and the gathered
+    Eq. 2.2 / 2.3 / adjoint results match the oracle on the global lattice in all three precisions.  (The send / recv transport needs
+    NCCL, which does not run two ranks on one GPU, and gloo does not move device tensors point to point: that transport is covered
+    by the gloo ring tests on CPU tensors and by H3 with one rank.)"""
+    import os
+    import socket
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    n = 1
+    for v in extra[extra.index("--grid") + 1].split(","):
+        n *= int(v)
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n), "--master-addr", "127.0.0.1",
+                        "--master-port", str(port), os.path.join(root, "tests", "run_sharded_torchrun.py"), "--one-gpu"] + extra,
+                       capture_output=True, text=True, timeout=900, cwd=root)
+    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-3000:]
+    assert "sharded ok: world %d" % n in r.stdout
