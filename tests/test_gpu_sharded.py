@@ -309,8 +309,8 @@ def test_h7_peer_buffers_map_across_processes_with_cuda_ipc(world):
     assert sorted(r for r, _ in got) == list(range(world)) and all(ok for _, ok in got)
 
 
-@pytest.mark.parametrize("extra", [["--peer", "--grid", "1,1,2"], ["--peer", "--grid", "1,2,2"], ["--peer", "--grid", "2,1,2"]],
-                         ids=["peer-t2", "peer-z2t2", "peer-y2t2"])
+@pytest.mark.parametrize("extra", [["--peer", "--grid", "1,1,2", "--cg"], ["--peer", "--grid", "1,2,2"], ["--peer", "--grid", "2,1,2"]],
+                         ids=["peer-t2-cg", "peer-z2t2", "peer-y2t2"])
 def test_h8_two_and_four_processes_on_one_gpu(extra):
     """tests/run_sharded_torchrun.py with SEVERAL ranks, all on this box's one GPU (--one-gpu: gloo; the peer transport with host
     barriers in place of the flag words, so that no kernel waits for another process): every rank holds its sub-lattice in its own
@@ -335,3 +335,5 @@ def test_h8_two_and_four_processes_on_one_gpu(extra):
                        capture_output=True, text=True, timeout=900, cwd=root)
     assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-3000:]
     assert "sharded ok: world %d" % n in r.stdout
+    if "--cg" in extra:                # the solver across two processes: operator callback + all-reduce hook (gloo on device scalars)
+        assert "sharded cg ok" in r.stdout
