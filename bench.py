@@ -486,17 +486,20 @@ def kernels_extra(w, args, sm_mhz, peak):
             g = g or lat.gauge(host_u, prec, recon)
             for nf in (1, 2):
                 fin, fx, fout = fields[(prec, nf)]
-                for kt, label in ((0, "A"), (1, "A-xpay"), (2, "B"), (3, "REC"), (0, "A wilson")):
+                for kt, label in ((0, "A"), (1, "A-xpay"), (2, "B"), (3, "REC"), (0, "A wilson"), (6, "R^-1 D R^-1 (fused)")):
                     if label == "A wilson" and (nf == 2 or recon != 12):
+                        continue
+                    if kt == 6 and recon != 12:
                         continue
                     p = wilson if label == "A wilson" else w.params[nf]
                     time.sleep(0.05)         # "alone": not on top of the power / thermal state the previous kernel's launches left behind
-                    us = time_alone(lambda: tm.dslash_apply(fout, fin, None if kt == 0 else fx, g, p, 1, 0, kt), lat.sync)
-                    b = bytes_per_site(nf, prec, recon, kt) * vh
-                    f = flops_per_site(nf, kt) * vh
+                    us = time_alone(lambda: tm.dslash_apply(fout, fin, None if kt in (0, 6) else fx, g, p, 1, 0, kt), lat.sync)
+                    # the fused D R^-1 form reads the whole neighbour site on the time hops: one spinor (+ norms) more than kernel A
+                    b = (bytes_per_site(nf, prec, recon, 0 if kt == 6 else kt) + (nf * 12 * prec + (4 * nf if prec == 2 else 0) if kt == 6 else 0)) * vh
+                    f = (flops_per_site(nf, 0 if kt == 6 else kt) + (8 * (48 + 24 if nf == 1 else 240) if kt == 6 else 0)) * vh
                     k = {"kernel": tm.tm_last_kernel_name(lat.ctx), "flavors": nf, "prec": PREC_NAME[prec], "type": label, "recon": recon,
                          "us": us, "gflops": f / us / 1e3, "alg_gbs": b / us / 1e3, "frac_of_measured_peak": b / us / 1e3 / peak,
-                         "bytes_per_site": bytes_per_site(nf, prec, recon, kt), "prec_bytes": prec}
+                         "bytes_per_site": b // vh, "prec_bytes": prec}
                     annotate_bound(k, vh, sm_mhz)
                     out.append(k)
             del g

@@ -163,7 +163,7 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
  * intermediate R_oo^-1 D_oe in_e.  dagger: the exact adjoint.  ASYM: the same two launches with the daggered
  * kernels.  SYM: M^_sym^dag = 1 - kappa^2 D^dag_eo R^dag^-1_oo D^dag_oe R^dag^-1_ee (C7) = the fused
  * TM_TWIST_INV_DSLASH_TWIST_INV^dag kernel (R^dag^-1 D^dag R^dag^-1) and the plain xpay kernel: two launches as well
- * (fp64 and half-precision doublets: the local twist into out_e first, three launches; out_e must not alias in_e, TM_ERR_ALIAS).
+ * (half-precision doublets: the local twist into out_e first, three launches; out_e must not alias in_e, TM_ERR_ALIAS).
  * Asynchronous. */
 int tm_mat_pc(tm_field *out_e, const tm_field *in_e, tm_field *tmp_o, const tm_gauge *g, const tm_params *p,
               tm_matpc type, int dagger);
@@ -175,7 +175,7 @@ int tm_twist_apply(tm_field *out, const tm_field *in, const tm_params *p, int in
 
 /* Right-hand side of Eq. 2.2 (ASYM: rhs_e = b_e + kappa D_eo R_oo^-1 b_o) or Eq. 2.3 (SYM: rhs_e = R_ee^-1 (b_e +
  * kappa D_eo R_oo^-1 b_o)), PAPER.md:60-64 in the reading C4 of DESIGN.md.  One launch of the fused D R^-1 kernel
- * (TM_DSLASH_TWIST_INV_AXPY / TM_RECONSTRUCT_TWIST_INV); fp64 and half-precision doublets, for which the fused kernel measured
+ * (TM_DSLASH_TWIST_INV_AXPY / TM_RECONSTRUCT_TWIST_INV); half-precision doublets, for which the fused kernel measured
  * slower, take the local twist into tmp_o and the plain kernel instead (two launches).  tmp_o is scratch: a valid field that does
  * not alias b_e, b_o or rhs_e (TM_ERR_ALIAS); rhs_e may alias b_e.  Asynchronous. */
 int tm_prepare_rhs(tm_field *rhs_e, const tm_field *b_e, const tm_field *b_o, tm_field *tmp_o, const tm_gauge *g,

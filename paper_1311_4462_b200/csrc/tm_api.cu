@@ -97,10 +97,10 @@ size_t field_bytes(const TmGeom &g, int prec, int nf)
 }
 
 // The fused D R^-1 kernels (TWIN) replace a separate local pass (read + write of one field) by 8 register twists and full-site
-// time hops.  Measured at 32^3 x 64 (profiles/r2_tuning.md), fused against kernel A + local pass: fp64 195 / 189 + 62 us, fp32 97 / 95 + 31,
-// half 90 / 78 + 17, fp32 doublet 167 / 150 + 62; but the fp64 doublet (254 registers, 344 / 267 + 62) and the half doublet (bound by
-// the FP32 datapath, 176 / 127 + 35) lose: they keep the local pass.
-bool fused_twist_in_pays(const tm_field *f) { return !(f->nf == 2 && f->prec != TM_SINGLE); }
+// time hops.  Measured at 32^3 x 64 (profiles/r2_tuning.md section 2), fused against kernel A + local pass: fp64 195 / 189 + 62 us,
+// fp32 97 / 95 + 31, half 90 / 78 + 17, fp64 doublet 311 / 273 + 123, fp32 doublet 167 / 150 + 61; only the half doublet, bound by
+// the FP32 datapath (176 / 127 + 33), loses and keeps the local pass.
+bool fused_twist_in_pays(const tm_field *f) { return !(f->nf == 2 && f->prec == TM_HALF); }
 
 bool overlap(const tm_field *a, const tm_field *b)
 {

@@ -555,7 +555,7 @@ def test_t3e_sym_dagger_is_the_adjoint_and_rhs_preparation(kw):
         assert rel_l2(bench.prepare_rhs(b, pg, tm.TM_MATPC_SYM, prec, recon, nf, alias=True),
                       oracle.prepare_rhs(b, bench.U, po, tm.TM_MATPC_SYM)) <= TOL[prec]
     # the normal operator M^_sym^dag M^_sym is four launches (the adjoint's leading twist is fused into the D R^-1 kernel) -- five for
-    # the fp64 and half doublets, which keep the local pass -- and the right-hand side of Eq. 2.2 / 2.3 one launch (two)
+    # the half-precision doublet, which keeps the local pass -- and the right-hand side of Eq. 2.2 / 2.3 one launch (two)
     lat = bench.lat
     for prec in PRECS:
         g = bench.gauge(prec, tm.TM_RECON_12)
@@ -564,7 +564,7 @@ def test_t3e_sym_dagger_is_the_adjoint_and_rhs_preparation(kw):
         n0 = lat.launches()
         tm.mat_pc(f[1], f[0], f[2], g, pg, tm.TM_MATPC_SYM, 0)
         tm.mat_pc(f[3], f[1], f[2], g, pg, tm.TM_MATPC_SYM, 1)
-        extra = 1 if (prec != tm.TM_SINGLE and nf == 2) else 0      # the fp64 and half doublets keep the local pass (measured slower fused)
+        extra = 1 if (prec == tm.TM_HALF and nf == 2) else 0      # the half doublet keeps the local pass (measured slower fused)
         assert lat.launches() - n0 == 4 + extra
         n0 = lat.launches()
         tm.prepare_rhs(f[3], f[0], f[1], f[2], g, pg, tm.TM_MATPC_SYM)
