@@ -667,6 +667,9 @@ def run_ours(args, log):
     w = Workload(local, log, slab)
     lat, vh = w.lat, w.vh
     tm.tm_set_path(lat.ctx, args.path)
+    for kv in [t for t in args.tune.split(",") if t]:
+        k, v = kv.split("=")
+        tm.tm_set_tuning(lat.ctx, k, int(v))
     ops = step_ops()
     step_flops = sum(op_flops(o, vh) for o in ops)
     step_bytes = sum(op_bytes(o, vh) for o in ops)
@@ -789,7 +792,8 @@ def run_ours(args, log):
                           "parallelism": ("sub-lattices of 32^3 x 64 on a (y, z, t) process grid %s, one per GPU, face exchange per dslash through %s (--sharded)"
                                           % (args.grid or "1,1,%d" % world, "peer-mapped buffers + flag words" if args.peer else "torch.distributed send / recv"))
                           if args.sharded else ("replicas only (north_star: no sharding)" if world > 1 else "single GPU"),
-                          "l2": "inputs larger than L2 (gauge fields 201-805 MB each, 2.3 GB touched per step)"},
+                          "l2": "inputs larger than L2 (gauge fields 201-805 MB each, 2.3 GB touched per step)",
+                          "tune": args.tune or "defaults"},
                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                "step_flops": step_flops, "step_alg_bytes": step_bytes, "kernels": kernels, "kernels_extra": extra, "cg": cg, "config5": c5,
                "paper_table1_gflops_12real": {"%s/%s" % ("deg" if k[0] == 1 else "ndeg", PREC_NAME[k[1]]): v
@@ -813,7 +817,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernels", default="", help="time single kernels alone instead: PREC:NF:RECON:KT[,...] (tuning runs; see run_kernels)")
     ap.add_argument("--dims", default="32,32,32,64", help="--kernels: lattice extents")
-    ap.add_argument("--tune", default="", help="--kernels: tm_set_tuning overrides, key=value[,...]")
+    ap.add_argument("--tune", default="", help="tm_set_tuning overrides, key=value[,...] (non-default values are recorded in config.tune)")
     ap.add_argument("--config5", action="store_true", help="time BASELINE.json configs[4] instead (48^3x96 fp64 doublet, Eq. 2.3 operator x 100; ~25 GB of host memory)")
     ap.add_argument("--no-extra", action="store_true", help="skip the kernels_extra table (every kernel type x precision x compression, timed alone)")
     ap.add_argument("--sass-mix", action="store_true", help="host only: write profiles/sass_mix.csv + profiles/r2_sass_histogram.md from the built objects")

@@ -298,7 +298,9 @@ int tm_set_path(tm_ctx *ctx, int path);
  *   "stage_links": 1 = the 8 links of a site are copied to shared memory with cp.async before the hops, 0 = direct
  *   loads, -1 = library default;   "block_threads": 32 / 64 / 128 sites per thread block, 0 = library default;
  *   "z_chunks": the thread blocks walk the lattice in n chunks of Z / n z-planes (all time slices of a chunk first) so that
- *   the input spinor's reuse window fits the L2; -1 = library default (from the size of three time slices).
+ *   the input spinor's reuse window fits the L2; -1 = library default (from the size of three time slices);
+ *   "tile_kernel": half precision, 18- / 12-real links: 0 = thread-per-site kernels only, 1 or -1 (default) = the warp-per-tile
+ *   kernel wherever the geometry fits (X/2 in {4, 8, 16}, Y a multiple of 64/X); both give bit-identical results.
  *   Unknown key or bad value -> TM_ERR_ARG. */
 int tm_set_tuning(tm_ctx *ctx, const char *key, int value);
 

@@ -657,9 +657,9 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     const TmKernelEntry *tab = (c->path == 0 && (int)prec != TM_DOUBLE) ? tm_f2_table((int)prec, out->nf) : nullptr;
     if (!tab || !tab[kidx].fn) tab = tm_generic_table((int)prec, out->nf);
     // half precision: the warp-per-tile kernel with shared-memory staged operands (tm_dslash_tile.cuh) where the lattice allows it.
-    // Measured (profiles/r2_tuning.md): 4-6 % faster than the staged thread-per-site kernel for one flavor, no faster (A) or slower (B)
-    // for the doublet, whose 26 KB of shared memory per warp leave 8 warps per SM: default for one flavor only ("tile_kernel" = 1 forces it)
-    const bool tile = (int)prec == TM_HALF && c->path == 0 && !twin && g->recon != 8 && (c->tile_kernel == 1 || (c->tile_kernel < 0 && out->nf == 1)) &&
+    // Measured (profiles/r2_tuning.md section 4): 6-7 % faster than the staged thread-per-site kernel for one flavor, 2-4 % for the doublet
+    // (26 KB of shared memory per warp, 8 warps per SM): the default wherever the geometry fits ("tile_kernel" = 0 turns it off)
+    const bool tile = (int)prec == TM_HALF && c->path == 0 && !twin && g->recon != 8 && c->tile_kernel != 0 &&
                       (c->g.Xh == 4 || c->g.Xh == 8 || c->g.Xh == 16) && c->g.X[1] % (32 / c->g.Xh) == 0 && c->g.Vh % 32 == 0;
     const TmKernelEntry &k = tile ? (out->nf == 1 ? tm_tile_table_2_1() : tm_tile_table_2_2())[((g->recon == 18 ? 0 : 1) * 4 + kcode) * 2 + (dagger ? 1 : 0)]
                            : twin ? tm_twin_table((int)prec, out->nf, c->path == 0)[((g->recon == 18 ? 0 : g->recon == 12 ? 1 : 2) * 2 + (kcode == 3 ? 1 : 0)) * 2 + (dagger ? 1 : 0)]

@@ -19,40 +19,89 @@ struct TileGeom {
     int Xh, R, lg;         // sites per x-row of one parity (= 1 << lg); x-rows per tile
     int tps;               // tiles per (z, t) slab = Y / R
     TmFastDiv dtps, dZ;    // tile -> (slab, tile within slab); slab -> (t, z)
+    const void *gauge_f, *gauge_b;   // the gauge blocks of the output parity / of the other parity
 };
 
 #ifndef TM_TILE_MINB_1
 #define TM_TILE_MINB_1 12
 #endif
 #ifndef TM_TILE_MINB_2
-#define TM_TILE_MINB_2 8
+#define TM_TILE_MINB_2 9
 #endif
 
-// ---- asynchronous copies of one slot (one site's share) of a tile ----------------------------------------------------------
+// ---- asynchronous copies of a tile: every lane moves 16 bytes per plane ---------------------------------------------------------
+// `src` = the tile's address in global memory PLUS lane * 16, `dst` = the tile's shared-memory address plus lane * 16: one 64-bit
+// address per (tile, lane) serves every plane through immediate offsets.  The narrow planes (norms: 4 bytes per site; link tails: 8
+// or 4) are moved in 16-byte pieces too, by the first 8 or 16 lanes, so that they need no address of their own.
 // PART: 0 all planes, 1 upper spin half only, 2 lower half only (half precision: planes {0,1} / {1,2}; the norm always)
 template <int PREC, int PART>
-TM_DEV void tile_copy_spinor(unsigned dst, const char *src, int slot)
+TM_DEV void tile_copy_spinor_planes(unsigned dst, const char *src)
 {
     static_assert(PREC == 2, "the tile kernel is instantiated for half precision");
-    if constexpr (PART != 2) cp_async_u32<16>(dst + slot * 16, src + slot * 16);
-    cp_async_u32<16>(dst + TM_PLANE + slot * 16, src + TM_PLANE + slot * 16);
-    if constexpr (PART != 1) cp_async_u32<16>(dst + 2 * TM_PLANE + slot * 16, src + 2 * TM_PLANE + slot * 16);
-    cp_async_u32<4>(dst + 3 * TM_PLANE + slot * 4, src + 3 * TM_PLANE + slot * 4);
+    if constexpr (PART != 2) cp_async_u32<16>(dst, src);
+    cp_async_u32<16>(dst + TM_PLANE, src + TM_PLANE);
+    if constexpr (PART != 1) cp_async_u32<16>(dst + 2 * TM_PLANE, src + 2 * TM_PLANE);
+}
+TM_DEV void tile_copy_spinor_norms(unsigned dst, const char *src, int lane)      // 32 floats = 8 pieces
+{
+    if (lane < 8) cp_async_u32<16>(dst + 3 * TM_PLANE, src + 3 * TM_PLANE);
+}
+template <int PREC, int PART>
+TM_DEV void tile_copy_spinor(unsigned dst, const char *src, int lane)
+{
+    tile_copy_spinor_planes<PREC, PART>(dst, src);
+    tile_copy_spinor_norms(dst, src, lane);
+}
+// the time hops need one spin half (PART 1: planes 0, 1; PART 2: planes 1, 2): two planes and the norms, packed into TM_HALF_TILE bytes
+constexpr int TM_HALF_TILE = 2 * TM_PLANE + TM_TILE * 4;
+template <int PREC, int PART>
+TM_DEV void tile_copy_half_spinor(unsigned dst, const char *src, int lane)
+{
+    static_assert(PREC == 2 && (PART == 1 || PART == 2), "half precision, one spin half");
+    constexpr int K0 = PART == 1 ? 0 : 1;
+    cp_async_u32<16>(dst, src + K0 * TM_PLANE);
+    cp_async_u32<16>(dst + TM_PLANE, src + (K0 + 1) * TM_PLANE);
+    if (lane < 8) cp_async_u32<16>(dst + 2 * TM_PLANE, src + 3 * TM_PLANE);
 }
 template <int PREC, int RECON>
-TM_DEV void tile_copy_link(unsigned dst, const char *src, int slot)
+TM_DEV void tile_copy_link_planes(unsigned dst, const char *src)
+{
+    constexpr int N16 = link_n16<PREC, RECON>();
+#pragma unroll
+    for (int k = 0; k < N16; k++) cp_async_u32<16>(dst + k * TM_PLANE, src + k * TM_PLANE);
+}
+template <int PREC, int RECON>
+TM_DEV void tile_copy_link_tail(unsigned dst, const char *src, int lane)          // 32 x 8 bytes = 16 pieces, 32 x 4 bytes = 8 pieces
 {
     constexpr int N16 = link_n16<PREC, RECON>(), TW = link_tailw<PREC, RECON>();
-#pragma unroll
-    for (int k = 0; k < N16; k++) cp_async_u32<16>(dst + k * TM_PLANE + slot * 16, src + k * TM_PLANE + slot * 16);
-    if constexpr (TW == 8) cp_async_u32<8>(dst + N16 * TM_PLANE + slot * 8, src + N16 * TM_PLANE + slot * 8);
-    if constexpr (TW == 4) cp_async_u32<4>(dst + N16 * TM_PLANE + slot * 4, src + N16 * TM_PLANE + slot * 4);
+    if constexpr (TW > 0) {
+        if (lane < 2 * TW) cp_async_u32<16>(dst + N16 * TM_PLANE, src + N16 * TM_PLANE);
+    }
+}
+template <int PREC, int RECON>
+TM_DEV void tile_copy_link(unsigned dst, const char *src, int lane)
+{
+    tile_copy_link_planes<PREC, RECON>(dst, src);
+    tile_copy_link_tail<PREC, RECON>(dst, src, lane);
 }
 
 // ---- shared memory -> the raw words of one hop (what issue_link / issue_spinor load from global memory) ---------------------
 TM_DEV uint4 lds_u4(unsigned a) { uint4 v; asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a)); return v; }
 TM_DEV uint2 lds_u2(unsigned a) { uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a)); return v; }
 TM_DEV unsigned lds_u1(unsigned a) { unsigned v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a)); return v; }
+
+template <int PREC, int NF, int RECON>
+TM_DEV void tile_read_spinor(HopRaw<PREC, NF, RECON> &r, unsigned stile, int slot)
+{
+    constexpr int STB = spinor_tile_bytes(PREC);
+#pragma unroll
+    for (int f = 0; f < NF; f++) {
+        const unsigned p = stile + f * STB;
+#pragma unroll
+        for (int k = 0; k < 3; k++) r.s[f][k] = lds_u4(p + k * TM_PLANE + slot * 16);
+        r.n[f] = __uint_as_float(lds_u1(p + 3 * TM_PLANE + slot * 4));
+    }
+}
 
 template <int PREC, int NF, int RECON, int PART>
 TM_DEV void tile_read_hop(HopRaw<PREC, NF, RECON> &r, unsigned stile, unsigned ltile, int sslot, int lslot)
@@ -63,11 +112,18 @@ TM_DEV void tile_read_hop(HopRaw<PREC, NF, RECON> &r, unsigned stile, unsigned l
     else r.lt = lds_u2(ltile + TM_PLANE + lslot * 8);
 #pragma unroll
     for (int f = 0; f < NF; f++) {
-        const unsigned p = stile + f * STB;
-        if constexpr (PART != 2) r.s[f][0] = lds_u4(p + sslot * 16);
-        r.s[f][1] = lds_u4(p + TM_PLANE + sslot * 16);
-        if constexpr (PART != 1) r.s[f][2] = lds_u4(p + 2 * TM_PLANE + sslot * 16);
-        r.n[f] = __uint_as_float(lds_u1(p + 3 * TM_PLANE + sslot * 4));
+        if constexpr (PART == 0) {
+            const unsigned p = stile + f * STB;
+#pragma unroll
+            for (int k = 0; k < 3; k++) r.s[f][k] = lds_u4(p + k * TM_PLANE + sslot * 16);
+            r.n[f] = __uint_as_float(lds_u1(p + 3 * TM_PLANE + sslot * 4));
+        } else {                                                   // a packed half tile (tile_copy_half_spinor)
+            constexpr int K0 = PART == 1 ? 0 : 1;
+            const unsigned p = stile + f * TM_HALF_TILE;
+            r.s[f][K0] = lds_u4(p + sslot * 16);
+            r.s[f][K0 + 1] = lds_u4(p + TM_PLANE + sslot * 16);
+            r.n[f] = __uint_as_float(lds_u1(p + 2 * TM_PLANE + sslot * 4));
+        }
     }
 }
 
@@ -76,10 +132,10 @@ __global__ void __launch_bounds__(32, NF == 1 ? TM_TILE_MINB_1 : TM_TILE_MINB_2)
 {
     constexpr int STB = spinor_tile_bytes(PREC), LTB = link_tile_bytes(PREC, RECON);
     constexpr int FS = NF * STB;                                   // all flavors of one spinor tile
-    // shared memory of the warp: six spinor tiles (own index, assembled y, +z, -z, +t, -t), the 4 forward link tiles, 4 backward ones
+    // shared memory of the warp: four spinor tiles (own index, assembled y, +z, -z), two half tiles (+t, -t), the 4 forward link tiles, 4 backward ones
     const unsigned sm = smem_u32(tm_smem);
-    const unsigned SX = sm, SY = sm + FS, SZP = sm + 2 * FS, SZM = sm + 3 * FS, STP = sm + 4 * FS, STM = sm + 5 * FS;
-    const unsigned LF = sm + 6 * FS, LBX = LF + 4 * LTB, LBY = LBX + LTB, LBZ = LBY + LTB, LBT = LBZ + LTB;
+    const unsigned SX = sm, SY = sm + FS, SZP = sm + 2 * FS, SZM = sm + 3 * FS, STP = sm + 4 * FS, STM = STP + NF * TM_HALF_TILE;
+    const unsigned LF = STM + NF * TM_HALF_TILE, LBX = LF + 4 * LTB, LBY = LBX + LTB, LBZ = LBY + LTB, LBT = LBZ + LTB;
 
     // a2, per warp: the tile's place on the lattice and its neighbour tiles (functions of blockIdx: uniform)
     const int T = blockIdx.x, l = threadIdx.x;
@@ -95,43 +151,67 @@ __global__ void __launch_bounds__(32, NF == 1 ? TM_TILE_MINB_1 : TM_TILE_MINB_2)
     const int y = tin * R + row;
     const int q = (y + z + t + a.parity) & 1;
 
-    const char *in = static_cast<const char *>(a.in);
-    const size_t PB = (size_t)tm_tiles(a.Vh) * 4 * LTB;
-    const char *gf = static_cast<const char *>(a.gauge) + (size_t)a.parity * PB;
-    const char *gb = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * PB;
+    // per-lane 64-bit bases with the lane's 16 bytes folded in: a tile's address is then ONE multiply-add (tile index x tile bytes + base)
+    const char *in_l = static_cast<const char *>(a.in) + l * 16;
+    const char *gf_l = static_cast<const char *>(tg.gauge_f) + l * 16;     // forward links: the block of the output parity
+    const char *gb_l = static_cast<const char *>(tg.gauge_b) + l * 16;     // backward links: the other parity's block
+    // (opaque to the compiler, which otherwise keeps the pointer uniform and pays a 64-bit add per tile for the lane offset)
+    asm volatile("" : "+l"(in_l), "+l"(gf_l), "+l"(gb_l));
+    const unsigned sl = l * 16;
+    auto spinor_tile = [&](int tile) { return in_l + (size_t)(unsigned)tile * FS; };
+    auto link_tile = [&](const char *g, int tile, int mu) { return g + (size_t)(unsigned)(tile * 4 + mu) * LTB; };
 
     // ---- 1. every operand of the warp on its way to shared memory: four commit groups, in the order the hops consume them
+    {
+        const char *s0 = spinor_tile(T);
 #pragma unroll
-    for (int f = 0; f < NF; f++) tile_copy_spinor<PREC, 0>(SX + f * STB, in + (size_t)T * FS + f * STB, l);
+        for (int f = 0; f < NF; f++) tile_copy_spinor<PREC, 0>(SX + f * STB + sl, s0 + f * STB, l);
+        const char *l0 = link_tile(gf_l, T, 0);
 #pragma unroll
-    for (int mu = 0; mu < 4; mu++) tile_copy_link<PREC, RECON>(LF + mu * LTB, gf + ((size_t)T * 4 + mu) * LTB, l);
-    tile_copy_link<PREC, RECON>(LBX, gb + ((size_t)T * 4 + 0) * LTB, l);
+        for (int mu = 0; mu < 4; mu++) tile_copy_link<PREC, RECON>(LF + mu * LTB + sl, l0 + mu * LTB, l);
+        tile_copy_link<PREC, RECON>(LBX + sl, link_tile(gb_l, T, 0), l);
+    }
     cp_async_commit();
     {   // the y-tile: slots [0, Xh) from the tile after this one, slots [32 - Xh, 32) from the tile before (Xh = 16: every lane copies)
         const bool lo = l < Xh, hi = l >= 32 - Xh;
-        const int ty = lo ? Typ : Tym;
         if (lo || hi) {
+            const char *sy = spinor_tile(lo ? Typ : Tym);
 #pragma unroll
-            for (int f = 0; f < NF; f++) tile_copy_spinor<PREC, 0>(SY + f * STB, in + (size_t)ty * FS + f * STB, l);
+            for (int f = 0; f < NF; f++) tile_copy_spinor_planes<PREC, 0>(SY + f * STB + sl, sy + f * STB);
+        }
+        {   // its norms in 16-byte pieces of 4 slots (Xh is a multiple of 4: a piece never straddles the two source tiles)
+            const bool nlo = 4 * l < Xh, nhi = 4 * l >= 32 - Xh;
+            if (l < 8 && (nlo || nhi)) {
+                const char *sn = spinor_tile(nlo ? Typ : Tym);
+#pragma unroll
+                for (int f = 0; f < NF; f++) cp_async_u32<16>(SY + f * STB + 3 * TM_PLANE + sl, sn + f * STB + 3 * TM_PLANE);
+            }
         }
         // backward y links: U_y(x - y) sits at the neighbour's index: slots [0, 32 - Xh) in this tile, the rest in the tile before
-        const int tl = (l < 32 - Xh) ? T : Tym;
-        tile_copy_link<PREC, RECON>(LBY, gb + ((size_t)tl * 4 + 1) * LTB, l);
+        tile_copy_link_planes<PREC, RECON>(LBY + sl, link_tile(gb_l, (l < 32 - Xh) ? T : Tym, 1));
+        constexpr int SPP = 16 / (link_tailw<PREC, RECON>() > 0 ? link_tailw<PREC, RECON>() : 16);      // slots per 16-byte tail piece
+        tile_copy_link_tail<PREC, RECON>(LBY + sl, link_tile(gb_l, (SPP * l < 32 - Xh) ? T : Tym, 1), l);
     }
     cp_async_commit();
+    {
+        const char *zp = spinor_tile(Tzp), *zm = spinor_tile(Tzm);
 #pragma unroll
-    for (int f = 0; f < NF; f++) {
-        tile_copy_spinor<PREC, 0>(SZP + f * STB, in + (size_t)Tzp * FS + f * STB, l);
-        tile_copy_spinor<PREC, 0>(SZM + f * STB, in + (size_t)Tzm * FS + f * STB, l);
+        for (int f = 0; f < NF; f++) {
+            tile_copy_spinor<PREC, 0>(SZP + f * STB + sl, zp + f * STB, l);
+            tile_copy_spinor<PREC, 0>(SZM + f * STB + sl, zm + f * STB, l);
+        }
+        tile_copy_link<PREC, RECON>(LBZ + sl, link_tile(gb_l, Tzm, 2), l);
     }
-    tile_copy_link<PREC, RECON>(LBZ, gb + ((size_t)Tzm * 4 + 2) * LTB, l);
     cp_async_commit();
+    {   // a3: the time hops need half a spinor: (1 - gamma_4) keeps the lower half, (1 + gamma_4) the upper
+        const char *tp = spinor_tile(Ttp), *tmn = spinor_tile(Ttm);
 #pragma unroll
-    for (int f = 0; f < NF; f++) {      // a3: the time hops need half a spinor: (1 - gamma_4) keeps the lower half, (1 + gamma_4) the upper
-        tile_copy_spinor<PREC, DAG ? 1 : 2>(STP + f * STB, in + (size_t)Ttp * FS + f * STB, l);
-        tile_copy_spinor<PREC, DAG ? 2 : 1>(STM + f * STB, in + (size_t)Ttm * FS + f * STB, l);
+        for (int f = 0; f < NF; f++) {
+            tile_copy_half_spinor<PREC, DAG ? 1 : 2>(STP + f * TM_HALF_TILE + sl, tp + f * STB, l);
+            tile_copy_half_spinor<PREC, DAG ? 2 : 1>(STM + f * TM_HALF_TILE + sl, tmn + f * STB, l);
+        }
+        tile_copy_link<PREC, RECON>(LBT + sl, link_tile(gb_l, Ttm, 3), l);
     }
-    tile_copy_link<PREC, RECON>(LBT, gb + ((size_t)Ttm * 4 + 3) * LTB, l);
     cp_async_commit();
 
     // hop weights (HopCtx of tm_dslash_f2.cuh): time boundary sign, and 0 for a hop that leaves a cut sub-lattice
@@ -167,13 +247,23 @@ __global__ void __launch_bounds__(32, NF == 1 ? TM_TILE_MINB_1 : TM_TILE_MINB_2)
     consume_hop<PREC, NF, RECON, DAG, false, 2>(A, r, c);
     tile_read_hop<PREC, NF, RECON, 0>(r, SYM, LBY, ym, ym);
     consume_hop<PREC, NF, RECON, DAG, false, 3>(A, r, c);
-    cp_async_wait<1>();
+    if constexpr (KT != 0) {
+        // the x operand of the epilogue (the warp's own tile of another field) takes the place of the own-index tile, which the x and y hops
+        // are done with: a fifth commit group, in flight during the z and t hops
+        __syncwarp();
+        const char *x_l = static_cast<const char *>(a.x) + l * 16;
+        const char *xs = x_l + (size_t)(unsigned)T * FS;
+#pragma unroll
+        for (int f = 0; f < NF; f++) tile_copy_spinor<PREC, 0>(SX + f * STB + sl, xs + f * STB, l);
+        cp_async_commit();
+    }
+    cp_async_wait<(KT != 0) ? 2 : 1>();
     __syncwarp();
     tile_read_hop<PREC, NF, RECON, 0>(r, SZP, LF + 2 * LTB, l, l);
     consume_hop<PREC, NF, RECON, DAG, false, 4>(A, r, c);
     tile_read_hop<PREC, NF, RECON, 0>(r, SZM, LBZ, l, l);
     consume_hop<PREC, NF, RECON, DAG, false, 5>(A, r, c);
-    cp_async_wait<0>();
+    cp_async_wait<(KT != 0) ? 1 : 0>();
     __syncwarp();
     tile_read_hop<PREC, NF, RECON, DAG ? 1 : 2>(r, STP, LF + 3 * LTB, l, l);
     consume_hop<PREC, NF, RECON, DAG, false, 6>(A, r, c);
@@ -181,13 +271,14 @@ __global__ void __launch_bounds__(32, NF == 1 ? TM_TILE_MINB_1 : TM_TILE_MINB_2)
     consume_hop<PREC, NF, RECON, DAG, false, 7>(A, r, c);
 
     // a7, a8: the epilogue and the single store of tm_dslash_f2 (x and out are the warp's own tile: one address)
-    const size_t own = (size_t)T * FS + (size_t)l * 16;
     if constexpr (KT != 0) {
-        issue_spinor<PREC, NF, RECON, 0>(r, static_cast<const char *>(a.x) + own, l);
+        cp_async_wait<0>();
+        __syncwarp();
+        tile_read_spinor<PREC, NF, RECON>(r, SX, l);
         load_x<PREC, NF, RECON>(X, r);
     }
     epilogue_f2<NF, KT>(A, X, (float)a.alpha, (float)a.beta, (float)a.scale, (float)a.kappa, (float)a.kappa2);
-    char *os = static_cast<char *>(a.out) + own;
+    char *os = static_cast<char *>(a.out) + (size_t)T * FS + (size_t)l * 16;
 #pragma unroll
     for (int f = 0; f < NF; f++) store_spinor_f2<PREC>(A + 12 * f, os + f * STB, l);
 }
@@ -202,7 +293,10 @@ cudaError_t tm_launch_tile(const DslashArgs &a, cudaStream_t s)
     tg.lg = a.Xh == 4 ? 2 : a.Xh == 8 ? 3 : 4;
     tg.dtps = tm_fastdiv(tg.tps > 1 ? tg.tps : 2);       // not used when tps == 1
     tg.dZ = tm_fastdiv(a.Z);
-    const size_t smem = (size_t)6 * NF * spinor_tile_bytes(PREC) + (size_t)8 * link_tile_bytes(PREC, RECON);
+    const size_t PB = (size_t)tm_tiles(a.Vh) * 4 * link_tile_bytes(PREC, RECON);
+    tg.gauge_f = static_cast<const char *>(a.gauge) + (size_t)a.parity * PB;
+    tg.gauge_b = static_cast<const char *>(a.gauge) + (size_t)(1 - a.parity) * PB;
+    const size_t smem = (size_t)NF * (4 * spinor_tile_bytes(PREC) + 2 * TM_HALF_TILE) + (size_t)8 * link_tile_bytes(PREC, RECON);
     static std::atomic<unsigned long long> raised{0};
     cudaError_t e = tm_raise_smem(tm_dslash_tile<PREC, NF, RECON, KT, DAG>, raised);
     if (e != cudaSuccess) return e;

@@ -226,7 +226,7 @@ def test_t2f_warp_per_tile_half_kernel_matches_oracle(dims, kw):
         want = oracle.kernel(inp, x, bench.U, po, parity, dagger, kt) if kt < 4 else \
             oracle.hop_xpay(inp, x, bench.U, po, parity, dagger, -KAPPA ** 2 if kt == 4 else KAPPA)
         for recon in RECONS:
-            tm.tm_set_tuning(bench.lat.ctx, "tile_kernel", 1)          # default: on for one flavor; 1 forces it for the doublet too
+            tm.tm_set_tuning(bench.lat.ctx, "tile_kernel", 1)          # (the default where the geometry fits)
             got = bench.kernel(inp, None if kt == 0 else x, pg, parity, dagger, kt, tm.TM_HALF, recon, nf)
             assert tm.tm_last_kernel_name(bench.lat.ctx).startswith("tile<"), tm.tm_last_kernel_name(bench.lat.ctx)
             assert rel_l2(got, want) <= TOL[tm.TM_HALF], (recon, parity, dagger, kt, rel_l2(got, want))
