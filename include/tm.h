@@ -193,6 +193,18 @@ int tm_field_axpby(tm_field *z, double a, const tm_field *x, double b, const tm_
 /* *result (HOST) = Re <x, y> = sum over sites, flavors, spin, color of re x re y + im x im y, accumulated in double in
  * a fixed order (deterministic).  x = y gives |x|^2.  Synchronises the context stream. */
 int tm_field_redot(const tm_field *x, const tm_field *y, double *result);
+/* The same sum for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): *dev_result (DEVICE pointer to one double, the caller's) = Re <x, y>.  Calls no cudaMalloc / cudaFree and no
+ * allocating library routine, copies nothing to the host and does not synchronise: two launches on the context stream.  Its
+ * scratch (per-block partial sums) is a fixed 512 KiB __device__ array inside the library, held by every GPU that loads the
+ * library until the process exits, hence the limit: fields of more than TM_NOALLOC_MAX_SITES sites per parity ->
+ * TM_ERR_UNSUPPORTED (use tm_field_redot).  Same arithmetic and summation order as tm_field_redot: identical result.  Every call
+ * on a device shares the array: calls that OVERLAP on the GPU (two contexts / streams on one device, two host threads) race
+ * and return garbage; calls on one context are ordered by its stream.  The first call on a device looks up the array's
+ * device address (cudaGetSymbolAddress: make one call before starting a capture).  With tm_set_allreduce the hook is applied
+ * to *dev_result. */
+#define TM_NOALLOC_MAX_SITES 8388608L     /* 65536 partial sums x 128 sites; 48^3 x 96 has 5 308 416 sites per parity */
+int tm_field_redot_noalloc(const tm_field *x, const tm_field *y, double *dev_result);
 
 /* Multi-GPU reductions: after tm_set_allreduce(ctx, fn, user) every sum the library forms (tm_field_redot, the scalars of
  * tm_invert_cg) is passed through fn(dev_sums, n, cuda_stream, user): dev_sums is a DEVICE array of n doubles holding this

@@ -34,7 +34,7 @@ EXPORTS = [
     "tm_init", "tm_set_stream", "tm_sync", "tm_finalize", "tm_field_bytes", "tm_field_alloc", "tm_field_free",
     "tm_field_device_ptr", "tm_set_host_basis", "tm_field_upload", "tm_field_download", "tm_field_upload_cb", "tm_field_download_cb", "tm_field_upload_cb_async", "tm_field_download_cb_async", "tm_field_upload_cb_async_f32", "tm_field_download_cb_async_f32",
     "tm_gauge_load", "tm_gauge_free", "tm_dslash_apply", "tm_mat_pc", "tm_reconstruct_odd", "tm_twist_apply",
-    "tm_prepare_rhs", "tm_set_open_time", "tm_set_open_dirs", "tm_halo_bytes", "tm_halo_pack", "tm_halo_apply", "tm_field_axpby", "tm_field_redot", "tm_invert_cg", "tm_cg_release", "tm_set_allreduce", "tm_last_error",
+    "tm_prepare_rhs", "tm_set_open_time", "tm_set_open_dirs", "tm_halo_bytes", "tm_halo_pack", "tm_halo_apply", "tm_field_axpby", "tm_field_redot", "tm_field_redot_noalloc", "tm_invert_cg", "tm_cg_release", "tm_set_allreduce", "tm_last_error",
     "tm_launch_count", "tm_last_kernel_name", "tm_set_path", "tm_set_tuning", "tm_timing_enable", "tm_timing_read",
 ]
 
@@ -115,6 +115,7 @@ def lib():
     L.tm_halo_apply.argtypes = [vp, vp, vp, vp, pp, i, i, i, i, i, i, vp, vp, ctypes.c_uint]
     L.tm_field_axpby.argtypes = [vp, d, vp, d, vp]
     L.tm_field_redot.argtypes = [vp, vp, ctypes.POINTER(d)]
+    L.tm_field_redot_noalloc.argtypes = [vp, vp, vp]
     L.tm_invert_cg.argtypes = [vp, vp, vp, vp, pp, i, ctypes.POINTER(tm_cg_params), ctypes.POINTER(tm_cg_info)]
     L.tm_cg_release.argtypes = [vp]
     L.tm_cg_release.restype = None
@@ -287,6 +288,14 @@ def tm_field_redot(x, y):
     r = ctypes.c_double(0.0)
     _check(lib().tm_field_redot(x, y, ctypes.byref(r)))
     return r.value
+
+
+TM_NOALLOC_MAX_SITES = 8388608      # include/tm.h: sites per parity the fixed scratch array of tm_field_redot_noalloc covers
+
+
+def tm_field_redot_noalloc(x, y, dev_result):
+    """dev_result: DEVICE address of one double (e.g. torch tensor .data_ptr()); nothing is allocated or synchronised."""
+    _check(lib().tm_field_redot_noalloc(x, y, ctypes.c_void_p(int(dev_result))))
 
 
 def tm_invert_cg(x_e, b_e, g_precise, g_sloppy, p, matpc_type, tol, max_iter, sloppy_precision, delta, op=None):

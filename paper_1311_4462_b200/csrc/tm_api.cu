@@ -850,6 +850,19 @@ int tm_field_redot(const tm_field *x, const tm_field *y, double *result)
     return TM_OK;
 }
 
+int tm_field_redot_noalloc(const tm_field *x, const tm_field *y, double *dev_result)
+{
+    if (!x || !y || !dev_result) return fail(TM_ERR_ARG, "tm_field_redot_noalloc: NULL argument");
+    if (x->ctx != y->ctx) return fail(TM_ERR_MISMATCH, "operands belong to different contexts");
+    if (x->nf != y->nf || x->prec != y->prec) return fail(TM_ERR_MISMATCH, "precision or flavor count mismatch");
+    if ((long)x->ctx->g.Vh > TM_NOALLOC_MAX_SITES)
+        return fail(TM_ERR_UNSUPPORTED, "tm_field_redot_noalloc: %d sites per parity exceed the fixed scratch array's maximum of %ld "
+                                        "(TM_NOALLOC_MAX_SITES); use tm_field_redot", x->ctx->g.Vh, TM_NOALLOC_MAX_SITES);
+    cudaError_t e = tm_noalloc_redot(x, y, dev_result);
+    if (e != cudaSuccess) return cuda_fail(e, "tm_field_redot_noalloc");
+    return TM_OK;
+}
+
 namespace {
 
 // Work fields of tm_invert_cg: library-owned device memory kept on the context between solves (zero-filled once so that tile

@@ -183,6 +183,11 @@ cudaError_t tm_blas_redot_dev(const tm_field *x, const tm_field *y, double *out,
 cudaError_t tm_blas_cg_update_dev(tm_field *x, tm_field *r, const tm_field *p, const tm_field *Ap, double a, double *rr,
                                   const double *anum, const double *aden, double *dev_rr);
 
+// Re <x, y> with its scratch in a fixed __device__ array (tm_noalloc.cu): no allocation, result left in DEVICE memory
+#define TM_NOALLOC_BLOCK 128
+#define TM_NOALLOC_MAX_BLOCKS ((int)(TM_NOALLOC_MAX_SITES / TM_NOALLOC_BLOCK))
+cudaError_t tm_noalloc_redot(const tm_field *x, const tm_field *y, double *dev_out);
+
 // surface kernels of the domain decomposition (tm_halo.cu); dir = 1 (y), 2 (z), 3 (t)
 cudaError_t tm_launch_halo_pack(const tm_field *in, const tm_gauge *g, int out_parity, int dagger, int dir, void *to_prev, void *to_next,
                                 unsigned *flag_prev, unsigned *flag_next, unsigned epoch, unsigned *counter, cudaStream_t s);
