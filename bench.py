@@ -96,12 +96,32 @@ def measured_peak():
 
 
 class ClockSampler:
-    """nvidia-smi clocks + throttle reasons while the GPU is under load (B200_PROFILING.md clocks line)."""
+    """SM clock, throttle reasons and board power while the GPU is under load (B200_PROFILING.md clocks line), sampled through NVML
+    every 2 ms from a thread (the power limiter of the board acts within tens of milliseconds: nvidia-smi's 20 ms loop sees 3-4
+    samples of a 75 ms region and misses the dips); falls back to an `nvidia-smi -lms 20` subprocess when pynvml is missing."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    REASONS = ((0x8, "hw_slowdown"), (0x40, "hw_thermal_slowdown"), (0x20, "sw_thermal_slowdown"), (0x4, "sw_power_cap"),
+               (0x80, "hw_power_brake_slowdown"))
 
     def __init__(self, index):
-        self.rows, self.proc = [], None
+        self.rows, self.proc, self.nv, self.samples, self.halt = [], None, None, [], False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            idx = str(index)
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(int(idx)) if idx.isdigit() else pynvml.nvmlDeviceGetHandleByUUID(idx)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            try:
+                self.limit_w = pynvml.nvmlDeviceGetEnforcedPowerLimit(self.h) / 1e3
+            except Exception:
+                self.limit_w = None
+            self.nv = pynvml
+            self.th = threading.Thread(target=self._poll, daemon=True)
+            self.th.start()
+            return
+        except Exception:
+            self.nv = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
                                           "-lms", "20", "-i", str(index)], stdout=subprocess.PIPE,
@@ -111,11 +131,45 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
+    def _poll(self):
+        nv = self.nv
+        while not self.halt:
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                watts = nv.nvmlDeviceGetPowerUsage(self.h) / 1e3            # the driver's average over about 100 ms
+                try:                                                        # the instantaneous figure shows the cap tens of ms earlier
+                    inst = nv.nvmlDeviceGetFieldValues(self.h, [nv.NVML_FI_DEV_POWER_INSTANT])[0].value.uiVal / 1e3
+                except Exception:
+                    inst = None
+                self.samples.append((time.time(), float(mhz), int(mask), watts, inst))
+            except Exception:
+                pass
+            time.sleep(0.002)
+
     def _read(self):
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
     def stop(self, t0, t1):
+        if self.nv is not None:
+            time.sleep(0.01)
+            self.halt = True
+            self.th.join(timeout=2)
+            rows = [r for r in self.samples if t0 <= r[0] <= t1] or self.samples[-3:]
+            if not rows:
+                return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["no NVML samples"]}
+            sm = [r[1] for r in rows]
+            mask = 0
+            for r in rows:
+                mask |= r[2]
+            return {"sm_mhz": float(np.median(sm)), "sm_min_mhz": min(sm), "sm_max_mhz": self.max_mhz,
+                    "reasons": sorted(n for b, n in self.REASONS if mask & b), "samples": len(sm), "power_max_w": max(r[3] for r in rows),
+                    "power_instant_max_w": max([r[4] for r in rows if r[4] is not None], default=None),
+                    "power_limit_w": self.limit_w, "source": "NVML, 2 ms period"}
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.05)
@@ -138,7 +192,7 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "source": "nvidia-smi -lms 20"}
 
 
 def reduce_over_ranks(ms_local, world):
@@ -698,9 +752,10 @@ def run_ours(args, log):
     barrier()
     ms_local = ev0.elapsed_time(ev1)
     launches = lat.launches() - n0
-    # the same K steps again with a CUDA event pair around every launch (tm_timing_enable): the per-kernel durations of the roofline.
-    # The event records cost about 5 us per launch (gaps between kernels + start latency inside each pair), which is why they
-    # are kept out of the region the headline value is taken from; both regions are reported.
+    # the same K steps again with one CUDA event between consecutive launches (tm_timing_enable(ctx, 2): a launch's interval runs from
+    # its predecessor's stop event to its own, so the per-kernel durations of the roofline tile the region without gaps and add up to
+    # ms_per_step_with_launch_events).  An event record between two kernels still costs 1-2 us of front-end time (an event PAIR around
+    # every launch cost 5 us), which is why the headline value is taken from the region without them; both are reported.
     # (half a second of idle and the warm-up steps again first: the board's power limiter acts on a window of about 100 ms, and the
     # second region should start from the same state as the first, not 90 ms into it)
     t1 = time.time()
@@ -708,7 +763,7 @@ def run_ours(args, log):
     for _ in range(max(args.warmup, 3)):
         w.step()
     barrier()
-    tm.tm_timing_enable(lat.ctx, 1)
+    tm.tm_timing_enable(lat.ctx, 2)
     ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev2.record()
     for _ in range(args.steps):
@@ -719,6 +774,27 @@ def run_ours(args, log):
     records = tm.tm_timing_read(lat.ctx, 1 << 20)
     tm.tm_timing_enable(lat.ctx, 0)
     clocks = sampler.stop(t0, t1)
+    # ---- the same step in the board's sustained state.  This step draws the board's full power limit (NVML instantaneous power at the
+    # 1000 W limit): after an idle the board runs about 50 ms at its maximum clocks, then the limiter lowers the SM clock in two or three
+    # stages to ~1.5 GHz (sw_power_cap; profiles/r2_tuning.md section 7).  The default K = 30 timed steps lie mostly inside that first window,
+    # as the burst figure of MEASURED_PEAKS.json does; `sustained` reports what a long run gets: 60 untimed steps, then 100 timed ones.
+    sustained = None
+    if not args.no_sustained:
+        for _ in range(60):
+            w.step()
+        barrier()
+        s_sampler = ClockSampler(smi_index)
+        ts0 = time.time()
+        ev4, ev5 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev4.record()
+        for _ in range(100):
+            w.step()
+        ev5.record()
+        barrier()
+        ts1 = time.time()
+        s_ms = reduce_over_ranks(ev4.elapsed_time(ev5), world) / 100
+        sustained = {"ms_per_step": s_ms, "value": world * step_flops / (s_ms * 1e-3) / 1e9, "unit": "GFLOPS", "steps": 100, "after_untimed_steps": 60,
+                     "clocks": s_sampler.stop(ts0, ts1)}
     ms = reduce_over_ranks(ms_local, world)
     ms_per_step = ms / args.steps
     value = world * step_flops / (ms_per_step * 1e-3) / 1e9
@@ -811,7 +887,7 @@ def run_ours(args, log):
                           if args.sharded else ("replicas only (north_star: no sharding)" if world > 1 else "single GPU"),
                           "l2": "inputs larger than L2 (gauge fields 201-805 MB each, 2.3 GB touched per step)",
                           "tune": args.tune or "defaults"},
-               "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+               "roofline": roofline, "sustained": sustained, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                "step_flops": step_flops, "step_alg_bytes": step_bytes, "kernels": kernels, "kernels_extra": extra, "cg": cg, "config5": c5,
                "paper_table1_gflops_12real": {"%s/%s" % ("deg" if k[0] == 1 else "ndeg", PREC_NAME[k[1]]): v
                                               for k, v in PAPER_GFLOPS.items()},
@@ -836,6 +912,7 @@ def main():
     ap.add_argument("--dims", default="32,32,32,64", help="--kernels: lattice extents")
     ap.add_argument("--tune", default="", help="tm_set_tuning overrides, key=value[,...] (non-default values are recorded in config.tune)")
     ap.add_argument("--config5", action="store_true", help="time BASELINE.json configs[4] instead (48^3x96 fp64 doublet, Eq. 2.3 operator x 100; ~25 GB of host memory)")
+    ap.add_argument("--no-sustained", action="store_true", help="skip the `sustained` leg (100 timed steps in the board's power-limited state)")
     ap.add_argument("--no-extra", action="store_true", help="skip the kernels_extra table (every kernel type x precision x compression, timed alone)")
     ap.add_argument("--sass-mix", action="store_true", help="host only: write profiles/sass_mix.csv + profiles/r2_sass_histogram.md from the built objects")
     ap.add_argument("--import-ncu", metavar="CSV", help="host only: turn an `ncu --csv --page raw` export of this build into profiles/traffic.csv")

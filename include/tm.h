@@ -299,7 +299,11 @@ long tm_launch_count(const tm_ctx *ctx);
 const char *tm_last_kernel_name(const tm_ctx *ctx);
 /* Per-launch device timing (bench.py's roofline leg): while enabled, every dslash launch is bracketed by CUDA
  * events on the context stream.  tm_timing_read synchronises, writes up to max_records (kernel name, milliseconds)
- * pairs in launch order into the HOST arrays names / ms, stores the number written in *n, and clears the log. */
+ * pairs in launch order into the HOST arrays names / ms, stores the number written in *n, and clears the log.
+ * on = 1: an event pair around every launch (start, launch, stop).  on = 2: ONE event between consecutive launches -- a launch's
+ * interval runs from its predecessor's stop event to its own, so the intervals tile the stream without gaps (whatever else the
+ * caller enqueues between two dslash launches is charged to the later one) and cost half the event records; the first launch
+ * after enabling or reading records its own start.  on = 0: off, the log is dropped. */
 int tm_timing_enable(tm_ctx *ctx, int on);
 int tm_timing_read(tm_ctx *ctx, int max_records, const char **names, float *ms, int *n);
 /* Force a code path: 0 = automatic (default), 1 = generic direct-load kernels only.  For tests / profiling. */

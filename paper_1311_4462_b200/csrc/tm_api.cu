@@ -209,6 +209,7 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->open_mask = 0;
     c->halo_counter = nullptr;
     c->timing = false;
+    c->timing_chain = false;
     e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
     if (e != cudaSuccess) { delete c; return cuda_fail(e, "cudaDeviceGetAttribute"); }
     *ctx = c;
@@ -255,21 +256,23 @@ void tm_finalize(tm_ctx *ctx)
     if (ctx->cgs) cudaFree(ctx->cgs);
     if (ctx->halo_counter) cudaFree(ctx->halo_counter);
     if (ctx->cgs_host) cudaFreeHost(ctx->cgs_host);
-    for (auto &t : ctx->timed) { cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
+    for (auto &t : ctx->timed) { if (t.own_start) cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
     delete ctx;
 }
 
 static void clear_timed(tm_ctx *ctx)
 {
-    for (auto &t : ctx->timed) { cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
+    for (auto &t : ctx->timed) { if (t.own_start) cudaEventDestroy(t.start); cudaEventDestroy(t.stop); }
     ctx->timed.clear();
 }
 
 int tm_timing_enable(tm_ctx *ctx, int on)
 {
     if (!ctx) return fail(TM_ERR_ARG, "tm_timing_enable: NULL context");
+    if (on < 0 || on > 2) return fail(TM_ERR_ARG, "tm_timing_enable: on must be 0, 1 or 2");
+    if (on == 0 || (on == 2) != ctx->timing_chain) clear_timed(ctx);
     ctx->timing = on != 0;
-    if (!ctx->timing) clear_timed(ctx);
+    ctx->timing_chain = on == 2;
     return TM_OK;
 }
 
@@ -668,9 +671,14 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     if (c->timing) {
         tm_ctx::TimedLaunch t;
         t.name = k.name;
-        if ((e = cudaEventCreate(&t.start)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
-        if ((e = cudaEventCreate(&t.stop)) != cudaSuccess) { cudaEventDestroy(t.start); return cuda_fail(e, "cudaEventCreate"); }
-        cudaEventRecord(t.start, c->stream);
+        t.own_start = !(c->timing_chain && !c->timed.empty());
+        if (t.own_start) {
+            if ((e = cudaEventCreate(&t.start)) != cudaSuccess) return cuda_fail(e, "cudaEventCreate");
+        } else {
+            t.start = c->timed.back().stop;            // chained: the event between the previous launch and this one
+        }
+        if ((e = cudaEventCreate(&t.stop)) != cudaSuccess) { if (t.own_start) cudaEventDestroy(t.start); return cuda_fail(e, "cudaEventCreate"); }
+        if (t.own_start) cudaEventRecord(t.start, c->stream);
         e = k.fn(a, c->stream);
         cudaEventRecord(t.stop, c->stream);
         c->timed.push_back(t);

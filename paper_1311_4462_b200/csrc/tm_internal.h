@@ -62,7 +62,8 @@ struct tm_ctx {
     size_t red_n;
     size_t staging_bytes;
     bool timing;          // tm_timing_enable
-    struct TimedLaunch { cudaEvent_t start, stop; const char *name; };
+    bool timing_chain;    // tm_timing_enable(ctx, 2): one event BETWEEN consecutive launches (a launch's start is its predecessor's stop)
+    struct TimedLaunch { cudaEvent_t start, stop; const char *name; bool own_start; };
     std::vector<TimedLaunch> timed;
 };
 

@@ -701,6 +701,41 @@ def test_t5_host_spin_basis_chiral_and_custom():
 
 # ---- T6: error paths of the boundary --------------------------------------------------------------
 
+def test_t8_launch_timing_modes_pair_and_chained():
+    """tm_timing_enable: 1 = an event pair around every launch, 2 = one event between consecutive launches (intervals tile the stream)."""
+    import torch
+    dims = (16, 16, 16, 16)
+    lat = tm.Lattice(dims)
+    kw = FLAVORS[0]
+    pg = tm.params(KAPPA, **kw)
+    g = lat.gauge(si.gauge_field(dims, 5, "haar"), tm.TM_SINGLE, tm.TM_RECON_12)
+    f = [lat.field(tm.TM_SINGLE, 1) for _ in range(3)]
+    f[0].upload(0, si.mask_parity(si.spinor_field(dims, 1, 6), dims, 0))
+    ref = None
+    for mode in (1, 2):
+        tm.tm_timing_enable(lat.ctx, mode)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(lat.stream)
+        for _ in range(10):
+            tm.mat_pc(f[1], f[0], f[2], g, pg, tm.TM_MATPC_ASYM, 0)         # two launches
+        e1.record(lat.stream)
+        rec = tm.tm_timing_read(lat.ctx)
+        total = e0.elapsed_time(e1)
+        assert len(rec) == 20 and all(ms > 0 for _, ms in rec)
+        assert [n for n, _ in rec[:2]] * 10 == [n for n, _ in rec]
+        assert sum(ms for _, ms in rec) <= total * 1.001 + 1e-3                # the intervals lie inside the bracket and do not overlap
+        assert tm.tm_timing_read(lat.ctx) == []                                # the read clears the log
+        tm.mat_pc(f[1], f[0], f[2], g, pg, tm.TM_MATPC_ASYM, 0)             # after a read the chain starts afresh
+        assert len(tm.tm_timing_read(lat.ctx)) == 2
+        tm.tm_timing_enable(lat.ctx, 0)
+        out = f[1].download(0)
+        if ref is None:
+            ref = out
+        assert np.array_equal(out, ref)                                        # timing never changes results
+    with pytest.raises(tm.TmError):
+        tm.tm_timing_enable(lat.ctx, 3)
+
+
 def test_t6_error_paths():
     dims = (4, 4, 4, 8)
     bench = bench_for(dims, "haar", 1)
