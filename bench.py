@@ -756,10 +756,11 @@ def run_ours(args, log):
     # its predecessor's stop event to its own, so the per-kernel durations of the roofline tile the region without gaps and add up to
     # ms_per_step_with_launch_events).  An event record between two kernels still costs 1-2 us of front-end time (an event PAIR around
     # every launch cost 5 us), which is why the headline value is taken from the region without them; both are reported.
-    # (half a second of idle and the warm-up steps again first: the board's power limiter acts on a window of about 100 ms, and the
-    # second region should start from the same state as the first, not 90 ms into it)
+    # (a second of idle and the warm-up steps again first: the board grants its maximum clocks for about 50 ms after an idle before the
+    # power limiter steps in (profiles/r2_tuning.md section 7), and the second region should start from the same state as the first,
+    # not 90 ms into it; `sustained` below reports the other state)
     t1 = time.time()
-    time.sleep(0.5)
+    time.sleep(1.0)
     for _ in range(max(args.warmup, 3)):
         w.step()
     barrier()
