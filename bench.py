@@ -787,7 +787,7 @@ def run_ours(args, log):
     for _ in range(max(args.warmup, 3)):
         w.step()
     barrier()
-    tm.tm_timing_enable(lat.ctx, 2)
+    tm.tm_timing_enable(lat.ctx, 1 if args.sharded else 2)      # --sharded: halo kernels run between the dslash launches: event pairs
     ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev2.record()
     for _ in range(args.steps):
