@@ -99,7 +99,11 @@ int tm_set_stream(tm_ctx *ctx, void *cuda_stream);
 int tm_sync(tm_ctx *ctx);           /* cudaStreamSynchronize; surfaces asynchronous faults */
 void tm_finalize(tm_ctx *ctx);      /* does not free fields / gauges created from it */
 
-/* ---- fields (a1 of DESIGN.md: checkerboarded SoA layouts) ------------------------------------------ */
+/* ---- fields (a1 of DESIGN.md: checkerboarded SoA layouts) ------------------------------------------
+ * A field is one parity of a spinor -- the operands of the even-odd preconditioned operators of PAPER.md:56-66 (Eq. 2.2-2.4
+ * act on psi_e / psi_o) --, with n_flavor = 1 for the degenerate doublet (epsilon = 0 in Eq. 2.1: the flavors
+ * decouple) or 2 for the non-degenerate one ("one has to apply the dslash on both flavors"), in one of the three
+ * storage precisions of Table 1. */
 size_t tm_field_bytes(const tm_ctx *ctx, tm_precision prec, int n_flavor);   /* 0 on bad arguments */
 /* ext_dev_ptr == NULL: the library allocates (and frees in tm_field_free).  Otherwise ext_dev_ptr is DEVICE
  * memory of at least tm_field_bytes() bytes, 256-byte aligned, BORROWED (e.g. a torch tensor's storage). */
@@ -146,7 +150,9 @@ typedef enum { TM_BASIS_NONREL = 0, TM_BASIS_CHIRAL = 1, TM_BASIS_CUSTOM = 2 } t
 int tm_set_host_basis(tm_ctx *ctx, tm_basis basis, const double *custom);
 
 /* ---- gauge (a1, a4) -------------------------------------------------------------------------------- */
-/* host_links: HOST pointer, canonical gauge field; copied (may be freed on return). */
+/* The gauge links U_mu(x) of the Wilson term D_W (Eq. 2.1; "re-use the gauge field"), stored per parity in the precision of the kernels
+ * that read them and in one of the compressed forms of PAPER.md:97 ("12 or 8 parameter reconstruct"; 18 = uncompressed).
+ * host_links: HOST pointer, canonical gauge field; copied (may be freed on return). */
 int tm_gauge_load(tm_ctx *ctx, const double *host_links, tm_precision prec, tm_recon recon, tm_gauge **g);
 void tm_gauge_free(tm_gauge *g);
 
