@@ -321,6 +321,8 @@ int tm_set_path(tm_ctx *ctx, int path);
  *   loads, -1 = library default;   "block_threads": 32 / 64 / 128 sites per thread block, 0 = library default;
  *   "z_chunks": the thread blocks walk the lattice in n chunks of Z / n z-planes (all time slices of a chunk first) so that
  *   the input spinor's reuse window fits the L2; -1 = library default (from the size of three time slices);
+ *   "pdl": 1 (default) = the fused kernels are launched with the programmatic-stream-serialization attribute (each waits with
+ *   griddepcontrol.wait for its predecessor before touching a field; hides the launch gap, 1 % of a 20-launch step), 0 = plain launches;
  *   "tile_kernel": half precision, 18- / 12-real links: 0 = thread-per-site kernels only, 1 or -1 (default) = the warp-per-tile
  *   kernel wherever the geometry fits (X/2 in {4, 8, 16}, Y a multiple of 64/X); both give bit-identical results.
  *   Unknown key or bad value -> TM_ERR_ARG. */

@@ -188,6 +188,7 @@ int tm_init(const int dims[4], int cuda_device, tm_ctx **ctx)
     c->stage = -1;
     c->z_chunks = -1;
     c->tile_kernel = -1;
+    c->pdl = 1;
     c->block_threads = 0;
     c->sm_count = 0;
     c->basis_on = 0;
@@ -352,6 +353,11 @@ int tm_set_tuning(tm_ctx *ctx, const char *key, int value)
     if (!strcmp(key, "stage_links")) {
         if (value < -1 || value > 1) return fail(TM_ERR_ARG, "stage_links must be -1 (default), 0 or 1");
         ctx->stage = value;
+        return TM_OK;
+    }
+    if (!strcmp(key, "pdl")) {
+        if (value < 0 || value > 1) return fail(TM_ERR_ARG, "pdl must be 0 or 1");
+        ctx->pdl = value;
         return TM_OK;
     }
     if (!strcmp(key, "tile_kernel")) {
@@ -633,6 +639,7 @@ int tm_dslash_apply(tm_field *out, const tm_field *in, const tm_field *x, const 
     // L2 prefetch of the tiles 8 blocks ahead (tm_stream.cuh), where it measured faster at both 32^3 x 64 and 48^3 x 96 (profiles/r2_tuning.md
     // section 5): the fp32 doublet kernels (+6..11 %), the fp64 kernels without an x input (+2..5 %), the fp64 doublet with 12-real links
     const bool pf_on = ((int)prec == TM_SINGLE && out->nf == 2) || ((int)prec == TM_DOUBLE && (kcode == 0 || (out->nf == 2 && g->recon == 12)));
+    a.pdl = c->pdl;
     a.pf_dist = c->pf_dist >= 0 ? c->pf_dist : (pf_on ? 8 : 0);
     int stage = c->stage >= 0 ? c->stage : ((int)prec == TM_HALF ? 1 : 0);
     a.block_threads = c->block_threads ? c->block_threads : 128;

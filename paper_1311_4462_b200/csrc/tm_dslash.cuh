@@ -218,6 +218,7 @@ template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, bool TWIN = f
 __global__ void __launch_bounds__(128, (PREC == 8 && NF == 1 && !STG) ? (RECON == 18 ? 2 : TM_MINB_8_1) : (PREC == 8 ? 2 : 1)) tm_dslash_generic(const DslashArgs a)
 {
     typedef typename PrecTraits<PREC>::real real;
+    tm_pdl_enter();
     const int Vh = a.Vh;
     const int vblock = tm_virtual_block(a, blockIdx.x);
     prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, vblock);
@@ -304,8 +305,7 @@ cudaError_t tm_launch_generic(const DslashArgs &a, cudaStream_t s)
         cudaError_t e = tm_raise_smem(tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG, TWIN>, raised);
         if (e != cudaSuccess) return e;
     }
-    tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG, TWIN><<<blocks, threads, smem, s>>>(a);
-    return cudaGetLastError();
+    return tm_launch_kernel(tm_dslash_generic<PREC, NF, RECON, KT, DAG, STG, TWIN>, a.pdl, blocks, threads, smem, s, a);
 }
 
 // table index: [recon 18 / 12 / 8 -> 0 / 1 / 2][kt 0..3][dagger 0..1][staged 0..1]; 8-real links are never staged

@@ -564,6 +564,7 @@ template <int PREC, int NF, int RECON, int KT, bool DAG, bool STG, bool TWIN = f
 __global__ void __launch_bounds__(128, f2_min_blocks<PREC, NF>()) tm_dslash_f2(const DslashArgs a)
 {
     constexpr int PD = f2_pipeline_depth<PREC, NF>();
+    tm_pdl_enter();
     const int Vh = a.Vh;
     const int vblock = tm_virtual_block(a, blockIdx.x);
     prefetch_tile<PREC, NF, RECON, KT != 0>(a, blockDim.x, vblock);
@@ -626,8 +627,7 @@ cudaError_t tm_launch_f2(const DslashArgs &a, cudaStream_t s)
         cudaError_t e = tm_raise_smem(tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG, TWIN>, raised);
         if (e != cudaSuccess) return e;
     }
-    tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG, TWIN><<<blocks, threads, smem, s>>>(a);
-    return cudaGetLastError();
+    return tm_launch_kernel(tm_dslash_f2<PREC, NF, RECON, KT, DAG, STG, TWIN>, a.pdl, blocks, threads, smem, s, a);
 }
 
 // table index: [recon18?0:1][kt 0..3][dagger 0..1][staged 0..1]

@@ -139,6 +139,7 @@ __global__ void __launch_bounds__(32, NF == 1 ? TM_TILE_MINB_1 : TM_TILE_MINB_2)
 
     // a2, per warp: the tile's place on the lattice and its neighbour tiles (functions of blockIdx: uniform)
     const int T = blockIdx.x, l = threadIdx.x;
+    tm_pdl_enter();
     const int Xh = tg.Xh, R = tg.R, tps = tg.tps;
     const int slab = tps == 1 ? T : tm_div(T, tg.dtps), tin = T - slab * tps;
     const int t = tm_div(slab, tg.dZ), z = slab - t * a.Z;
@@ -300,8 +301,7 @@ cudaError_t tm_launch_tile(const DslashArgs &a, cudaStream_t s)
     static std::atomic<unsigned long long> raised{0};
     cudaError_t e = tm_raise_smem(tm_dslash_tile<PREC, NF, RECON, KT, DAG>, raised);
     if (e != cudaSuccess) return e;
-    tm_dslash_tile<PREC, NF, RECON, KT, DAG><<<a.Vh / TM_TILE, 32, smem, s>>>(a, tg);
-    return cudaGetLastError();
+    return tm_launch_kernel(tm_dslash_tile<PREC, NF, RECON, KT, DAG>, a.pdl, a.Vh / TM_TILE, 32, smem, s, a, tg);
 }
 // the lattices the tile kernel covers (tm_dslash_apply falls back to the thread-per-site kernels otherwise)
 inline bool tm_tile_geometry_ok(int Xh, int Y, int Vh) { return (Xh == 4 || Xh == 8 || Xh == 16) && Y % (32 / Xh) == 0 && Vh % TM_TILE == 0; }

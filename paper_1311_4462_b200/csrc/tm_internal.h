@@ -37,6 +37,7 @@ struct tm_ctx {
     int pf_dist; // tm_set_tuning("prefetch_blocks")
     int stage;   // tm_set_tuning("stage_links"): -1 library default, 0 direct loads, 1 links staged through shared memory
     int block_threads;   // tm_set_tuning("block_threads"): 0 library default, else 32 / 64 / 128
+    int pdl;             // tm_set_tuning("pdl"): 1 (default) = fused kernels are launched with programmatic stream serialization, 0 = plain launches
     int tile_kernel;     // tm_set_tuning("tile_kernel"): -1 library default (on where the geometry allows), 0 off, 1 on
     int z_chunks;        // tm_set_tuning("z_chunks"): -1 library default (from the L2 working set), else the number of z-chunks
     int sm_count;
@@ -119,6 +120,7 @@ struct DslashArgs {
     double alpha;        // local twist, flavor 0:  w = scale * (v + i alpha gamma5 v + beta v_otherflavor)
     double beta;
     double scale;
+    int pdl;             // launch with programmatic stream serialization (the kernels call griddepcontrol themselves)
     double alpha_in, beta_in, scale_in;   // TWIN kernels: the twist applied to the input sites (same form as alpha / beta / scale)
     double kappa;        // REC
     double kappa2;       // A-xpay, B
@@ -159,6 +161,25 @@ inline cudaError_t tm_raise_smem(K kernel, std::atomic<unsigned long long> &done
     e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     if (e == cudaSuccess && dev < 64) done.fetch_or(bit, std::memory_order_relaxed);
     return e;
+}
+
+// Launch of a fused dslash kernel.  pdl != 0: with the programmatic-stream-serialization attribute, so that the launch is set up on the
+// GPU while the previous kernel of the stream still runs (every fused kernel executes griddepcontrol.wait before its first access to a
+// field and none triggers its dependents early: execution order = that of plain launches, tm_stream.cuh).
+template <class... KArgs, class... Args>
+inline cudaError_t tm_launch_kernel(void (*kernel)(KArgs...), int pdl, unsigned grid, unsigned block, size_t smem, cudaStream_t s, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
 // kernel launchers (one translation unit per precision x flavor count)

@@ -11,6 +11,17 @@
 #include "tm_internal.h"
 #include "tm_layout.cuh"
 
+// Programmatic dependent launch (tm_launch_kernel, tm_internal.h).  tm_pdl_enter() is the first statement of every fused kernel: with the
+// launch attribute the kernel may be set up on the GPU while the previous kernel of the stream is still running, and this instruction
+// then holds it until that kernel has completed and its writes are visible -- before any field is read or written.  No kernel signals
+// griddepcontrol.launch_dependents early (measured: blocks of the next kernel resident during the last wave make the step 25 % slower,
+// profiles/r2_tuning.md section 10), so the order of execution is that of plain launches; what is saved is the launch gap (1.1 % of the
+// step).  A no-op in a kernel launched without the attribute.
+TM_DEV void tm_pdl_enter()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 template <int PREC, int NF, int RECON, bool HAS_X>
 TM_DEV void prefetch_tile(const DslashArgs &a, int sites_per_block, int vblock)
 {
