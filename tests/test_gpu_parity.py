@@ -54,6 +54,7 @@ def bench_for(dims, kind, seed):
     tm.tm_set_tuning(ctx, "prefetch_blocks", -1)
     tm.tm_set_tuning(ctx, "z_chunks", -1)
     tm.tm_set_tuning(ctx, "tile_kernel", -1)
+    tm.tm_set_tuning(ctx, "pdl", 1)
     return _cache[key]
 
 
@@ -734,6 +735,35 @@ def test_t8_launch_timing_modes_pair_and_chained():
         assert np.array_equal(out, ref)                                        # timing never changes results
     with pytest.raises(tm.TmError):
         tm.tm_timing_enable(lat.ctx, 3)
+
+
+@pytest.mark.parametrize("kw", [FLAVORS[0], FLAVORS[2]], ids=["deg+", "ndeg"])
+def test_t10_programmatic_dependent_launch_keeps_the_order_of_dependent_kernels(kw):
+    """tm_set_tuning("pdl"): the fused kernels are launched with programmatic stream serialization and wait (griddepcontrol.wait) for
+    their predecessor before touching a field.  A chain of kernels in which each reads what the previous one wrote, and overwrites what
+    the one before that read (RAW and WAR through the same stream), must give bit for bit the results of plain launches -- at a size
+    with several waves of blocks (16^3 x 32: 512 blocks of 128 sites, 2048 tiles), in every precision."""
+    dims, nf = (16, 16, 16, 32), nf_of(kw)
+    lat = tm.Lattice(dims)
+    pg = tm.params(KAPPA, **kw)
+    U = si.gauge_field(dims, 21, "haar")
+    x = si.mask_parity(si.spinor_field(dims, nf, 22), dims, 0)
+    for prec in PRECS:
+        g = lat.gauge(U, prec, tm.TM_RECON_12)
+        f = [lat.field(prec, nf) for _ in range(3)]
+        res = {}
+        for pdl in (0, 1):
+            tm.tm_set_tuning(lat.ctx, "pdl", pdl)
+            f[0].upload(0, x)
+            for _ in range(6):                       # e -> o -> e -> o ...: f0 -> f1 -> f2 -> f0 -> ... each launch reads the previous output
+                tm.dslash_apply(f[1], f[0], None, g, pg, 1, 0, 0)
+                tm.dslash_apply(f[2], f[1], f[0], g, pg, 0, 0, 2)
+                tm.dslash_apply(f[0], f[2], f[1], g, pg, 1, 1, 1)
+            res[pdl] = [f[k].download(p) for k, p in ((0, 1), (1, 1), (2, 0))]
+        for a, b in zip(res[0], res[1]):
+            assert np.isfinite(a).all() and np.array_equal(a, b), PREC_NAME[prec]
+    with pytest.raises(tm.TmError):
+        tm.tm_set_tuning(lat.ctx, "pdl", 2)
 
 
 def test_t9_composites_are_cuda_graph_capturable():
